@@ -1,0 +1,190 @@
+/*
+ * tpcclus.h -- C ABI of libtpcclus.so, the B200-native (sm_100a) TPC clusterizer.
+ *
+ * The hot path behind this boundary is the one BASELINE.json north_star (NS) names, the
+ * data-parallel front of the TPC online processing of arxiv/paper_2511_17018 (PAPER.md
+ * lines 8 and 18: ">95 %" of the online workload, "highly parallelizable"):
+ *
+ *   zero-suppressed digits -> pad x time charge map -> 3x3 peaks above threshold ->
+ *   peak noise suppression -> 5x5 centre-of-gravity clusters -> compaction -> sort.
+ *
+ * The paper never spells the algorithm out; every rule is fixed in SURVEY.md 8(c),
+ * steps O0..O5 and readings Q1..Q23 (restated in DESIGN.md).  The paper contributes the
+ * run modes: the deterministic mode (PAPER.md 24-50, section 2), run-time compilation
+ * with constants baked in (PAPER.md 87-93, section 5) and constant-memory parameters
+ * that may change between time frames (PAPER.md 79-85, section 4.1).
+ *
+ * Plain C: no exception crosses this boundary, no torch / C++ type appears in it.
+ * Every pointer is marked HOST or DEVICE.  All device memory (digits, clusters,
+ * counters, workspace) is owned by the caller; the handle owns host state, the
+ * uploaded parameters and, for RTC handles, the NVRTC-built module.
+ */
+#ifndef TPCCLUS_H
+#define TPCCLUS_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TPCCLUS_API __attribute__((visibility("default")))
+
+typedef struct tpcclus_handle tpcclus_handle; /* opaque, owned by the library */
+
+/* Zero-suppressed digit, 8 bytes, little-endian, one 64-bit load.
+ * charge: ADC, 10 bit; > 1023 is clamped to 1023, 0 is ignored (Q4).
+ * Out-of-range sector/row/pad/time: the digit is ignored and BAD_DIGITS is raised (Q4).
+ * Two digits on one cell: the larger charge wins in DETERMINISTIC mode; in FAST mode
+ * either may win (Q5).  The digit array may be in ANY order (NS (5)). */
+typedef struct {
+  uint16_t charge;
+  uint16_t time;   /* 0 .. n_time-1        */
+  uint8_t pad;     /* 0 .. n_pads[row]-1   */
+  uint8_t row;     /* 0 .. n_rows-1        */
+  uint8_t sector;  /* 0 .. n_sectors-1     */
+  uint8_t reserved; /* ignored on input    */
+} tpcclus_digit;
+
+/* Cluster, 32 bytes (fields per O3/O4).  Cell (p,t) has its centre at the
+ * integer (p,t); means and sigmas are in bins (Q11, Q13). */
+typedef struct {
+  float pad_mean;    /* p_c + Sp/Q                      */
+  float time_mean;   /* t_c + St/Q                      */
+  float sigma_pad;   /* sqrt(Q*Spp - Sp^2)/Q            */
+  float sigma_time;  /* sqrt(Q*Stt - St^2)/Q            */
+  uint32_t q_tot;    /* Q: sum over the clipped 5x5     */
+  uint16_t q_max;    /* charge of the peak cell         */
+  uint16_t time_peak;
+  uint8_t pad_peak, row, sector;
+  uint8_t flags;     /* TPCCLUS_FLAG_*                  */
+  uint32_t reserved; /* always 0; part of the byte compare */
+} tpcclus_cluster;
+
+enum {
+  TPCCLUS_FLAG_EDGE_PAD = 1,  /* p_c < 2 or p_c + 2 >= n_pads[row] */
+  TPCCLUS_FLAG_EDGE_TIME = 2, /* t_c < 2 or t_c + 2 >= n_time      */
+  TPCCLUS_FLAG_SATURATED = 4  /* q_max == 1023                     */
+};
+
+/* run modes (NS (5); PAPER.md 28-50) */
+enum {
+  TPCCLUS_MODE_FAST = 0,          /* cluster order unspecified; every field as in DETERMINISTIC */
+  TPCCLUS_MODE_DETERMINISTIC = 1  /* ascending (sector,row,time_peak,pad_peak); bitwise equal to
+                                     the host oracle, invariant under input permutation and
+                                     across runs (PAPER.md 26-28, 36, 47-48) */
+};
+
+/* create flags */
+enum {
+  TPCCLUS_RTC = 1 /* build the kernels with NVRTC at create(), geometry and thresholds baked
+                     in as literals (PAPER.md 89-93); without it the offline-compiled kernels
+                     read them from __constant__ memory (PAPER.md 79-85) */
+};
+
+/* data-dependent conditions, OR-ed into *status on the device (never return codes) */
+enum {
+  TPCCLUS_STATUS_OVERFLOW = 1,  /* more clusters than out->capacity; *n_clusters is still the
+                                   true total, the buffer holds `capacity` valid records (FAST:
+                                   any subset; DETERMINISTIC: the first `capacity` in order) */
+  TPCCLUS_STATUS_BAD_DIGITS = 2 /* at least one digit was out of range and ignored */
+};
+
+/* return codes */
+enum {
+  TPCCLUS_OK = 0,
+  TPCCLUS_ERR_INVALID_ARG = -1,
+  TPCCLUS_ERR_CUDA = -2,
+  TPCCLUS_ERR_NVRTC = -3,
+  TPCCLUS_ERR_WORKSPACE_TOO_SMALL = -4,
+  TPCCLUS_ERR_UNSUPPORTED_GEOMETRY = -5 /* n_sectors*n_rows*ceil(n_time/16256) > 5632 coarse bins */
+};
+
+typedef struct {
+  uint32_t struct_size;   /* = sizeof(tpcclus_params), for versioning                        */
+  uint32_t n_sectors;     /* 1..256                                                          */
+  uint32_t n_rows;        /* 1..256                                                          */
+  uint32_t n_time;        /* 1..65536 time bins per time frame (PAPER.md 12: 32 orbits)      */
+  const uint16_t* n_pads; /* HOST, n_rows entries, each 1..256; copied by create             */
+  uint16_t thr_peak;      /* peak threshold, test is q >= thr_peak (Q6); default 6           */
+  uint16_t noise_eps;     /* ridge tolerance of the suppression (O2, Q9); default 4          */
+  uint64_t max_digits;    /* sizing only: largest n that run() will be given                 */
+  uint32_t flags;         /* TPCCLUS_RTC                                                     */
+  int32_t device;         /* CUDA ordinal                                                    */
+  void* workspace;        /* DEVICE, caller-owned, 256-byte aligned, lives as long as the handle */
+  uint64_t workspace_bytes; /* >= tpcclus_workspace_bytes(params)                            */
+} tpcclus_params;
+
+typedef struct {
+  tpcclus_cluster* clusters; /* DEVICE, caller-owned, 16-byte aligned                        */
+  uint64_t capacity;         /* in clusters                                                  */
+  uint64_t* n_clusters;      /* DEVICE, caller-owned: true count, also on overflow           */
+  uint32_t* status;          /* DEVICE, TPCCLUS_STATUS_* bits; may be NULL                   */
+} tpcclus_out;
+
+/* Bytes of device workspace a handle with these parameters needs (depends on the geometry
+ * and max_digits only).  Returns 0 for invalid or unsupported parameters.  Host call. */
+TPCCLUS_API uint64_t tpcclus_workspace_bytes(const tpcclus_params* params);
+
+/* Validates, copies the geometry, lays out the workspace, uploads nothing yet (the
+ * parameter block goes to __constant__ memory at the head of every run(), stream-ordered,
+ * so several handles with different geometry can share a process: PAPER.md 85).  With
+ * TPCCLUS_RTC the kernels are compiled here for sm_100a by NVRTC and loaded as a module
+ * (PAPER.md 64, 91).  Host call, synchronous.  *out is NULL on failure. */
+TPCCLUS_API int tpcclus_create(const tpcclus_params* params, tpcclus_handle** out);
+
+/* Clusterizes one time frame: enqueues every step of the path (NS (1)..(5)) on
+ * `cuda_stream` (a cudaStream_t; NULL = legacy default stream) and returns without
+ * synchronising.  d_digits: DEVICE, 8-byte aligned, n <= max_digits records, any order,
+ * not modified.  out: HOST struct of DEVICE pointers.  The result depends only on
+ * (params, digit multiset, mode), never on earlier runs (Q17).  One run at a time per
+ * handle (the workspace is per handle).  The caller synchronises the stream before
+ * reading *n_clusters / *status / clusters. */
+TPCCLUS_API int tpcclus_run(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n,
+                            const tpcclus_out* out, int mode, void* cuda_stream);
+
+/* Same as run() but every pointer in `digits`/`out` is HOST memory (pinned or pageable):
+ * copies the digits to a staging area inside the workspace, runs, copies n_clusters,
+ * status and min(n_clusters, capacity) clusters back, and synchronises the stream.  The
+ * workspace must have been sized with tpcclus_workspace_bytes_host().  This is the
+ * end-to-end entry bench.py times (e2e). */
+TPCCLUS_API uint64_t tpcclus_workspace_bytes_host(const tpcclus_params* params, uint64_t cluster_capacity);
+TPCCLUS_API int tpcclus_run_host(tpcclus_handle* h, const tpcclus_digit* h_digits, uint64_t n,
+                                 tpcclus_cluster* h_clusters, uint64_t capacity,
+                                 uint64_t* h_n_clusters, uint32_t* h_status, int mode,
+                                 void* cuda_stream);
+
+TPCCLUS_API int tpcclus_destroy(tpcclus_handle* h);
+
+/* Static string for a return code.  Never NULL. */
+TPCCLUS_API const char* tpcclus_error_string(int code);
+
+/* Detail of the last failure on this handle (NVRTC log, CUDA error string); "" if none.
+ * Valid until the next call on the handle.  h may be NULL: then the detail of the last
+ * failed create() on this thread. */
+TPCCLUS_API const char* tpcclus_last_error(const tpcclus_handle* h);
+
+/* ---- introspection used by bench.py / tests (no effect on results) -------------------- */
+
+/* Number of kernels one run() launches in `mode` (bench.py's gpu_launches). */
+TPCCLUS_API int tpcclus_launches_per_run(const tpcclus_handle* h, int mode);
+
+/* Per-kernel device times of the LAST run() on this handle, when timing was enabled with
+ * tpcclus_set_timing(h, 1): fills up to `cap` entries (name pointers are static strings,
+ * ms from CUDA events recorded on the run's stream) and returns the number of kernels.
+ * Synchronises on the recorded events. */
+TPCCLUS_API int tpcclus_set_timing(tpcclus_handle* h, int enable);
+TPCCLUS_API int tpcclus_last_timing(tpcclus_handle* h, const char** names, float* ms, int cap);
+
+/* RTC build time in milliseconds (0 for non-RTC handles). */
+TPCCLUS_API double tpcclus_rtc_build_ms(const tpcclus_handle* h);
+
+/* Debug/parity hook for step a1 (the charge map): after a run(), rebuilds the dense
+ * [sector][row][time][pad] uint16 map (O0) from the binned digits into d_map (DEVICE,
+ * n_sectors * n_time * sum(n_pads) entries).  Not on the hot path. */
+TPCCLUS_API int tpcclus_debug_dense_map(tpcclus_handle* h, uint16_t* d_map, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TPCCLUS_H */

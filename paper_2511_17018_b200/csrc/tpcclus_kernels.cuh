@@ -1,0 +1,804 @@
+// tpcclus_kernels.cuh -- device code of the B200-native TPC clusterizer (sm_100a).
+//
+// ONE source for both builds (PAPER.md 89-93, section 5): nvcc compiles it offline with
+// the geometry/thresholds read from a __constant__ parameter block (PAPER.md 79-85), and
+// create(TPCCLUS_RTC) hands the very same text to NVRTC with `#define TPC_RTC 1` and one
+// `#define TPC_<field> <literal>` per parameter in front, so every PRM(x) below becomes a
+// literal and the dead branches (e.g. the time-chunk duplication) fold away.
+// Self-contained on purpose: no #include, so NVRTC needs no header search path.
+//
+// The path (rules: SURVEY.md 8(c) O0..O5):
+//   K1 partition_coarse  digits(8 B) -> 4-byte records binned by (sector,row,time-chunk)
+//   K2 dir_count / K3 dir_scan / K4 dir_fill   chunk directory -> per-bin chunk lists
+//   K5 partition_fine    per bin: batch-local counting sort by time slab (+3-bin halo copy)
+//   K6 cluster_tiles     per (sector,row,slab) tile: charge map in shared memory (O0),
+//                        3x3 peaks (O1), suppression (O2), 5x5 CoG (O3,O4), compaction,
+//                        ordered emission (O5)
+//   K7 scan_local / K8 scan_sums   deterministic mode: exclusive scan of per-tile counts
+#pragma once
+
+typedef unsigned int u32;
+typedef unsigned long long u64;
+typedef unsigned short u16;
+typedef unsigned char u8;
+
+// ---- fixed design constants ------------------------------------
+#define TPC_TS 128u            // time bins a tile owns
+#define TPC_HALO 3u            // halo: peaks at distance 2 need charges at distance 3 (O2)
+#define TPC_TT (TPC_TS + 2u * TPC_HALO)   // rows of a tile in shared memory
+#define TPC_TC 16256u          // time bins per coarse time-chunk: 127*128, +6 halo < 2^14
+#define TPC_STAGE 8u           // records (32 B) staged per coarse bin in K1
+#define TPC_CHUNK 64u          // records per pool chunk (256 B)
+#define TPC_CPB 128u           // chunks per K5 batch (<= 8192 records)
+#define TPC_K1_THREADS 1024
+#define TPC_K1_DPT 4           // digits per thread per round
+#define TPC_K5_THREADS 512
+#define TPC_K6_THREADS 256
+#define TPC_SCAN_THREADS 1024
+#define TPC_SCAN_PER_CTA 4096u
+
+#define TPC_STATUS_OVERFLOW 1u
+#define TPC_STATUS_BAD_DIGITS 2u
+
+struct TpcParams {
+  u32 n_sectors, n_rows, n_time;
+  u32 n_tc;        // coarse time-chunks = ceil(n_time / TPC_TC)
+  u32 n_bins;      // NB = n_sectors * n_rows * n_tc
+  u32 n_sl;        // tiles (slabs) per bin = ceil(min(n_time, TPC_TC) / TPC_TS)
+  u32 pitch;       // u16 cells per tile row = roundup8(max_pads + 6)
+  u32 max_pads;
+  u32 thr_peak, noise_eps;
+  u32 max_peaks;   // capacity of the per-tile peak list
+  u32 pad_[1];
+  u16 n_pads[256];
+};
+
+#ifdef TPC_RTC
+#define PRM(x) (TPC_##x)
+#define PRM_NPADS(r) (TPC_NPADS_TABLE[r])   // emitted by the host in front of this text
+#else
+__constant__ TpcParams c_prm;
+#define PRM(x) (c_prm.x)
+#define PRM_NPADS(r) (c_prm.n_pads[r])
+#endif
+
+// ---- shared-memory sizes (bytes); the host launches with exactly these --------------------
+__host__ __device__ inline u32 tpc_k1_smem_bytes(u32 nb) {
+  return (nb * TPC_STAGE + nb + ((nb + 1u) >> 1) + 4u) * 4u + 512u;
+}
+__host__ __device__ inline u32 tpc_k6_smem_bytes(u32 pitch, u32 max_peaks) {
+  return (TPC_TT * pitch / 2u + 2u * 256u + 2u + (max_peaks + 1u) / 2u + TPC_TT * 8u + TPC_TT + 2u + 256u + 1u + 8u + 4u) * 4u + 16u;
+}
+
+// ---- small PTX helpers -------------------------------------------------------------------
+__device__ __forceinline__ uint2 ld_stream_u2(const uint2* p) {   // read-once input: keep out of L1
+  uint2 v;
+  asm volatile("ld.global.nc.L1::no_allocate.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ uint4 ld_stream_u4(const uint4* p) {
+  uint4 v;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ void st_256(void* p, uint4 a, uint4 b) {   // one 32-byte sector, one request
+#ifdef TPC_NO_ST256   // an NVRTC older than 12.9 has no 256-bit vector store
+  ((uint4*)p)[0] = a; ((uint4*)p)[1] = b;
+  return;
+#endif
+  asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "r"(a.x), "r"(a.y), "r"(a.z),
+               "r"(a.w), "r"(b.x), "r"(b.y), "r"(b.z), "r"(b.w) : "memory");
+}
+__device__ __forceinline__ u32 lane_id() { return threadIdx.x & 31u; }
+
+// ==========================================================================================
+// K1  partition_coarse  (NS (1) "digit -> charge-map scatter", first half: O0's validity,
+//     clamp and zero rules, and the routing of each digit to its (sector,row) map)
+//
+// One persistent CTA per SM.  Shared memory holds a 32-byte write-combining stage per
+// coarse bin; a full stage leaves as ONE 32-byte sector store into a 256-byte chunk that
+// is private to (CTA, bin), so there is no global atomic and no histogram pre-pass.
+// The chunk directory dir[] (bin<<8 | records) is turned into per-bin lists by K2..K4.
+//
+// record (4 B):  pad[0:8) | u[8:22) | q[22:32)   with u = time - tc*TPC_TC + 3  (14 bit)
+// ==========================================================================================
+struct K1Smem {   // layout computed identically on the host (tpcclus.cu)
+  u32* stage;     // [NB][8]
+  u32* pos;       // [NB]  (chunk_local << 4) | sectors_filled(0..8)
+  u32* cnt;       // [(NB+1)/2] two 16-bit counters per word
+  u32* misc;      // [0] next chunk, [1] bad flag
+  u16* npads;     // [256]
+};
+__device__ __forceinline__ K1Smem k1_smem(u32* base, u32 nb) {
+  K1Smem s;
+  s.stage = base;
+  s.pos = s.stage + (u64)nb * TPC_STAGE;
+  s.cnt = s.pos + nb;
+  s.misc = s.cnt + ((nb + 1u) >> 1);
+  s.npads = (u16*)(s.misc + 4);
+  return s;
+}
+
+__device__ __forceinline__ void k1_flush(const K1Smem& s, u32 bin, u32 slice_base, u32 slice_cap,
+                                         uint4* pool, u32* dir) {
+  u32 p = s.pos[bin];
+  u32 fill = p & 15u, c = p >> 4;
+  if (fill == 8u) {
+    c = atomicAdd(&s.misc[0], 1u);
+    fill = 0u;
+    if (c < slice_cap) dir[slice_base + c] = (bin << 8) | TPC_CHUNK;
+  }
+  const uint4* st = (const uint4*)(s.stage + (u64)bin * TPC_STAGE);
+  uint4 a = st[0], b = st[1];
+  if (c < slice_cap) st_256(pool + ((u64)(slice_base + c) * 16u + fill * 2u), a, b);
+  s.pos[bin] = (c << 4) | (fill + 1u);
+  atomicSub(&s.cnt[bin >> 1], 8u << ((bin & 1u) * 16u));
+}
+
+// Inserts up to K records per thread into the stages; block-synchronous.  bin == 0xFFFFFFFF
+// means "no record".  Handles any skew: a round in which one bin receives more than 8
+// records loops, flushing 8 at a time.
+template <int K>
+__device__ __forceinline__ void k1_insert(const K1Smem& s, const u32 (&bin)[K], const u32 (&rec)[K],
+                                          u32 slice_base, u32 slice_cap, uint4* pool, u32* dir) {
+  u32 slot[K];
+  u32 pending = 0u, flush = 0u;
+#pragma unroll
+  for (int k = 0; k < K; ++k) {
+    if (bin[k] != 0xFFFFFFFFu) {
+      u32 sh = (bin[k] & 1u) * 16u;
+      slot[k] = (atomicAdd(&s.cnt[bin[k] >> 1], 1u << sh) >> sh) & 0xFFFFu;
+      pending |= 1u << k;
+    } else {
+      slot[k] = 0u;
+    }
+  }
+  for (;;) {
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+      if (pending & (1u << k)) {
+        if (slot[k] < TPC_STAGE) {
+          s.stage[(u64)bin[k] * TPC_STAGE + slot[k]] = rec[k];
+          pending &= ~(1u << k);
+          if (slot[k] == TPC_STAGE - 1u) flush |= 1u << k;
+        } else {
+          slot[k] -= TPC_STAGE;
+        }
+      }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < K; ++k)
+      if (flush & (1u << k)) k1_flush(s, bin[k], slice_base, slice_cap, pool, dir);
+    flush = 0u;
+    if (!__syncthreads_or((int)pending)) break;
+  }
+}
+
+extern "C" __global__ void __launch_bounds__(TPC_K1_THREADS, 1)
+k_partition_coarse(const uint2* __restrict__ digits, u64 n, u64 per_cta, uint4* __restrict__ pool,
+                   u32* __restrict__ dir, u32* __restrict__ used, u32 slice_cap, u32* __restrict__ status) {
+  extern __shared__ __align__(16) u32 smem_u32[];
+  const u32 nb = PRM(n_bins);
+  const K1Smem s = k1_smem(smem_u32, nb);
+  for (u32 i = threadIdx.x; i < nb; i += TPC_K1_THREADS) s.pos[i] = 8u;
+  for (u32 i = threadIdx.x; i < ((nb + 1u) >> 1); i += TPC_K1_THREADS) s.cnt[i] = 0u;
+  if (threadIdx.x < 4) s.misc[threadIdx.x] = 0u;
+  if (threadIdx.x < 256) s.npads[threadIdx.x] = threadIdx.x < PRM(n_rows) ? PRM_NPADS(threadIdx.x) : (u16)0;
+  __syncthreads();
+
+  const u32 slice_base = blockIdx.x * slice_cap;
+  const u64 begin = (u64)blockIdx.x * per_cta;
+  u64 end = begin + per_cta;
+  if (end > n) end = n;
+  const u32 ROUND = TPC_K1_THREADS * TPC_K1_DPT;
+  const u32 S = PRM(n_sectors), R = PRM(n_rows), T = PRM(n_time), NTC = PRM(n_tc);
+
+  uint2 nxt[TPC_K1_DPT];
+#pragma unroll
+  for (int k = 0; k < TPC_K1_DPT; ++k) {
+    u64 i = begin + (u64)k * TPC_K1_THREADS + threadIdx.x;
+    nxt[k] = (begin < end && i < end) ? ld_stream_u2(digits + i) : make_uint2(0u, 0u);
+  }
+  bool bad = false;
+  for (u64 base = begin; base < end; base += ROUND) {
+    uint2 cur[TPC_K1_DPT];
+#pragma unroll
+    for (int k = 0; k < TPC_K1_DPT; ++k) cur[k] = nxt[k];
+#pragma unroll
+    for (int k = 0; k < TPC_K1_DPT; ++k) {   // prefetch the next round while this one is binned
+      u64 i = base + ROUND + (u64)k * TPC_K1_THREADS + threadIdx.x;
+      nxt[k] = (i < end) ? ld_stream_u2(digits + i) : make_uint2(0u, 0u);
+    }
+    u32 bin[TPC_K1_DPT], rec[TPC_K1_DPT], dbin[TPC_K1_DPT], drec[TPC_K1_DPT];
+    bool anydup = false;
+#pragma unroll
+    for (int k = 0; k < TPC_K1_DPT; ++k) {
+      u64 i = base + (u64)k * TPC_K1_THREADS + threadIdx.x;
+      bin[k] = 0xFFFFFFFFu; rec[k] = 0u; dbin[k] = 0xFFFFFFFFu; drec[k] = 0u;
+      if (i < end) {
+        u32 w0 = cur[k].x, w1 = cur[k].y;
+        u32 q = w0 & 0xFFFFu, t = w0 >> 16, pad = w1 & 0xFFu, row = (w1 >> 8) & 0xFFu, sec = (w1 >> 16) & 0xFFu;
+        if (sec >= S || row >= R || t >= T || pad >= (u32)s.npads[row]) {   // O0 / Q4: ignore + flag
+          bad = true;
+        } else if (q != 0u) {                                               // Q4: zero charge ignored
+          q = q > 1023u ? 1023u : q;                                        // Q4: clamp
+          u32 tc = (NTC > 1u) ? t / TPC_TC : 0u;
+          u32 v = t - tc * TPC_TC;
+          u32 b0 = (sec * R + row) * NTC + tc;
+          bin[k] = b0;
+          rec[k] = pad | ((v + TPC_HALO) << 8) | (q << 22);
+          if (NTC > 1u) {   // halo copy into the neighbouring time-chunk's bin
+            if (v < TPC_HALO && tc > 0u) {
+              dbin[k] = b0 - 1u; drec[k] = pad | ((v + TPC_TC + TPC_HALO) << 8) | (q << 22); anydup = true;
+            } else if (v + TPC_HALO >= TPC_TC && tc + 1u < NTC) {
+              dbin[k] = b0 + 1u; drec[k] = pad | ((v + TPC_HALO - TPC_TC) << 8) | (q << 22); anydup = true;
+            }
+          }
+        }
+      }
+    }
+    k1_insert<TPC_K1_DPT>(s, bin, rec, slice_base, slice_cap, pool, dir);
+    if (NTC > 1u) {
+      if (__syncthreads_or((int)anydup)) k1_insert<TPC_K1_DPT>(s, dbin, drec, slice_base, slice_cap, pool, dir);
+    }
+  }
+  if (bad) atomicOr(status, TPC_STATUS_BAD_DIGITS);
+  __syncthreads();
+  // drain: every bin's partial stage goes to its current (or a fresh) chunk; fix the
+  // record count of that last chunk in the directory.
+  for (u32 b = threadIdx.x; b < nb; b += TPC_K1_THREADS) {
+    u32 m = (s.cnt[b >> 1] >> ((b & 1u) * 16u)) & 0xFFFFu;   // 0..7 staged
+    u32 p = s.pos[b];
+    u32 fill = p & 15u, c = p >> 4;
+    if (m != 0u) {
+      if (fill == 8u) { c = atomicAdd(&s.misc[0], 1u); fill = 0u; }
+      const uint4* st = (const uint4*)(s.stage + (u64)b * TPC_STAGE);
+      if (c < slice_cap) {
+        st_256(pool + ((u64)(slice_base + c) * 16u + fill * 2u), st[0], st[1]);
+        dir[slice_base + c] = (b << 8) | (fill * 8u + m);
+      }
+    } else if (fill != 8u && fill != 0u) {
+      if (c < slice_cap) dir[slice_base + c] = (b << 8) | (fill * 8u);
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    u32 u = s.misc[0];
+    if (u > slice_cap) { u = slice_cap; atomicOr(status, 0x80000000u); }   // cannot happen (bound in DESIGN.md)
+    used[blockIdx.x] = u;
+  }
+}
+
+// ==========================================================================================
+// K2..K4  chunk directory -> per-bin chunk lists (bookkeeping of the scatter; ~2.6e7 chunks
+// at CFG[4], 4 bytes each).  The order of chunks inside a bin is whatever the atomics give:
+// nothing downstream depends on it (the map build is a max, O0/Q5).
+// ==========================================================================================
+extern "C" __global__ void __launch_bounds__(256)
+k_dir_count(const u32* __restrict__ dir, const u32* __restrict__ used, u32 slice_cap, u32* __restrict__ bin_nchunks) {
+  const u32 cta = blockIdx.y;
+  const u32 n = used[cta];
+  for (u32 c = blockIdx.x * 256u + threadIdx.x; c < n; c += gridDim.x * 256u)
+    atomicAdd(&bin_nchunks[dir[(u64)cta * slice_cap + c] >> 8], 1u);
+}
+
+// single CTA: exclusive scans over the bins.
+//   bin_chunk_start[b] = sum_{b'<b} nchunks[b']          (NB+1 entries)
+//   batch_start[b]     = sum_{b'<b} ceil(nchunks[b']/CPB) (NB+1 entries; [NB] = total batches)
+extern "C" __global__ void __launch_bounds__(TPC_SCAN_THREADS)
+k_dir_scan(const u32* __restrict__ bin_nchunks, u32* __restrict__ bin_chunk_start, u32* __restrict__ batch_start) {
+  __shared__ u32 s_a[TPC_SCAN_THREADS], s_b[TPC_SCAN_THREADS];
+  const u32 nb = PRM(n_bins);
+  const u32 per = (nb + TPC_SCAN_THREADS - 1u) / TPC_SCAN_THREADS;
+  const u32 lo = threadIdx.x * per;
+  u32 hi = lo + per;
+  if (hi > nb) hi = nb;
+  u32 sa = 0u, sb = 0u;
+  for (u32 b = lo; b < hi; ++b) { u32 c = bin_nchunks[b]; sa += c; sb += (c + TPC_CPB - 1u) / TPC_CPB; }
+  s_a[threadIdx.x] = sa; s_b[threadIdx.x] = sb;
+  __syncthreads();
+  for (u32 d = 1u; d < TPC_SCAN_THREADS; d <<= 1) {   // Hillis-Steele inclusive scan
+    u32 va = 0u, vb = 0u;
+    if (threadIdx.x >= d) { va = s_a[threadIdx.x - d]; vb = s_b[threadIdx.x - d]; }
+    __syncthreads();
+    s_a[threadIdx.x] += va; s_b[threadIdx.x] += vb;
+    __syncthreads();
+  }
+  u32 ea = s_a[threadIdx.x] - sa, eb = s_b[threadIdx.x] - sb;   // exclusive prefix of this thread's range
+  for (u32 b = lo; b < hi; ++b) {
+    u32 c = bin_nchunks[b];
+    bin_chunk_start[b] = ea; batch_start[b] = eb;
+    ea += c; eb += (c + TPC_CPB - 1u) / TPC_CPB;
+  }
+  if (threadIdx.x == TPC_SCAN_THREADS - 1u) { bin_chunk_start[nb] = s_a[threadIdx.x]; batch_start[nb] = s_b[threadIdx.x]; }
+}
+
+extern "C" __global__ void __launch_bounds__(256)
+k_dir_fill(const u32* __restrict__ dir, const u32* __restrict__ used, u32 slice_cap,
+           const u32* __restrict__ bin_chunk_start, u32* __restrict__ bin_fill, u32* __restrict__ chunk_list) {
+  const u32 cta = blockIdx.y;
+  const u32 n = used[cta];
+  for (u32 c = blockIdx.x * 256u + threadIdx.x; c < n; c += gridDim.x * 256u) {
+    u32 id = cta * slice_cap + c;
+    u32 bin = dir[id] >> 8;
+    chunk_list[bin_chunk_start[bin] + atomicAdd(&bin_fill[bin], 1u)] = id;
+  }
+}
+
+// ==========================================================================================
+// K7/K8  exclusive scan of per-tile cluster counts (deterministic mode, O5 / PAPER.md 47-50:
+// the ordered-scan compaction is the "slower deterministic algorithm" that replaces atomics)
+// ==========================================================================================
+extern "C" __global__ void __launch_bounds__(TPC_SCAN_THREADS)
+k_scan_local(const u32* __restrict__ in, u32* __restrict__ out_local, u32* __restrict__ block_sum, u32 n) {
+  __shared__ u32 s[TPC_SCAN_THREADS];
+  const u32 base = blockIdx.x * TPC_SCAN_PER_CTA + threadIdx.x * 4u;
+  u32 v[4], t = 0u;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) { v[k] = (base + k < n) ? in[base + k] : 0u; t += v[k]; }
+  s[threadIdx.x] = t;
+  __syncthreads();
+  for (u32 d = 1u; d < TPC_SCAN_THREADS; d <<= 1) {
+    u32 a = threadIdx.x >= d ? s[threadIdx.x - d] : 0u;
+    __syncthreads();
+    s[threadIdx.x] += a;
+    __syncthreads();
+  }
+  u32 e = s[threadIdx.x] - t;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) { if (base + k < n) out_local[base + k] = e; e += v[k]; }
+  if (threadIdx.x == TPC_SCAN_THREADS - 1u) block_sum[blockIdx.x] = s[threadIdx.x];
+}
+
+// single CTA: block_prefix[i] = sum_{j<i} block_sum[j] (64 bit); *total = grand total.
+extern "C" __global__ void __launch_bounds__(TPC_SCAN_THREADS)
+k_scan_sums(const u32* __restrict__ block_sum, u64* __restrict__ block_prefix, u32 nblocks, u64* __restrict__ total) {
+  __shared__ u64 s[TPC_SCAN_THREADS];
+  __shared__ u64 carry;
+  if (threadIdx.x == 0) carry = 0ull;
+  __syncthreads();
+  for (u32 base = 0u; base < nblocks; base += TPC_SCAN_THREADS) {
+    u32 i = base + threadIdx.x;
+    u64 v = i < nblocks ? (u64)block_sum[i] : 0ull;
+    s[threadIdx.x] = v;
+    __syncthreads();
+    for (u32 d = 1u; d < TPC_SCAN_THREADS; d <<= 1) {
+      u64 a = threadIdx.x >= d ? s[threadIdx.x - d] : 0ull;
+      __syncthreads();
+      s[threadIdx.x] += a;
+      __syncthreads();
+    }
+    if (i < nblocks) block_prefix[i] = carry + s[threadIdx.x] - v;
+    __syncthreads();
+    if (threadIdx.x == TPC_SCAN_THREADS - 1u) carry += s[threadIdx.x];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) *total = carry;
+}
+
+// ==========================================================================================
+// K5  partition_fine  (NS (1), second half: route every record to the tile(s) whose shared-
+//     memory charge map needs it; a record within 3 time bins of a slab border is copied
+//     into the neighbouring tile as halo)
+//
+// A batch = up to TPC_CPB chunks (<= 8192 records) of ONE coarse bin.  The CTA counting-sorts
+// the batch by slab in shared memory and writes the sorted batch as one contiguous blob
+// (runs padded to 32 B), plus one index entry per (tile, batch):  pos[0:40) | count[40:64).
+// index layout: idx[n_sl * batch_start[b] + sl * nbatch_b + kb], so a tile finds the runs
+// of all batches of its bin in one contiguous read.
+//
+// tile record (4 B):  pad[0:8) | tl[8:16) | q[16:26)   tl = row of the tile, 0..TPC_TT-1
+// tile sl of a bin holds u in [sl*TS, sl*TS + TS + 6);  it OWNS tl in [3, TS+3).
+// ==========================================================================================
+#define TPC_K5_BUF (2u * TPC_CPB * TPC_CHUNK + 8u * 128u)   // u32 words: records + halo copies + run padding
+
+extern "C" __global__ void __launch_bounds__(TPC_K5_THREADS, 2)
+k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, const u32* __restrict__ chunk_list,
+                 const u32* __restrict__ bin_chunk_start, const u32* __restrict__ batch_start,
+                 u32* __restrict__ blob, u64* __restrict__ blob_cursor, u64* __restrict__ idx) {
+  extern __shared__ __align__(16) u32 smem_u32[];
+  u32* buf = smem_u32;                       // [TPC_K5_BUF]
+  u32* s_cnt = buf + TPC_K5_BUF;             // [128] primaries per slab
+  u32* s_dcnt = s_cnt + 128;                 // [128] halo copies per slab
+  u32* s_off = s_dcnt + 128;                 // [129] run start (multiple of 8)
+  u32* s_dcur = s_off + 132;                 // [128]
+  __shared__ u64 s_gbase;
+  const u32 nb = PRM(n_bins), nsl = PRM(n_sl);
+  const u32 n_batches = batch_start[nb];
+
+  for (u32 batch = blockIdx.x; batch < n_batches; batch += gridDim.x) {
+    // bin of this batch: last b with batch_start[b] <= batch
+    u32 lo = 0u, hi = nb;
+    while (hi - lo > 1u) { u32 mid = (lo + hi) >> 1; if (batch_start[mid] <= batch) lo = mid; else hi = mid; }
+    const u32 b = lo;
+    const u32 kb = batch - batch_start[b];
+    const u32 nbatch_b = batch_start[b + 1] - batch_start[b];
+    const u32 c0 = bin_chunk_start[b] + kb * TPC_CPB;
+    u32 c1 = c0 + TPC_CPB;
+    if (c1 > bin_chunk_start[b + 1]) c1 = bin_chunk_start[b + 1];
+    const u32 nch = c1 - c0;
+
+    if (threadIdx.x < 128) { s_cnt[threadIdx.x] = 0u; s_dcnt[threadIdx.x] = 0u; s_dcur[threadIdx.x] = 0u; }
+    __syncthreads();
+
+    // ---- load <= 16 records per thread, count per slab, remember the rank ------------------
+    u32 rec[16];
+    u32 rank[8];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      u32 q4 = threadIdx.x + (u32)i * TPC_K5_THREADS;   // 16-byte piece of the batch
+      u32 ch = q4 >> 4, sub = q4 & 15u;
+      uint4 v = make_uint4(0u, 0u, 0u, 0u);
+      u32 nrec = 0u;
+      if (ch < nch) {
+        u32 cid = chunk_list[c0 + ch];
+        nrec = dir[cid] & 0xFFu;
+        v = ld_stream_u4(pool + (u64)cid * 16u + sub);
+      }
+      u32 r4[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        u32 r = (sub * 4u + (u32)j < nrec) ? r4[j] : 0u;   // q >= 1 in every valid record, so 0 = none
+        u32 rk = 0u;
+        if (r != 0u) {
+          u32 u = (r >> 8) & 0x3FFFu;
+          u32 sl1 = u / TPC_TS, m = u - sl1 * TPC_TS;
+          if (sl1 < nsl) rk = atomicAdd(&s_cnt[sl1], 1u);
+          if (sl1 >= 1u && m < 2u * TPC_HALO) atomicAdd(&s_dcnt[sl1 - 1u], 1u);
+        }
+        rec[i * 4 + j] = r;
+        if (j & 1) rank[i * 2 + (j >> 1)] |= rk << 16; else rank[i * 2 + (j >> 1)] = rk;
+      }
+    }
+    __syncthreads();
+    // ---- exclusive scan of padded run lengths (one warp, 4 slabs per lane) -----------------
+    if (threadIdx.x < 32) {
+      u32 len[4], t = 0u;
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        u32 sl = threadIdx.x * 4u + (u32)k;
+        len[k] = sl < nsl ? ((s_cnt[sl] + s_dcnt[sl] + 7u) & ~7u) : 0u;
+        t += len[k];
+      }
+      u32 inc = t;
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) { u32 o = __shfl_up_sync(0xFFFFFFFFu, inc, d); if ((int)threadIdx.x >= d) inc += o; }
+      u32 e = inc - t;
+#pragma unroll
+      for (int k = 0; k < 4; ++k) { s_off[threadIdx.x * 4u + (u32)k] = e; e += len[k]; }
+      if (threadIdx.x == 31) {
+        s_off[128] = inc;
+        s_gbase = atomicAdd(blob_cursor, (u64)inc);
+      }
+    }
+    __syncthreads();
+    // ---- place ------------------------------------------------------------------------------
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+      u32 r = rec[k];
+      if (r != 0u) {
+        u32 u = (r >> 8) & 0x3FFFu;
+        u32 sl1 = u / TPC_TS, m = u - sl1 * TPC_TS;
+        u32 base = (r & 0xFFu) | ((r >> 22) << 16);
+        u32 rk = (rank[k >> 1] >> ((k & 1) * 16)) & 0xFFFFu;
+        if (sl1 < nsl) buf[s_off[sl1] + rk] = base | (m << 8);
+        if (sl1 >= 1u && m < 2u * TPC_HALO) {
+          u32 d = atomicAdd(&s_dcur[sl1 - 1u], 1u);
+          buf[s_off[sl1 - 1u] + s_cnt[sl1 - 1u] + d] = base | ((m + TPC_TS) << 8);
+        }
+      }
+    }
+    __syncthreads();
+    // ---- dump the sorted batch + its index entries -----------------------------------------
+    const u64 gbase = s_gbase;
+    const u32 total = s_off[128];
+    uint4* dst = (uint4*)(blob + gbase);       // gbase is a multiple of 8 records (32 B)
+    const uint4* src = (const uint4*)buf;
+    for (u32 i = threadIdx.x; i < (total >> 2); i += TPC_K5_THREADS) dst[i] = src[i];
+    if (threadIdx.x < nsl) {
+      u32 sl = threadIdx.x;
+      idx[(u64)nsl * batch_start[b] + (u64)sl * nbatch_b + kb] =
+          (gbase + s_off[sl]) | ((u64)(s_cnt[sl] + s_dcnt[sl]) << 40);
+    }
+    __syncthreads();
+  }
+}
+
+// ==========================================================================================
+// K6  cluster_tiles  (NS (1) last step + (2) + (3) + (4); rules O0..O5 of SURVEY.md 8(c))
+//
+// Persistent CTAs; one tile = (bin, slab) at a time.  The tile's charge map lives in shared
+// memory as u16 [TPC_TT][pitch] with 3 zero guard pads on each side; bit 15 of a cell marks
+// a peak (O1).  Survivors of O2 are marked in a per-row pad bitmask, which gives every
+// cluster its rank in (time, pad) order inside the tile without a sort; the base of the
+// tile comes from one atomic (FAST) or from the exclusive scan of the tile counts
+// (DETERMINISTIC: K6 runs once to count, K7/K8 scan, K6 runs again to emit).
+// ==========================================================================================
+#define TPC_MODE_FAST 0
+#define TPC_MODE_DET_COUNT 1
+#define TPC_MODE_DET_EMIT 2
+#define TPC_MODE_DUMP_MAP 3
+#define TPC_K6_GROUP 256u   // index entries (runs) handled per pass
+
+struct K6Args {
+  const u32* blob; const u64* idx; const u32* batch_start;
+  uint4* out; u64 capacity; u64* n_clusters; u32* status;
+  u32* tile_cnt; const u32* tile_local; const u64* block_prefix;
+  u16* dmap; const u64* row_off;   // DUMP_MAP only: row_off[r] = cells of rows < r in one sector; [n_rows] = per sector
+};
+
+struct K6Smem {
+  u16* tile; u32* tile32; u16* peaks; u32* rowmask; u32* rowpre; u64* rpos; u32* rpre; u32* wsum; u32* misc; u64* base;
+};
+__device__ __forceinline__ K6Smem k6_smem(u32* p) {
+  K6Smem s;
+  const u32 tile_words = TPC_TT * PRM(pitch) / 2u;
+  s.tile32 = p; s.tile = (u16*)p; p += tile_words;
+  s.rpos = (u64*)p; p += 2u * TPC_K6_GROUP;
+  s.base = (u64*)p; p += 2;
+  s.peaks = (u16*)p; p += (PRM(max_peaks) + 1u) / 2u;
+  s.rowmask = p; p += TPC_TT * 8u;
+  s.rowpre = p; p += TPC_TT + 2u;
+  s.rpre = p; p += TPC_K6_GROUP + 1u;
+  s.wsum = p; p += 8;
+  s.misc = p;   // [0] n_peaks, [1] total survivors
+  return s;
+}
+
+// loads index entries [g0, g0+ng) of this tile into shared memory and scans their counts.
+__device__ __forceinline__ u32 k6_load_group(const K6Smem& s, const u64* __restrict__ idx, u64 ib, u32 g0, u32 ng) {
+  u32 c = 0u;
+  if (threadIdx.x < ng) {
+    u64 e = idx[ib + g0 + threadIdx.x];
+    s.rpos[threadIdx.x] = e & ((1ull << 40) - 1ull);
+    c = (u32)(e >> 40);
+  }
+  u32 inc = c;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) { u32 o = __shfl_up_sync(0xFFFFFFFFu, inc, d); if ((int)lane_id() >= d) inc += o; }
+  if (lane_id() == 31u) s.wsum[threadIdx.x >> 5] = inc;
+  __syncthreads();
+  u32 wp = 0u;
+  for (u32 w = 0; w < (threadIdx.x >> 5); ++w) wp += s.wsum[w];
+  s.rpre[threadIdx.x + 1u] = wp + inc;   // inclusive -> rpre[i+1]
+  if (threadIdx.x == 0) s.rpre[0] = 0u;
+  __syncthreads();
+  return s.rpre[TPC_K6_GROUP];
+}
+
+// calls f(record) for every record of the loaded group, flat over the block.
+template <class F>
+__device__ __forceinline__ void k6_for_records(const K6Smem& s, const u32* __restrict__ blob, u32 total, F f) {
+  u32 run = 0u;
+  for (u32 j = threadIdx.x; j < total; j += TPC_K6_THREADS) {
+    while (j >= s.rpre[run + 1u]) ++run;
+    f(blob[s.rpos[run] + (j - s.rpre[run])]);
+  }
+}
+
+// runs f over ALL records of the tile (several groups only for bins with > 256 batches).
+template <class F>
+__device__ __forceinline__ void k6_phase(const K6Smem& s, const K6Args& a, u64 ib, u32 nbatch, u32 total0, F f) {
+  if (nbatch <= TPC_K6_GROUP) {
+    k6_for_records(s, a.blob, total0, f);
+  } else {
+    for (u32 g0 = 0u; g0 < nbatch; g0 += TPC_K6_GROUP) {
+      u32 ng = nbatch - g0 < TPC_K6_GROUP ? nbatch - g0 : TPC_K6_GROUP;
+      __syncthreads();
+      u32 t = k6_load_group(s, a.idx, ib, g0, ng);
+      k6_for_records(s, a.blob, t, f);
+    }
+  }
+}
+
+template <int MODE>
+__device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
+  const K6Smem s = k6_smem(smem);
+  const u32 nb = PRM(n_bins), nsl = PRM(n_sl), pitch = PRM(pitch);
+  const u32 n_tiles = nb * nsl;
+  const u32 thr = PRM(thr_peak), eps = PRM(noise_eps);
+  const u32 tile_words = TPC_TT * pitch / 2u;
+
+  for (u32 tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    const u32 b = tile / nsl, sl = tile - b * nsl;
+    const u32 bs0 = a.batch_start[b];
+    const u32 nbatch = a.batch_start[b + 1] - bs0;
+    const u64 ib = (u64)nsl * bs0 + (u64)sl * nbatch;
+    __syncthreads();   // previous tile fully done with shared memory
+    u32 total0 = 0u;
+    if (nbatch != 0u) total0 = k6_load_group(s, a.idx, ib, 0u, nbatch < TPC_K6_GROUP ? nbatch : TPC_K6_GROUP);
+    if (nbatch == 0u || (nbatch <= TPC_K6_GROUP && total0 == 0u)) {   // block-uniform
+      if (MODE == TPC_MODE_DET_COUNT && threadIdx.x == 0) a.tile_cnt[tile] = 0u;
+      continue;
+    }
+    // ---- O0: zero the map, scatter the tile's records -------------------------------------
+    {
+      uint4* z = (uint4*)s.tile32;
+      for (u32 i = threadIdx.x; i < tile_words / 4u; i += TPC_K6_THREADS) z[i] = make_uint4(0u, 0u, 0u, 0u);
+      for (u32 i = threadIdx.x; i < TPC_TT * 8u; i += TPC_K6_THREADS) s.rowmask[i] = 0u;
+      if (threadIdx.x < 2) s.misc[threadIdx.x] = 0u;
+    }
+    __syncthreads();
+    k6_phase(s, a, ib, nbatch, total0, [&](u32 r) {
+      u32 cell = ((r >> 8) & 0xFFu) * pitch + (r & 0xFFu) + TPC_HALO;
+      s.tile[cell] = (u16)((r >> 16) & 0x3FFu);
+    });
+    if (MODE != TPC_MODE_FAST) {
+      // Q5, deterministic: two digits on one cell -> the maximum, whatever the order.  Re-check
+      // until stable; with duplicate-free input this is one read per record and one barrier.
+      for (;;) {
+        __syncthreads();
+        u32 any = 0u;
+        k6_phase(s, a, ib, nbatch, total0, [&](u32 r) {
+          u32 cell = ((r >> 8) & 0xFFu) * pitch + (r & 0xFFu) + TPC_HALO;
+          u16 q = (u16)((r >> 16) & 0x3FFu);
+          if (s.tile[cell] < q) { s.tile[cell] = q; any = 1u; }
+        });
+        if (!__syncthreads_or((int)any)) break;
+      }
+    } else {
+      __syncthreads();
+    }
+
+    const u32 tc = b % PRM(n_tc), sr = b / PRM(n_tc);
+    const u32 row = sr % PRM(n_rows), sector = sr / PRM(n_rows);
+    const u32 npads = PRM_NPADS(row);
+    const int t_base = (int)(tc * TPC_TC + sl * TPC_TS) - (int)TPC_HALO;   // time of tile row 0
+
+    if (MODE == TPC_MODE_DUMP_MAP) {
+      const u64 sector_cells = a.row_off[PRM(n_rows)];
+      for (u32 i = threadIdx.x; i < TPC_TS * npads; i += TPC_K6_THREADS) {
+        u32 tl = i / npads + TPC_HALO, p = i % npads;
+        int t = t_base + (int)tl;
+        if (t < (int)PRM(n_time))
+          a.dmap[(u64)sector * sector_cells + a.row_off[row] + (u64)t * npads + p] = s.tile[tl * pitch + p + TPC_HALO];
+      }
+      continue;
+    }
+
+    // ---- O1: 3x3 peaks; strict > against the 4 neighbours earlier in (t,p) order, >= later --
+    k6_phase(s, a, ib, nbatch, total0, [&](u32 r) {
+      u32 tl = (r >> 8) & 0xFFu, pad = r & 0xFFu, q = (r >> 16) & 0x3FFu;
+      if (q < thr || tl < 1u || tl > TPC_TT - 2u) return;
+      u32 cell = tl * pitch + pad + TPC_HALO;
+      const u16* c = s.tile + cell;
+      if ((c[0] & 0x3FFu) != q) return;   // a smaller duplicate of this cell
+      bool pk = q > (c[-(int)pitch - 1] & 0x3FFu) && q > (c[-(int)pitch] & 0x3FFu) && q > (c[-(int)pitch + 1] & 0x3FFu) &&
+                q > (c[-1] & 0x3FFu) && q >= (c[1] & 0x3FFu) &&
+                q >= (c[pitch - 1] & 0x3FFu) && q >= (c[pitch] & 0x3FFu) && q >= (c[pitch + 1] & 0x3FFu);
+      if (!pk) return;
+      u32 bit = 0x8000u << ((cell & 1u) * 16u);
+      u32 old = atomicOr(&s.tile32[cell >> 1], bit);
+      if (!(old & bit) && tl >= TPC_HALO && tl < TPC_TS + TPC_HALO) {
+        u32 i = atomicAdd(&s.misc[0], 1u);
+        s.peaks[i] = (u16)((tl << 8) | pad);
+      }
+    });
+    __syncthreads();
+    const u32 npk = s.misc[0];
+
+    // ---- O2: suppression against the un-updated peak set -----------------------------------
+    for (u32 i = threadIdx.x; i < npk; i += TPC_K6_THREADS) {
+      u32 e = s.peaks[i];
+      u32 tl = e >> 8, pad = e & 0xFFu;
+      const u16* c = s.tile + tl * pitch + pad + TPC_HALO;
+      u32 qc = c[0] & 0x3FFu;
+      u32 nq[3][3];
+#pragma unroll
+      for (int dt = -1; dt <= 1; ++dt)
+#pragma unroll
+        for (int dp = -1; dp <= 1; ++dp) nq[dt + 1][dp + 1] = c[dt * (int)pitch + dp] & 0x3FFu;
+      bool dead = false;
+#pragma unroll
+      for (int dt = -2; dt <= 2; ++dt)
+#pragma unroll
+        for (int dp = -2; dp <= 2; ++dp) {
+          if (dt != -2 && dt != 2 && dp != -2 && dp != 2) continue;
+          u32 v = c[dt * (int)pitch + dp];
+          if (!(v & 0x8000u)) continue;
+          u32 q2 = v & 0x3FFu;
+          bool beats = q2 > qc || (q2 == qc && (dt < 0 || (dt == 0 && dp < 0)));   // P:36 total order
+          if (!beats) continue;
+#pragma unroll
+          for (int mt = -1; mt <= 1; ++mt)
+#pragma unroll
+            for (int mp = -1; mp <= 1; ++mp) {
+              if (mt == 0 && mp == 0) continue;
+              if (mt - dt > 1 || dt - mt > 1 || mp - dp > 1 || dp - mp > 1) continue;
+              if (nq[mt + 1][mp + 1] + eps >= qc) dead = true;
+            }
+        }
+      if (!dead) atomicOr(&s.rowmask[tl * 8u + (pad >> 5)], 1u << (pad & 31u));
+    }
+    __syncthreads();
+    // ---- rank rows: rowpre[tl] = survivors in rows < tl --------------------------------------
+    if (threadIdx.x < 32) {
+      u32 cnt[5], t = 0u;
+#pragma unroll
+      for (int k = 0; k < 5; ++k) {
+        u32 tl = threadIdx.x * 5u + (u32)k;
+        u32 n = 0u;
+        if (tl < TPC_TT) {
+#pragma unroll
+          for (int w = 0; w < 8; ++w) n += __popc(s.rowmask[tl * 8u + w]);
+        }
+        cnt[k] = n; t += n;
+      }
+      u32 inc = t;
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) { u32 o = __shfl_up_sync(0xFFFFFFFFu, inc, d); if ((int)threadIdx.x >= d) inc += o; }
+      u32 ex = inc - t;
+#pragma unroll
+      for (int k = 0; k < 5; ++k) { u32 tl = threadIdx.x * 5u + (u32)k; if (tl < TPC_TT) s.rowpre[tl] = ex; ex += cnt[k]; }
+      if (threadIdx.x == 31) {
+        s.misc[1] = inc;
+        if (MODE == TPC_MODE_DET_COUNT) a.tile_cnt[tile] = inc;
+        if (MODE == TPC_MODE_FAST) s.base[0] = atomicAdd(a.n_clusters, (u64)inc);
+        if (MODE == TPC_MODE_DET_EMIT) s.base[0] = a.block_prefix[tile / TPC_SCAN_PER_CTA] + a.tile_local[tile];
+      }
+    }
+    if (MODE == TPC_MODE_DET_COUNT) continue;
+    __syncthreads();
+    const u64 base = s.base[0];
+
+    // ---- O3 + O4 + O5: 5x5 sums, float32 finalisation (every op rounded once, no FMA), emit --
+    for (u32 i = threadIdx.x; i < npk; i += TPC_K6_THREADS) {
+      u32 e = s.peaks[i];
+      u32 tl = e >> 8, pad = e & 0xFFu;
+      u32 w = pad >> 5, bitpos = pad & 31u;
+      u32 mword = s.rowmask[tl * 8u + w];
+      if (!((mword >> bitpos) & 1u)) continue;
+      u32 rank = s.rowpre[tl] + __popc(mword & ((1u << bitpos) - 1u));
+      for (u32 k = 0; k < w; ++k) rank += __popc(s.rowmask[tl * 8u + k]);
+      const u16* c = s.tile + tl * pitch + pad + TPC_HALO;
+      u32 Q = 0u, Spp = 0u, Stt = 0u;
+      int Sp = 0, St = 0;
+#pragma unroll
+      for (int dt = -2; dt <= 2; ++dt)
+#pragma unroll
+        for (int dp = -2; dp <= 2; ++dp) {
+          u32 q = c[dt * (int)pitch + dp] & 0x3FFu;
+          Q += q; Sp += (int)q * dp; St += (int)q * dt;
+          Spp += q * (u32)(dp * dp); Stt += q * (u32)(dt * dt);
+        }
+      int Vp = (int)(Q * Spp) - Sp * Sp, Vt = (int)(Q * Stt) - St * St;
+      u32 qc = c[0] & 0x3FFu;
+      int t = t_base + (int)tl;
+      float fQ = __uint2float_rn(Q);
+      float pm = __fadd_rn(__uint2float_rn(pad), __fdiv_rn(__int2float_rn(Sp), fQ));
+      float tm = __fadd_rn(__int2float_rn(t), __fdiv_rn(__int2float_rn(St), fQ));
+      float sp = __fdiv_rn(__fsqrt_rn(__int2float_rn(Vp)), fQ);
+      float st = __fdiv_rn(__fsqrt_rn(__int2float_rn(Vt)), fQ);
+      u32 fl = 0u;
+      if (pad < 2u || pad + 2u >= npads) fl |= 1u;
+      if (t < 2 || (u32)t + 2u >= PRM(n_time)) fl |= 2u;
+      if (qc == 1023u) fl |= 4u;
+      u64 slot = base + rank;
+      if (slot < a.capacity) {
+        a.out[slot * 2u] = make_uint4(__float_as_uint(pm), __float_as_uint(tm), __float_as_uint(sp), __float_as_uint(st));
+        a.out[slot * 2u + 1u] = make_uint4(Q, qc | ((u32)t << 16), pad | (row << 8) | (sector << 16) | (fl << 24), 0u);
+      } else {
+        atomicOr(a.status, TPC_STATUS_OVERFLOW);
+      }
+    }
+  }
+}
+
+extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, 4) k_cluster_tiles_fast(K6Args a) {
+  extern __shared__ __align__(16) u32 smem_u32[];
+  k6_body<TPC_MODE_FAST>(a, smem_u32);
+}
+extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, 4) k_cluster_tiles_det_count(K6Args a) {
+  extern __shared__ __align__(16) u32 smem_u32[];
+  k6_body<TPC_MODE_DET_COUNT>(a, smem_u32);
+}
+extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, 4) k_cluster_tiles_det_emit(K6Args a) {
+  extern __shared__ __align__(16) u32 smem_u32[];
+  k6_body<TPC_MODE_DET_EMIT>(a, smem_u32);
+}
+extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, 4) k_cluster_tiles_dump_map(K6Args a) {
+  extern __shared__ __align__(16) u32 smem_u32[];
+  k6_body<TPC_MODE_DUMP_MAP>(a, smem_u32);
+}

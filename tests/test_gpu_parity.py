@@ -1,0 +1,275 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element
+on the same seeded digits.  Bar (NS / DESIGN.md): DETERMINISTIC = byte-identical cluster
+array (set, order, every field); FAST = identical cluster set after sorting by key,
+integer fields exact, float fields within 1e-4 absolute (in fact bit-equal, Q14)."""
+import json
+import os
+
+import numpy as np
+import pytest
+
+from oracle import t1
+from workloads import make_frame, n_pads_ramp
+
+pytestmark = pytest.mark.gpu
+
+FLOATS = ("pad_mean", "time_mean", "sigma_pad", "sigma_time")
+INTS = ("q_tot", "q_max", "time_peak", "pad_peak", "row", "sector", "flags", "reserved")
+
+
+@pytest.fixture(scope="module")
+def tp(cuda_device):
+    import paper_2511_17018_b200 as tp
+    tp.lib()   # fails loudly if the extension is missing
+    return tp
+
+
+def _key(cl):
+    return (cl["sector"].astype(np.int64) << 32) | (cl["row"].astype(np.int64) << 24) | \
+           (cl["time_peak"].astype(np.int64) << 8) | cl["pad_peak"].astype(np.int64)
+
+
+def _oracle(d_np, S, R, T, pads, thr=6, eps=4):
+    cl, st, cnt = t1.clusterize(d_np.view(t1.DIGIT), S, R, T, pads, thr, eps)
+    assert cnt == len(cl)
+    return cl, st
+
+
+def _check_fast(got, exp):
+    assert len(got) == len(exp)
+    g = got[np.argsort(_key(got), kind="stable")]
+    assert np.array_equal(_key(g), _key(exp))           # identical cluster set
+    for k in INTS:
+        assert np.array_equal(g[k], exp[k]), k
+    for k in FLOATS:
+        assert np.all(np.abs(g[k].astype(np.float64) - exp[k].astype(np.float64)) <= 1e-4), k
+
+
+def _run_both(tp, digits_t, S, R, T, pads, thr=6, eps=4, rtc=False, max_digits=None):
+    import torch
+    c = tp.Clusterizer(S, R, T, pads, max_digits or max(1, digits_t.numel()), thr, eps, rtc=rtc)
+    det, n_det, st_det = c.run_sync(digits_t, tp.MODE_DETERMINISTIC)
+    fast, n_fast, st_fast = c.run_sync(digits_t, tp.MODE_FAST)
+    c.close()
+    assert n_det == len(det) and n_fast == len(fast) and st_det == st_fast
+    return det, fast, st_det
+
+
+def _digits_tensor(d_np, device):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(d_np).view(np.int64).copy()).to(device)
+
+
+@pytest.mark.parametrize("k", [1, 0])
+def test_cfg_small_det_and_fast(tp, cuda_device, k):
+    fr = make_frame(k)
+    d_np = fr.digits_numpy()
+    exp, st = _oracle(d_np, fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads)
+    det, fast, st_gpu = _run_both(tp, fr.digits.to(cuda_device), fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads)
+    assert st_gpu == st == 0
+    assert det.tobytes() == exp.tobytes()               # deterministic mode: bitwise
+    _check_fast(fast, exp)
+    assert fast[np.argsort(_key(fast))].tobytes() == exp.tobytes()   # Q14: fast values are bit-equal too
+
+
+@pytest.mark.parametrize("k", [1, 0])
+def test_dense_map_step_a1(tp, cuda_device, k):
+    """Step a1 (digit -> charge map) in isolation: the tiles the kernels build equal O0's map."""
+    fr = make_frame(k)
+    _, _, _, m = t1.clusterize(fr.digits_numpy().view(t1.DIGIT), fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads,
+                               return_map=True)
+    c = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, fr.n_digits)
+    c.run_sync(fr.digits.to(cuda_device), tp.MODE_FAST)
+    got = c.dense_map().cpu().numpy().view(np.uint16)
+    c.close()
+    assert np.array_equal(got, m)
+
+
+def test_appendix_a_vectors_on_gpu(tp, cuda_device):
+    G = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "appendix_a.json")))
+    P, T = G["n_pads"], G["n_time"]
+    c = tp.Clusterizer(1, 1, T, [P], 64, G["thr_peak"], G["noise_eps"])
+    for case in G["cases"]:
+        d = t1.make_digits([(0, 0, p, t, q) for (p, t, q) in case["digits"]])
+        got, n, st = c.run_sync(_digits_tensor(d, cuda_device), tp.MODE_DETERMINISTIC)
+        assert st == 0 and n == len(case["clusters"]), case["name"]
+        for g, e in zip(got, case["clusters"]):
+            for k2 in ("pad_peak", "time_peak", "q_max", "q_tot", "flags"):
+                if k2 in e:
+                    assert int(g[k2]) == e[k2], (case["name"], k2)
+            for k2 in FLOATS:
+                if k2 in e:
+                    assert int(np.array(g[k2]).view(np.uint32)) == int(e[k2], 16), (case["name"], k2)
+    c.close()
+
+
+def test_permutation_and_repeat_invariance(tp, cuda_device):
+    """I4 / I14 / PAPER.md 47-48: det output is one byte string under any digit order and across runs."""
+    import torch
+    fr = make_frame(1)
+    d = fr.digits.to(cuda_device)
+    c = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, fr.n_digits)
+    ref = c.run_sync(d, tp.MODE_DETERMINISTIC)[0].tobytes()
+    g = torch.Generator(device="cpu").manual_seed(1)
+    for i in range(8):
+        perm = torch.randperm(d.numel(), generator=g).to(cuda_device)
+        assert c.run_sync(d[perm].contiguous(), tp.MODE_DETERMINISTIC)[0].tobytes() == ref
+    assert c.run_sync(torch.sort(d)[0], tp.MODE_DETERMINISTIC)[0].tobytes() == ref
+    for i in range(5):
+        assert c.run_sync(d, tp.MODE_DETERMINISTIC)[0].tobytes() == ref
+    c.close()
+
+
+def test_edge_inputs(tp, cuda_device):
+    import torch
+    pads = [16] * 4
+    c = tp.Clusterizer(2, 4, 300, pads, 64)
+    # empty input
+    cl, n, st = c.run_sync(torch.zeros(0, dtype=torch.int64, device=cuda_device), tp.MODE_DETERMINISTIC)
+    assert n == 0 and st == 0 and len(cl) == 0
+    cl, n, st = c.run_sync(torch.zeros(0, dtype=torch.int64, device=cuda_device), tp.MODE_FAST)
+    assert n == 0 and st == 0
+    # duplicates (Q5: max wins in det mode, either order), clamp, zero charge, out-of-range
+    rows = [(0, 0, 5, 5, 7), (0, 0, 5, 5, 9), (1, 3, 15, 299, 2000), (1, 3, 8, 8, 0),
+            (2, 0, 1, 1, 50), (0, 4, 1, 1, 50), (0, 0, 16, 1, 50), (0, 0, 1, 300, 50)]
+    for order in (rows, rows[::-1]):
+        d = t1.make_digits(order)
+        exp, st_exp = _oracle(d, 2, 4, 300, pads)
+        got, n, st = c.run_sync(_digits_tensor(d, cuda_device), tp.MODE_DETERMINISTIC)
+        assert st == st_exp == tp.STATUS_BAD_DIGITS and got.tobytes() == exp.tobytes() and n == 2
+        assert got[0]["q_tot"] == 9 and got[1]["q_max"] == 1023 and got[1]["flags"] == 7
+    # overflow: true count is returned, first `capacity` clusters in order (det)
+    d = t1.make_digits([(0, 0, 2, 2 + 10 * i, 50 + i) for i in range(20)])
+    exp, _ = _oracle(d, 2, 4, 300, pads)
+    got, n, st = c.run_sync(_digits_tensor(d, cuda_device), tp.MODE_DETERMINISTIC, capacity=7)
+    assert n == 20 and st == tp.STATUS_OVERFLOW and got.tobytes() == exp[:7].tobytes()
+    got, n, st = c.run_sync(_digits_tensor(d, cuda_device), tp.MODE_FAST, capacity=7)
+    assert n == 20 and st == tp.STATUS_OVERFLOW
+    c.close()
+
+
+def test_idempotent_between_different_inputs(tp, cuda_device):
+    """Q17: output never depends on an earlier run (stale workspace contents)."""
+    a, b = make_frame(1), make_frame(1, seed=99)
+    c = tp.Clusterizer(a.n_sectors, a.n_rows, a.n_time, a.n_pads, max(a.n_digits, b.n_digits))
+    ra = c.run_sync(a.digits.to(cuda_device), tp.MODE_DETERMINISTIC)[0].tobytes()
+    rb = c.run_sync(b.digits.to(cuda_device), tp.MODE_DETERMINISTIC)[0].tobytes()
+    assert c.run_sync(a.digits.to(cuda_device), tp.MODE_DETERMINISTIC)[0].tobytes() == ra and ra != rb
+    exp, _ = _oracle(b.digits_numpy(), b.n_sectors, b.n_rows, b.n_time, b.n_pads)
+    assert rb == exp.tobytes()
+    c.close()
+
+
+def test_thresholds_follow_params(tp, cuda_device):
+    """Constant buffers may change between time frames (PAPER.md 79): two handles with different
+    thresholds in one process each follow their own parameters."""
+    fr = make_frame(1)
+    d = fr.digits.to(cuda_device)
+    c1 = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, fr.n_digits, thr_peak=6, noise_eps=4)
+    c2 = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, fr.n_digits, thr_peak=20, noise_eps=0)
+    for c, thr, eps in ((c1, 6, 4), (c2, 20, 0), (c1, 6, 4)):
+        exp, _ = _oracle(fr.digits_numpy(), fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, thr, eps)
+        assert c.run_sync(d, tp.MODE_DETERMINISTIC)[0].tobytes() == exp.tobytes()
+    c1.close(); c2.close()
+
+
+def test_rtc_equals_generic(tp, cuda_device):
+    """I13 / PAPER.md 91: the run-time-compiled variant changes speed only, never results."""
+    fr = make_frame(1)
+    exp, _ = _oracle(fr.digits_numpy(), fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads)
+    det, fast, st = _run_both(tp, fr.digits.to(cuda_device), fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, rtc=True)
+    assert det.tobytes() == exp.tobytes() and st == 0
+    _check_fast(fast, exp)
+
+
+def test_multi_time_chunk_geometry(tp, cuda_device):
+    """n_time > 16256 exercises the coarse time-chunk halo copies of K1 (n_tc = 3), with clusters
+    planted across both chunk borders and random digits elsewhere."""
+    rng = np.random.default_rng(17)
+    T, pads = 40000, [24, 40]
+    rows = []
+    for tb in (16256, 32512):
+        for dt in range(-6, 7):
+            for r in (0, 1):
+                rows.append((0, r, 10 + (dt % 5), tb + dt, int(rng.integers(3, 200))))
+                rows.append((0, r, 3, tb + dt, 60))
+    n = 20000
+    t = rng.integers(0, T, n); r = rng.integers(0, 2, n); p = rng.integers(0, 24, n); q = rng.integers(1, 120, n)
+    seen = {(x[1], x[2], x[3]) for x in rows}
+    for i in range(n):
+        key = (int(r[i]), int(p[i]), int(t[i]))
+        if key not in seen:
+            seen.add(key)
+            rows.append((0, key[0], key[1], key[2], int(q[i])))
+    d = t1.make_digits(rows)
+    d = d[rng.permutation(len(d))]
+    exp, st_exp = _oracle(d, 1, 2, T, pads)
+    det, fast, st = _run_both(tp, _digits_tensor(d, cuda_device), 1, 2, T, pads)
+    assert st == st_exp == 0 and det.tobytes() == exp.tobytes()
+    _check_fast(fast, exp)
+
+
+def test_dense_adversarial_tile(tp, cuda_device):
+    """Maximum sizes: a fully occupied 138-pad row over 600 time bins with heavy ties (values 5..9),
+    plus a checkerboard (the densest possible peak pattern) -- stresses the peak list bound,
+    tie-breaking and the rank-by-bitmask emission."""
+    rng = np.random.default_rng(23)
+    T, P = 600, 138
+    q = rng.integers(5, 10, size=(T, P))
+    cb = np.zeros((T, P), dtype=np.int64)
+    cb[::2, ::2] = 50
+    rows = [(0, 0, p, t, int(q[t, p])) for t in range(T) for p in range(P)]
+    rows += [(0, 1, p, t, 50) for t in range(0, T, 2) for p in range(0, P, 2)]
+    d = t1.make_digits(rows)
+    d = d[rng.permutation(len(d))]
+    exp, _ = _oracle(d, 1, 2, T, [P, P])
+    det, fast, st = _run_both(tp, _digits_tensor(d, cuda_device), 1, 2, T, [P, P])
+    assert st == 0 and det.tobytes() == exp.tobytes()
+    _check_fast(fast, exp)
+    assert (exp["row"] == 1).sum() == (T // 2) * (P // 2)   # every checkerboard cell is its own cluster
+
+
+def test_skewed_input_one_bin(tp, cuda_device):
+    """All digits in one (sector,row): the write-combining stage of K1 overflows every round and
+    the bin spans many K5 batches; results must not change."""
+    rng = np.random.default_rng(29)
+    T, P = 14256, 100
+    n = 300000
+    cell = rng.choice(T * P, size=n, replace=False)
+    rows = np.zeros(n, dtype=t1.DIGIT)
+    rows["time"], rows["pad"] = cell // P, cell % P
+    rows["row"], rows["sector"] = 3, 1
+    rows["charge"] = rng.integers(3, 300, n)
+    exp, _ = _oracle(rows, 2, 5, T, [P] * 5)
+    det, fast, st = _run_both(tp, _digits_tensor(rows, cuda_device), 2, 5, T, [P] * 5)
+    assert st == 0 and det.tobytes() == exp.tobytes()
+    _check_fast(fast, exp)
+
+
+def test_run_host_e2e(tp, cuda_device):
+    import torch
+    fr = make_frame(0)
+    exp, _ = _oracle(fr.digits_numpy(), fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads)
+    c = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, fr.n_digits, host_capacity=fr.n_digits)
+    dh = fr.digits.pin_memory()
+    out = torch.empty((fr.n_digits, 32), dtype=torch.uint8).pin_memory()
+    n, st = c.run_host(dh, out, tp.MODE_DETERMINISTIC)
+    assert n == len(exp) and st == 0
+    assert out[:n].numpy().tobytes() == exp.tobytes()
+    n, st = c.run_host(dh, out, tp.MODE_FAST)
+    got = out[:n].numpy().view(tp.CLUSTER_DTYPE).reshape(-1)
+    _check_fast(got, exp)
+    c.close()
+
+
+def test_full_geometry_sector_slice(tp, cuda_device):
+    """CFG[2]/CFG[4] recipe on the full 36x152 ramp geometry, cut to a short time window so the
+    oracle finishes in seconds: several tiles per row, ragged last slab (T = 300), all row widths."""
+    for k in (2, 4):
+        fr = make_frame(k, device=cuda_device, sectors=[0, 7, 35], n_time=300)
+        d_np = fr.digits_numpy()
+        exp, _ = _oracle(d_np, fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads)
+        det, fast, st = _run_both(tp, fr.digits, fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads)
+        assert st == 0 and len(exp) > 1000
+        assert det.tobytes() == exp.tobytes()
+        _check_fast(fast, exp)
