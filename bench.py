@@ -1,0 +1,301 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the TPC clusterizer hot path on synthetic time frames.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--order shuffled]
+                    [--mode fast|det] [--rtc] [--impl reference]
+
+One "step" = one pass of the whole hot path (K1..K6 of
+DESIGN.md) over one Pb-Pb-like time frame (BASELINE.json configs[4]) that is already
+resident in HBM.  Prints ONE JSON line (contract in the task statement): metric value in
+digits/s, e2e through tpcclus_run_host (host buffers, copies inside the timed region),
+per-kernel roofline of the dominant kernel from CUDA events recorded on the run's stream,
+and the CPU oracle timed on a bounded sample of the same frame.
+
+N > 1 (torchrun): the path shards by time frame -- every rank clusterizes its own frame
+(seed + rank), no data-path collective (PAPER.md 97: one process per GPU, whole time
+frames each); value = digits of all ranks / max-over-ranks time; scaling "weak".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+_T0 = time.perf_counter()
+
+
+def _log(msg):
+    print("[bench %7.1fs] %s" % (time.perf_counter() - _T0, msg), file=sys.stderr, flush=True)
+
+
+METRIC = "TPC clusterizer digits/s on Pb-Pb-like time frame"
+UNIT = "digits/s"
+
+
+def _peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons sampled during the timed region."""
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        self.index, self.rows, self._stop, self._t = index, [], threading.Event(), None
+
+    def _loop(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                self.rows.append([x.strip() for x in out.strip().split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def __enter__(self):
+        self._t = threading.Thread(target=self._loop, daemon=True)
+        self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._t.join(timeout=6)
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+                for nm, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                pass
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def _oracle_sample(fr_digits_np, fr, n_sample_sectors):
+    """The oracle as it stands, single thread, on the first sectors of the frame."""
+    from oracle import t1
+    d = fr_digits_np.view(t1.DIGIT)
+    sub = np.ascontiguousarray(d[d["sector"] < n_sample_sectors])
+    tm = {}
+    cl, st, cnt = t1.clusterize(sub, n_sample_sectors, fr.n_rows, fr.n_time, fr.n_pads, capacity=max(len(sub) // 4, 1024), timing=tm)
+    return len(sub), cnt, tm["seconds"]
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle (oracle/, single thread) on bounded samples of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import torch
+    from workloads import make_frame
+    k = args.config
+    n_sec = 1 if k >= 2 else None
+    dev = "cuda" if torch.cuda.is_available() else "cpu"
+    if k >= 2:
+        fr = make_frame(k, device=dev, order=args.order, sectors=[0])
+    else:
+        fr = make_frame(k, order=args.order)
+    d_np = fr.digits_numpy()
+    times, nd = [], 0
+    for i in range(args.warmup + args.steps):
+        nd, cnt, sec = _oracle_sample(d_np, fr, 1 if k >= 2 else fr.n_sectors)
+        if i >= args.warmup:
+            times.append(sec)
+    t = float(np.mean(times))
+    val = nd / t
+    sample = "sector 0 of the %s frame (%d digits) per step, single thread" % (fr.meta["name"], nd)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "int32+f32", "data": "synthetic",
+        "config": {"workload": fr.meta["name"], "order": args.order, "n_digits": nd, "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--order", default="shuffled", choices=["shuffled", "readout", "cell"])
+    ap.add_argument("--mode", default="fast", choices=["fast", "det"])
+    ap.add_argument("--rtc", action="store_true")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-sectors", type=int, default=2)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+
+    import paper_2511_17018_b200 as tp
+    from workloads import SEED_BASE, make_frame
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device; there is no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    tp.lib()
+
+    k = args.config
+    fr = make_frame(k, device=dev, order=args.order, seed=SEED_BASE + k + 1000 * rank)
+    digits = fr.digits
+    n = fr.n_digits
+    torch.cuda.synchronize(dev)
+    _log("frame generated: %d digits" % n)
+    mode = tp.MODE_FAST if args.mode == "fast" else tp.MODE_DETERMINISTIC
+    c = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, n, rtc=args.rtc, device=local)
+    # size the output from a first (untimed) run
+    probe_cap = max(n // 3, 1024)
+    clusters = torch.empty((probe_cap, 32), dtype=torch.uint8, device=dev)
+    _, nt, stt = c.run(digits, mode, clusters=clusters)
+    torch.cuda.synchronize(dev)
+    n_clusters, status = int(nt.item()), int(stt.item())
+    assert status == 0 and n_clusters <= probe_cap, (status, n_clusters, probe_cap)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    for _ in range(max(args.warmup, 3)):
+        c.run(digits, mode, clusters=clusters)
+    c.set_timing(True)
+    per_kernel = {}
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clk:
+        e0.record()
+        for _ in range(args.steps):
+            c.run(digits, mode, clusters=clusters)
+            for nm, ms in c.last_timing():      # events recorded on the run's stream, inside the timed region
+                per_kernel.setdefault(nm, []).append(ms)
+        e1.record()
+        barrier()
+    ms_total = e0.elapsed_time(e1)
+    c.set_timing(False)
+    _log("timed region done: %.3f ms/step" % (ms_total / args.steps))
+    t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+    tot_digits = torch.tensor([float(n)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tot_digits, op=dist.ReduceOp.SUM)
+    ms_step = float(t.item()) / args.steps
+    value = float(tot_digits.item()) / (ms_step * 1e-3)
+
+    # ---- e2e: host buffers through tpcclus_run_host, copies inside the timed region -----------
+    e2e = None
+    if args.e2e_steps > 0:
+        cap = n_clusters + 1024
+        c.close()
+        del c, clusters
+        torch.cuda.empty_cache()
+        c = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, n, rtc=args.rtc, device=local, host_capacity=cap)
+        h_digits = torch.empty(n, dtype=torch.int64).pin_memory()
+        h_digits.copy_(digits)
+        h_clusters = torch.empty((cap, 32), dtype=torch.uint8).pin_memory()
+        _log("pinned host buffers ready")
+        c.run_host(h_digits, h_clusters, mode)      # warm-up
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            n_e2e, st_e2e = c.run_host(h_digits, h_clusters, mode)
+        barrier()
+        sec = (time.perf_counter() - t0) / args.e2e_steps
+        assert n_e2e == n_clusters and st_e2e == 0
+        te = torch.tensor([sec], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        e2e = {"value": float(tot_digits.item()) / float(te.item()), "unit": UNIT, "h2d_bytes_per_step": 8 * n,
+               "d2h_bytes_per_step": 32 * n_clusters + 16, "ms_per_step": float(te.item()) * 1e3,
+               "api": "tpcclus_run_host (pinned host buffers)"}
+        del h_clusters
+        _log("e2e done")
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (algorithmic bytes per launch) ---
+    peak, peak_src = _peaks()
+    avg = {nm: float(np.mean(v)) for nm, v in per_kernel.items()}
+    n_rec_fine = None
+    alg = {   # bytes one launch must move (per-unit figures x units of this frame)
+        "k_partition_coarse": 8 * n + 4 * n,                    # read every digit once, write one 4-byte record
+        "k_partition_fine": 4 * n + 4 * n,                      # read the records, write them tile-sorted
+        "k_cluster_tiles_fast": 4 * n + 32 * n_clusters,        # read the tile records, write the clusters
+        "k_cluster_tiles_det_count": 4 * n,
+        "k_cluster_tiles_det_emit": 4 * n + 32 * n_clusters,
+    }
+    dom = max(avg, key=lambda nm: avg[nm])
+    roof = None
+    if dom in alg:
+        ach = alg[dom] / (avg[dom] * 1e-3) / 1e9
+        roof = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                "traffic": None, "peak_source": peak_src, "kernel_ms": avg[dom],
+                "share_of_step": avg[dom] / sum(avg.values())}
+    b_alg = 8 * n + 32 * n_clusters
+    method = {"b_alg_bytes": b_alg, "achieved_gbs": b_alg / (ms_step * 1e-3) / 1e9,
+              "frac_of_peak": b_alg / (ms_step * 1e-3) / 1e9 / peak}
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        h = fr.digits_numpy() if e2e is None else h_digits.numpy().view(np.uint64)
+        ns = min(args.cpu_sectors, fr.n_sectors)
+        _log("cpu baseline: filtering sample")
+        nd, cnt, sec = _oracle_sample(h, fr, ns)
+        _log("cpu baseline done")
+        cpu = {"value": nd / sec, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": "sectors 0..%d of this frame (%d digits, %d clusters) in %.1f s, single thread" % (ns - 1, nd, cnt, sec)}
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "int32+f32", "data": "synthetic",
+        "config": {"workload": fr.meta["name"], "order": args.order, "mode": args.mode, "rtc": bool(args.rtc),
+                   "n_digits": n, "n_clusters": n_clusters, "occupancy": fr.meta["occupancy"],
+                   "checksum": "%016x" % fr.meta["checksum"], "l2": "inputs (%.1f GB) larger than L2" % (8 * n / 1e9)},
+        "clocks": clk.summary(), "e2e": e2e, "gpu_launches": c.launches_per_run(mode) * args.steps,
+        "roofline": roof, "method_roofline": method, "kernels_ms": avg, "cpu_baseline": cpu,
+    }
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
