@@ -249,15 +249,46 @@ def _gen_cfg1(cfg, pads, seed, device):
     return pack_digits(torch.zeros_like(r), r, p, t, q), truth
 
 
+def _feistel_perm(n: int, seed: int, device) -> torch.Tensor:
+    """A seeded bijection of [0, n) from elementwise ops only: a 6-round Feistel network on
+    the next even power-of-two domain, cycle-walked back into range.  Used for the full
+    time frames, where torch.randperm (n >= 2^30 on CUDA) takes many minutes."""
+    k = max(2, (n - 1).bit_length())
+    k += k & 1
+    h = k // 2
+    mask = (1 << h) - 1
+    keys = [((seed + 0x9E3779B1 * (r + 1)) * 0x85EBCA6B) & 0x7FFFFFFF for r in range(6)]
+
+    def f(x):
+        L, R = x >> h, x & mask
+        for key in keys:
+            y = (R * 0x2545F491 + key) & 0xFFFFFFFFFFFF          # < 2^48: no int64 overflow
+            y = ((y ^ (y >> 15)) * 0x2C1B3C6D) & 0xFFFFFFFFFFFF
+            y = (y ^ (y >> 13)) & mask
+            L, R = R, L ^ y
+        return (L << h) | R
+
+    x = f(torch.arange(n, dtype=torch.int64, device=device))
+    bad = (x >= n).nonzero(as_tuple=False).squeeze(1)
+    while bad.numel():
+        v = f(x[bad])
+        x[bad] = v
+        bad = bad[v >= n]
+    return x
+
+
 def _order(digits: torch.Tensor, order: str, seed: int) -> torch.Tensor:
     """Q23 input order.  'shuffled': one global seeded permutation (headline).
     'readout': grouped by sector, then 128-bin time slab, shuffled inside."""
     n = digits.numel()
     if n == 0 or order == "cell":
         return digits
-    g = torch.Generator(device=digits.device)
-    g.manual_seed((seed * 2654435761 + 97) & 0x7FFFFFFFFFFFFFFF)
-    perm = torch.randperm(n, generator=g, device=digits.device)
+    if n >= (1 << 28):
+        perm = _feistel_perm(n, seed, digits.device)
+    else:
+        g = torch.Generator(device=digits.device)
+        g.manual_seed((seed * 2654435761 + 97) & 0x7FFFFFFFFFFFFFFF)
+        perm = torch.randperm(n, generator=g, device=digits.device)
     if order == "shuffled":
         return digits[perm]
     if order == "readout":
