@@ -85,7 +85,7 @@ int make_geometry(const tpcclus_params* p, Geometry* g) {
   q.max_pads = maxp;
   q.pitch = (maxp + 2 * TPC_HALO + 7) / 8 * 8;
   q.thr_peak = p->thr_peak; q.noise_eps = p->noise_eps;
-  q.max_peaks = ((TPC_TS + 1) / 2) * ((maxp + 1) / 2);
+  q.max_peaks = ((TPC_TT - 2 + 1) / 2) * ((maxp + 1) / 2);   // no two peaks are 8-neighbours; rows 1..TT-2 are scanned
 
   g->max_digits = p->max_digits;
   g->g1 = (uint32_t)sm_count(p->device);
@@ -334,7 +334,7 @@ int tpcclus_create(const tpcclus_params* p, tpcclus_handle** out) {
   h->smem_k5 = (TPC_K5_BUF + 128u * 3u + 132u + 8u) * 4u;
   h->smem_k6 = tpc_k6_smem_bytes(g.prm.pitch, g.prm.max_peaks);
   h->grid_k5 = g.g1 * 2u;
-  h->grid_k6 = g.g1 * 4u < g.n_tiles ? g.g1 * 4u : g.n_tiles;
+  h->grid_k6 = g.g1 * 3u < g.n_tiles ? g.g1 * 3u : g.n_tiles;
   auto bail = [&](int code) { std::string e = h->err.empty() ? g_create_error : h->err; delete h; g_create_error = e; return code; };
   // static table for the debug map hook
   std::vector<uint64_t> ro(p->n_rows + 1, 0);

@@ -33,7 +33,6 @@ typedef unsigned char u8;
 #define TPC_K1_THREADS 1024
 #define TPC_K1_DPT 4           // digits per thread per round
 #define TPC_K5_THREADS 512
-#define TPC_K6_THREADS 256
 #define TPC_SCAN_THREADS 1024
 #define TPC_SCAN_PER_CTA 4096u
 
@@ -65,9 +64,6 @@ __constant__ TpcParams c_prm;
 // ---- shared-memory sizes (bytes); the host launches with exactly these --------------------
 __host__ __device__ inline u32 tpc_k1_smem_bytes(u32 nb) {
   return (nb * TPC_STAGE + nb + ((nb + 1u) >> 1) + 4u) * 4u + 512u;
-}
-__host__ __device__ inline u32 tpc_k6_smem_bytes(u32 pitch, u32 max_peaks) {
-  return (TPC_TT * pitch / 2u + 2u * 256u + 2u + (max_peaks + 1u) / 2u + TPC_TT * 8u + TPC_TT + 2u + 256u + 1u + 8u + 4u) * 4u + 16u;
 }
 
 // ---- small PTX helpers -------------------------------------------------------------------
@@ -490,6 +486,10 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
         }
       }
     }
+    if (threadIdx.x >= 128u && threadIdx.x < 128u + nsl) {   // zero the padding of every run (K6 skips record 0)
+      const u32 sl = threadIdx.x - 128u;
+      for (u32 k = s_off[sl] + s_cnt[sl] + s_dcnt[sl]; k < s_off[sl + 1u]; ++k) buf[k] = 0u;
+    }
     __syncthreads();
     // ---- dump the sorted batch + its index entries -----------------------------------------
     const u64 gbase = s_gbase;
@@ -509,18 +509,26 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
 // ==========================================================================================
 // K6  cluster_tiles  (NS (1) last step + (2) + (3) + (4); rules O0..O5 of SURVEY.md 8(c))
 //
-// Persistent CTAs; one tile = (bin, slab) at a time.  The tile's charge map lives in shared
-// memory as u16 [TPC_TT][pitch] with 3 zero guard pads on each side; bit 15 of a cell marks
-// a peak (O1).  Survivors of O2 are marked in a per-row pad bitmask, which gives every
-// cluster its rank in (time, pad) order inside the tile without a sort; the base of the
-// tile comes from one atomic (FAST) or from the exclusive scan of the tile counts
-// (DETERMINISTIC: K6 runs once to count, K7/K8 scan, K6 runs again to emit).
+// Persistent CTAs of 8 consumer warps + 1 producer warp; one tile = (bin, slab) at a time.
+// The producer warp stages the tile's record runs into shared memory with 1-D bulk copies
+// (cp.async.bulk -> mbarrier complete_tx) one tile ahead of the consumers, so no consumer
+// ever waits on a global load.  The consumers build the tile's charge map in shared memory
+// as u16 [TPC_TT][pitch] with 3 zero guard pads on each side (O0), find the 3x3 peaks with a
+// dense scan on packed u16x2 words (O1: a rolling 3-row window per word column, 2 cells per
+// max.u16x2), mark peaks with bit 15, run the suppression per listed peak (O2), mark the
+// survivors in a per-row pad bitmask -- which ranks every cluster in (time, pad) order inside
+// the tile without a sort -- and finalise the 5x5 sums (O3/O4).  The base of the tile comes
+// from one atomic (FAST) or from the exclusive scan of the tile counts (DETERMINISTIC: K6
+// runs once to count, K7/K8 scan, K6 runs again to emit).
 // ==========================================================================================
 #define TPC_MODE_FAST 0
 #define TPC_MODE_DET_COUNT 1
 #define TPC_MODE_DET_EMIT 2
 #define TPC_MODE_DUMP_MAP 3
-#define TPC_K6_GROUP 256u   // index entries (runs) handled per pass
+#define TPC_K6_CONSUMERS 256u                   // threads that compute
+#define TPC_K6_THREADS (TPC_K6_CONSUMERS + 32u)  // + the producer warp
+#define TPC_K6_CAP 4096u                         // records staged per round (16 KB)
+#define TPC_K6_CAPU (TPC_K6_CAP / 4u)            // ... in 16-byte units
 
 struct K6Args {
   const u32* blob; const u64* idx; const u32* batch_start;
@@ -529,68 +537,91 @@ struct K6Args {
   u16* dmap; const u64* row_off;   // DUMP_MAP only: row_off[r] = cells of rows < r in one sector; [n_rows] = per sector
 };
 
+// ---- mbarrier / bulk-copy / packed-max helpers (PTX; SASS: SYNCS.*, UBLKCP, VIMNMX3.U16x2) --
+__device__ __forceinline__ u32 smem_addr(const void* p) { u64 a; asm("cvta.to.shared.u64 %0, %1;" : "=l"(a) : "l"(p)); return (u32)a; }
+__device__ __forceinline__ void mbar_init(u64* bar, u32 count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(u64* bar, u32 bytes) {
+  asm volatile("mbarrier.expect_tx.relaxed.cta.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(u64* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_addr(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(u64* bar, u32 parity) {
+  u32 ok;
+  do {
+    asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+                 : "=r"(ok) : "r"(smem_addr(bar)), "r"(parity) : "memory");
+  } while (!ok);
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, u32 bytes, u64* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_addr(dst)), "l"(src), "r"(bytes), "r"(smem_addr(bar)) : "memory");
+}
+__device__ __forceinline__ u32 vmax2(u32 a, u32 b) { u32 d; asm("max.u16x2 %0, %1, %2;" : "=r"(d) : "r"(a), "r"(b)); return d; }
+// barrier 1 = the 256 consumer threads only (the producer warp never joins it)
+__device__ __forceinline__ void csync() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
+__device__ __forceinline__ u32 csync_or(u32 v) {
+  u32 r;
+  asm volatile("{\n.reg .pred p, q;\nsetp.ne.u32 p, %1, 0;\nbar.red.or.pred q, 1, 256, p;\nselp.u32 %0, 1, 0, q;\n}"
+               : "=r"(r) : "r"(v) : "memory");
+  return r;
+}
+
 struct K6Smem {
-  u16* tile; u32* tile32; u16* peaks; u32* rowmask; u32* rowpre; u64* rpos; u32* rpre; u32* wsum; u32* misc; u64* base;
+  u32* rec;        // [TPC_K6_CAP] staged records of one round
+  u16* tile; u32* tile32;
+  u64* bar;        // [0] full (producer -> consumers), [1] empty (consumers -> producer)
+  u64* base;
+  u32* rowmask; u32* rowpre; u32* misc; u16* peaks;
 };
+// misc: [0] n_peaks  [1] survivors  [2] total 16-byte units of the tile being staged
+__host__ __device__ inline u32 tpc_k6_smem_bytes(u32 pitch, u32 max_peaks) {
+  return (TPC_K6_CAP + TPC_TT * pitch / 2u + 4u + 2u + TPC_TT * 8u + TPC_TT + 2u + 8u + (max_peaks + 1u) / 2u) * 4u + 128u;
+}
 __device__ __forceinline__ K6Smem k6_smem(u32* p) {
   K6Smem s;
-  const u32 tile_words = TPC_TT * PRM(pitch) / 2u;
-  s.tile32 = p; s.tile = (u16*)p; p += tile_words;
-  s.rpos = (u64*)p; p += 2u * TPC_K6_GROUP;
+  p = (u32*)(((u64)p + 127ull) & ~127ull);   // bulk copies need 16-byte aligned destinations
+  s.rec = p; p += TPC_K6_CAP;
+  s.tile32 = p; s.tile = (u16*)p; p += TPC_TT * PRM(pitch) / 2u;
+  s.bar = (u64*)p; p += 4;
   s.base = (u64*)p; p += 2;
-  s.peaks = (u16*)p; p += (PRM(max_peaks) + 1u) / 2u;
   s.rowmask = p; p += TPC_TT * 8u;
   s.rowpre = p; p += TPC_TT + 2u;
-  s.rpre = p; p += TPC_K6_GROUP + 1u;
-  s.wsum = p; p += 8;
-  s.misc = p;   // [0] n_peaks, [1] total survivors
+  s.misc = p; p += 8;
+  s.peaks = (u16*)p;
   return s;
 }
 
-// loads index entries [g0, g0+ng) of this tile into shared memory and scans their counts.
-__device__ __forceinline__ u32 k6_load_group(const K6Smem& s, const u64* __restrict__ idx, u64 ib, u32 g0, u32 ng) {
-  u32 c = 0u;
-  if (threadIdx.x < ng) {
-    u64 e = idx[ib + g0 + threadIdx.x];
-    s.rpos[threadIdx.x] = e & ((1ull << 40) - 1ull);
-    c = (u32)(e >> 40);
-  }
-  u32 inc = c;
+// Producer warp: stages round `round` of a tile -- the 16-byte units [round*CAPU, (round+1)*CAPU)
+// of the concatenation of the tile's runs (one run per K5 batch of the bin, 32-byte aligned and
+// zero-padded by K5) -- and arrives on the full barrier.  Returns the tile's total units.
+__device__ __forceinline__ u32 k6_stage(const K6Smem& s, const K6Args& a, u64 ib, u32 nbatch, u32 round) {
+  const u32 lane = lane_id();
+  const u32 lo = round * TPC_K6_CAPU, hi = lo + TPC_K6_CAPU;
+  u32 pos = 0u;
+  for (u32 g0 = 0u; g0 < nbatch; g0 += 32u) {
+    const u32 g = g0 + lane;
+    u64 e = g < nbatch ? a.idx[ib + g] : 0ull;
+    const u32 units = ((u32)(e >> 40) + 3u) >> 2;
+    const u64 src = e & ((1ull << 40) - 1ull);
+    u32 inc = units;
 #pragma unroll
-  for (int d = 1; d < 32; d <<= 1) { u32 o = __shfl_up_sync(0xFFFFFFFFu, inc, d); if ((int)lane_id() >= d) inc += o; }
-  if (lane_id() == 31u) s.wsum[threadIdx.x >> 5] = inc;
-  __syncthreads();
-  u32 wp = 0u;
-  for (u32 w = 0; w < (threadIdx.x >> 5); ++w) wp += s.wsum[w];
-  s.rpre[threadIdx.x + 1u] = wp + inc;   // inclusive -> rpre[i+1]
-  if (threadIdx.x == 0) s.rpre[0] = 0u;
-  __syncthreads();
-  return s.rpre[TPC_K6_GROUP];
-}
-
-// calls f(record) for every record of the loaded group, flat over the block.
-template <class F>
-__device__ __forceinline__ void k6_for_records(const K6Smem& s, const u32* __restrict__ blob, u32 total, F f) {
-  u32 run = 0u;
-  for (u32 j = threadIdx.x; j < total; j += TPC_K6_THREADS) {
-    while (j >= s.rpre[run + 1u]) ++run;
-    f(blob[s.rpos[run] + (j - s.rpre[run])]);
-  }
-}
-
-// runs f over ALL records of the tile (several groups only for bins with > 256 batches).
-template <class F>
-__device__ __forceinline__ void k6_phase(const K6Smem& s, const K6Args& a, u64 ib, u32 nbatch, u32 total0, F f) {
-  if (nbatch <= TPC_K6_GROUP) {
-    k6_for_records(s, a.blob, total0, f);
-  } else {
-    for (u32 g0 = 0u; g0 < nbatch; g0 += TPC_K6_GROUP) {
-      u32 ng = nbatch - g0 < TPC_K6_GROUP ? nbatch - g0 : TPC_K6_GROUP;
-      __syncthreads();
-      u32 t = k6_load_group(s, a.idx, ib, g0, ng);
-      k6_for_records(s, a.blob, t, f);
+    for (int d = 1; d < 32; d <<= 1) { u32 o = __shfl_up_sync(0xFFFFFFFFu, inc, d); if ((int)lane >= d) inc += o; }
+    const u32 b = pos + inc - units, en = pos + inc;      // stream range of this run
+    const u32 c0 = b > lo ? b : lo, c1 = en < hi ? en : hi;
+    const u32 n = c1 > c0 ? c1 - c0 : 0u;
+    const u32 tot = __reduce_add_sync(0xFFFFFFFFu, n);
+    if (tot != 0u) {
+      if (lane == 0u) mbar_expect_tx(&s.bar[0], tot * 16u);
+      __syncwarp();
+      if (n != 0u) bulk_g2s(s.rec + (c0 - lo) * 4u, a.blob + src + (u64)(c0 - b) * 4u, n * 16u, &s.bar[0]);
     }
+    pos += __shfl_sync(0xFFFFFFFFu, inc, 31);
   }
+  if (lane == 0u) { s.misc[2] = pos; mbar_arrive(&s.bar[0]); }
+  return pos;
 }
 
 template <int MODE>
@@ -600,47 +631,93 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
   const u32 n_tiles = nb * nsl;
   const u32 thr = PRM(thr_peak), eps = PRM(noise_eps);
   const u32 tile_words = TPC_TT * pitch / 2u;
+  const u32 tid = threadIdx.x;
 
+  if (tid == 0) {
+    mbar_init(&s.bar[0], 1u);                       // full: the producer's arrive (+ tx bytes)
+    mbar_init(&s.bar[1], TPC_K6_CONSUMERS / 32u);   // empty: one arrive per consumer warp
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  if (tid >= TPC_K6_CONSUMERS) {
+    // ---- producer warp -----------------------------------------------------------------------
+    u32 ph = 1u;   // a fresh barrier passes a wait on parity 1: the buffer starts out free
+    for (u32 tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+      const u32 b = tile / nsl, sl = tile - b * nsl;
+      const u32 bs0 = a.batch_start[b];
+      const u32 nbatch = a.batch_start[b + 1] - bs0;
+      const u64 ib = (u64)nsl * bs0 + (u64)sl * nbatch;
+      u32 round = 0u, total;
+      do {
+        mbar_wait(&s.bar[1], ph); ph ^= 1u;
+        total = k6_stage(s, a, ib, nbatch, round);
+        ++round;
+      } while (round * TPC_K6_CAPU < total);
+    }
+    return;
+  }
+
+  // ---- consumers -------------------------------------------------------------------------------
+  u32 ph = 0u;
   for (u32 tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
     const u32 b = tile / nsl, sl = tile - b * nsl;
-    const u32 bs0 = a.batch_start[b];
-    const u32 nbatch = a.batch_start[b + 1] - bs0;
-    const u64 ib = (u64)nsl * bs0 + (u64)sl * nbatch;
-    __syncthreads();   // previous tile fully done with shared memory
-    u32 total0 = 0u;
-    if (nbatch != 0u) total0 = k6_load_group(s, a.idx, ib, 0u, nbatch < TPC_K6_GROUP ? nbatch : TPC_K6_GROUP);
-    if (nbatch == 0u || (nbatch <= TPC_K6_GROUP && total0 == 0u)) {   // block-uniform
-      if (MODE == TPC_MODE_DET_COUNT && threadIdx.x == 0) a.tile_cnt[tile] = 0u;
+    mbar_wait(&s.bar[0], ph); ph ^= 1u;
+    const u32 total = s.misc[2];
+    if (total == 0u) {   // block-uniform: nothing in this tile
+      __syncwarp();
+      if (lane_id() == 0u) mbar_arrive(&s.bar[1]);
+      if (MODE == TPC_MODE_DET_COUNT && tid == 0) a.tile_cnt[tile] = 0u;
       continue;
     }
     // ---- O0: zero the map, scatter the tile's records -------------------------------------
+    csync();   // every consumer is done with the previous tile's map
     {
       uint4* z = (uint4*)s.tile32;
-      for (u32 i = threadIdx.x; i < tile_words / 4u; i += TPC_K6_THREADS) z[i] = make_uint4(0u, 0u, 0u, 0u);
-      for (u32 i = threadIdx.x; i < TPC_TT * 8u; i += TPC_K6_THREADS) s.rowmask[i] = 0u;
-      if (threadIdx.x < 2) s.misc[threadIdx.x] = 0u;
+      for (u32 i = tid; i < tile_words / 4u; i += TPC_K6_CONSUMERS) z[i] = make_uint4(0u, 0u, 0u, 0u);
+      for (u32 i = tid; i < TPC_TT * 8u; i += TPC_K6_CONSUMERS) s.rowmask[i] = 0u;
+      if (tid < 2) s.misc[tid] = 0u;
     }
-    __syncthreads();
-    k6_phase(s, a, ib, nbatch, total0, [&](u32 r) {
-      u32 cell = ((r >> 8) & 0xFFu) * pitch + (r & 0xFFu) + TPC_HALO;
-      s.tile[cell] = (u16)((r >> 16) & 0x3FFu);
-    });
-    if (MODE != TPC_MODE_FAST) {
-      // Q5, deterministic: two digits on one cell -> the maximum, whatever the order.  Re-check
-      // until stable; with duplicate-free input this is one read per record and one barrier.
-      for (;;) {
-        __syncthreads();
-        u32 any = 0u;
-        k6_phase(s, a, ib, nbatch, total0, [&](u32 r) {
-          u32 cell = ((r >> 8) & 0xFFu) * pitch + (r & 0xFFu) + TPC_HALO;
-          u16 q = (u16)((r >> 16) & 0x3FFu);
-          if (s.tile[cell] < q) { s.tile[cell] = q; any = 1u; }
-        });
-        if (!__syncthreads_or((int)any)) break;
+    csync();
+    for (u32 round = 0u;;) {
+      u32 nu = total - round * TPC_K6_CAPU;
+      if (nu > TPC_K6_CAPU) nu = TPC_K6_CAPU;
+      const uint4* r4 = (const uint4*)s.rec;
+      for (u32 u = tid; u < nu; u += TPC_K6_CONSUMERS) {
+        const uint4 v = r4[u];
+        const u32 rr[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+          if (rr[k] != 0u)   // 0 = run padding (every real record has q >= 1)
+            s.tile[((rr[k] >> 8) & 0xFFu) * pitch + (rr[k] & 0xFFu) + TPC_HALO] = (u16)((rr[k] >> 16) & 0x3FFu);
       }
-    } else {
-      __syncthreads();
+      if (MODE != TPC_MODE_FAST) {
+        // Q5, deterministic: two digits on one cell -> the maximum, whatever the order.  Re-check
+        // until stable; with duplicate-free input this is one read per record and one barrier.
+        for (;;) {
+          csync();
+          u32 any = 0u;
+          for (u32 u = tid; u < nu; u += TPC_K6_CONSUMERS) {
+            const uint4 v = r4[u];
+            const u32 rr[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+              if (rr[k] != 0u) {
+                const u32 cell = ((rr[k] >> 8) & 0xFFu) * pitch + (rr[k] & 0xFFu) + TPC_HALO;
+                const u16 q = (u16)((rr[k] >> 16) & 0x3FFu);
+                if (s.tile[cell] < q) { s.tile[cell] = q; any = 1u; }
+              }
+          }
+          if (!csync_or(any)) break;
+        }
+      }
+      __syncwarp();
+      if (lane_id() == 0u) mbar_arrive(&s.bar[1]);   // this warp is done with the staged records
+      ++round;
+      if (round * TPC_K6_CAPU >= total) break;
+      mbar_wait(&s.bar[0], ph); ph ^= 1u;
     }
+    csync();
 
     const u32 tc = b % PRM(n_tc), sr = b / PRM(n_tc);
     const u32 row = sr % PRM(n_rows), sector = sr / PRM(n_rows);
@@ -649,7 +726,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
 
     if (MODE == TPC_MODE_DUMP_MAP) {
       const u64 sector_cells = a.row_off[PRM(n_rows)];
-      for (u32 i = threadIdx.x; i < TPC_TS * npads; i += TPC_K6_THREADS) {
+      for (u32 i = tid; i < TPC_TS * npads; i += TPC_K6_CONSUMERS) {
         u32 tl = i / npads + TPC_HALO, p = i % npads;
         int t = t_base + (int)tl;
         if (t < (int)PRM(n_time))
@@ -658,33 +735,66 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       continue;
     }
 
-    // ---- O1: 3x3 peaks; strict > against the 4 neighbours earlier in (t,p) order, >= later --
-    k6_phase(s, a, ib, nbatch, total0, [&](u32 r) {
-      u32 tl = (r >> 8) & 0xFFu, pad = r & 0xFFu, q = (r >> 16) & 0x3FFu;
-      if (q < thr || tl < 1u || tl > TPC_TT - 2u) return;
-      u32 cell = tl * pitch + pad + TPC_HALO;
-      const u16* c = s.tile + cell;
-      if ((c[0] & 0x3FFu) != q) return;   // a smaller duplicate of this cell
-      bool pk = q > (c[-(int)pitch - 1] & 0x3FFu) && q > (c[-(int)pitch] & 0x3FFu) && q > (c[-(int)pitch + 1] & 0x3FFu) &&
-                q > (c[-1] & 0x3FFu) && q >= (c[1] & 0x3FFu) &&
-                q >= (c[pitch - 1] & 0x3FFu) && q >= (c[pitch] & 0x3FFu) && q >= (c[pitch + 1] & 0x3FFu);
-      if (!pk) return;
-      u32 bit = 0x8000u << ((cell & 1u) * 16u);
-      u32 old = atomicOr(&s.tile32[cell >> 1], bit);
-      if (!(old & bit) && tl >= TPC_HALO && tl < TPC_TS + TPC_HALO) {
-        u32 i = atomicAdd(&s.misc[0], 1u);
-        s.peaks[i] = (u16)((tl << 8) | pad);
+    // ---- O1: 3x3 peaks, dense scan on packed u16x2 words ----------------------------------
+    // A thread owns one word column (2 pads) of a strip of rows and walks down the time axis with
+    // a rolling window.  For the word C of row r: L / R = the same two cells shifted one pad left /
+    // right, H(r) = max(L, C, R).  A cell is a peak iff q > the 4 neighbours earlier in (t,p) order
+    // and q >= the 4 later ones (O1), i.e. q >= max(max(H(r-1), L(r)) + 1, H(r+1), R(r)); an empty
+    // cell never passes (the bound is >= 1).  Rows 1..TT-2 are tested: owned rows plus the halo
+    // rows whose peak flags O2 needs.
+    {
+      const u32 nW = pitch >> 1;
+      const u32 nc = (npads + 2u) >> 1;                 // word columns 1..nc hold cells 3..npads+2
+      const u32 strips = TPC_K6_CONSUMERS / nc;         // >= 1: npads <= 256
+      const u32 rp = (TPC_TT - 2u + strips - 1u) / strips;
+      const u32 si = tid / nc, col = tid - si * nc + 1u;
+      if (si < strips) {
+        const u32 r0 = 1u + si * rp;
+        u32 r1 = r0 + rp;
+        if (r1 > TPC_TT - 1u) r1 = TPC_TT - 1u;
+        const u32* p = s.tile32 + (r0 - 1u) * nW + col;
+        u32 A = p[-1], C0 = p[0], B = p[1];
+        u32 H0 = vmax2(vmax2(__funnelshift_l(A, C0, 16), C0), __funnelshift_l(C0, B, 16));
+        p += nW;
+        A = p[-1]; u32 C1 = p[0]; B = p[1];
+        u32 L1 = __funnelshift_l(A, C1, 16), R1 = __funnelshift_l(C1, B, 16);
+        u32 H1 = vmax2(vmax2(L1, C1), R1);
+        for (u32 r = r0; r < r1; ++r) {
+          p += nW;
+          A = p[-1]; const u32 C2 = p[0]; B = p[1];
+          const u32 L2 = __funnelshift_l(A, C2, 16), R2 = __funnelshift_l(C2, B, 16);
+          const u32 H2 = vmax2(vmax2(L2, C2), R2);
+          const u32 M = vmax2(vmax2(vmax2(H0, L1) + 0x00010001u, H2), R1);
+          const u32 X = vmax2(C1, M) ^ C1;              // a zero half = that cell beats its 8 neighbours
+          if ((X & 0xFFFFu) == 0u || (X >> 16) == 0u) {
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+              const u32 q = (C1 >> (16 * h)) & 0xFFFFu;
+              if (((X >> (16 * h)) & 0xFFFFu) == 0u && q >= thr) {
+                const u32 i = atomicAdd(&s.misc[0], 1u);
+                s.peaks[i] = (u16)((r << 8) | (2u * col + (u32)h - TPC_HALO));
+              }
+            }
+          }
+          H0 = H1; H1 = H2; L1 = L2; C1 = C2; R1 = R2;
+        }
       }
-    });
-    __syncthreads();
+    }
+    csync();
     const u32 npk = s.misc[0];
+    for (u32 i = tid; i < npk; i += TPC_K6_CONSUMERS) {   // bit 15 of a cell = peak flag (distinct cells: plain stores)
+      const u32 e = s.peaks[i];
+      s.tile[(e >> 8) * pitch + (e & 0xFFu) + TPC_HALO] |= (u16)0x8000u;
+    }
+    csync();
 
-    // ---- O2: suppression against the un-updated peak set -----------------------------------
-    for (u32 i = threadIdx.x; i < npk; i += TPC_K6_THREADS) {
-      u32 e = s.peaks[i];
-      u32 tl = e >> 8, pad = e & 0xFFu;
+    // ---- O2: suppression of the owned peaks against the un-updated peak set -----------------
+    for (u32 i = tid; i < npk; i += TPC_K6_CONSUMERS) {
+      const u32 e = s.peaks[i];
+      const u32 tl = e >> 8, pad = e & 0xFFu;
+      if (tl < TPC_HALO || tl >= TPC_TS + TPC_HALO) continue;   // a halo row: its own tile emits it
       const u16* c = s.tile + tl * pitch + pad + TPC_HALO;
-      u32 qc = c[0] & 0x3FFu;
+      const u32 qc = c[0] & 0x3FFu;
       u32 nq[3][3];
 #pragma unroll
       for (int dt = -1; dt <= 1; ++dt)
@@ -696,10 +806,10 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
 #pragma unroll
         for (int dp = -2; dp <= 2; ++dp) {
           if (dt != -2 && dt != 2 && dp != -2 && dp != 2) continue;
-          u32 v = c[dt * (int)pitch + dp];
+          const u32 v = c[dt * (int)pitch + dp];
           if (!(v & 0x8000u)) continue;
-          u32 q2 = v & 0x3FFu;
-          bool beats = q2 > qc || (q2 == qc && (dt < 0 || (dt == 0 && dp < 0)));   // P:36 total order
+          const u32 q2 = v & 0x3FFu;
+          const bool beats = q2 > qc || (q2 == qc && (dt < 0 || (dt == 0 && dp < 0)));   // P:36 total order
           if (!beats) continue;
 #pragma unroll
           for (int mt = -1; mt <= 1; ++mt)
@@ -712,13 +822,13 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
         }
       if (!dead) atomicOr(&s.rowmask[tl * 8u + (pad >> 5)], 1u << (pad & 31u));
     }
-    __syncthreads();
+    csync();
     // ---- rank rows: rowpre[tl] = survivors in rows < tl --------------------------------------
-    if (threadIdx.x < 32) {
+    if (tid < 32) {
       u32 cnt[5], t = 0u;
 #pragma unroll
       for (int k = 0; k < 5; ++k) {
-        u32 tl = threadIdx.x * 5u + (u32)k;
+        const u32 tl = tid * 5u + (u32)k;
         u32 n = 0u;
         if (tl < TPC_TT) {
 #pragma unroll
@@ -728,11 +838,11 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       }
       u32 inc = t;
 #pragma unroll
-      for (int d = 1; d < 32; d <<= 1) { u32 o = __shfl_up_sync(0xFFFFFFFFu, inc, d); if ((int)threadIdx.x >= d) inc += o; }
+      for (int d = 1; d < 32; d <<= 1) { u32 o = __shfl_up_sync(0xFFFFFFFFu, inc, d); if ((int)tid >= d) inc += o; }
       u32 ex = inc - t;
 #pragma unroll
-      for (int k = 0; k < 5; ++k) { u32 tl = threadIdx.x * 5u + (u32)k; if (tl < TPC_TT) s.rowpre[tl] = ex; ex += cnt[k]; }
-      if (threadIdx.x == 31) {
+      for (int k = 0; k < 5; ++k) { const u32 tl = tid * 5u + (u32)k; if (tl < TPC_TT) s.rowpre[tl] = ex; ex += cnt[k]; }
+      if (tid == 31) {
         s.misc[1] = inc;
         if (MODE == TPC_MODE_DET_COUNT) a.tile_cnt[tile] = inc;
         if (MODE == TPC_MODE_FAST) s.base[0] = atomicAdd(a.n_clusters, (u64)inc);
@@ -740,16 +850,16 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       }
     }
     if (MODE == TPC_MODE_DET_COUNT) continue;
-    __syncthreads();
+    csync();
     const u64 base = s.base[0];
 
     // ---- O3 + O4 + O5: 5x5 sums, float32 finalisation (every op rounded once, no FMA), emit --
-    for (u32 i = threadIdx.x; i < npk; i += TPC_K6_THREADS) {
-      u32 e = s.peaks[i];
-      u32 tl = e >> 8, pad = e & 0xFFu;
-      u32 w = pad >> 5, bitpos = pad & 31u;
-      u32 mword = s.rowmask[tl * 8u + w];
-      if (!((mword >> bitpos) & 1u)) continue;
+    for (u32 i = tid; i < npk; i += TPC_K6_CONSUMERS) {
+      const u32 e = s.peaks[i];
+      const u32 tl = e >> 8, pad = e & 0xFFu;
+      const u32 w = pad >> 5, bitpos = pad & 31u;
+      const u32 mword = s.rowmask[tl * 8u + w];
+      if (!((mword >> bitpos) & 1u)) continue;   // suppressed, or a halo-row peak (never marked)
       u32 rank = s.rowpre[tl] + __popc(mword & ((1u << bitpos) - 1u));
       for (u32 k = 0; k < w; ++k) rank += __popc(s.rowmask[tl * 8u + k]);
       const u16* c = s.tile + tl * pitch + pad + TPC_HALO;
@@ -759,23 +869,23 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       for (int dt = -2; dt <= 2; ++dt)
 #pragma unroll
         for (int dp = -2; dp <= 2; ++dp) {
-          u32 q = c[dt * (int)pitch + dp] & 0x3FFu;
+          const u32 q = c[dt * (int)pitch + dp] & 0x3FFu;
           Q += q; Sp += (int)q * dp; St += (int)q * dt;
           Spp += q * (u32)(dp * dp); Stt += q * (u32)(dt * dt);
         }
-      int Vp = (int)(Q * Spp) - Sp * Sp, Vt = (int)(Q * Stt) - St * St;
-      u32 qc = c[0] & 0x3FFu;
-      int t = t_base + (int)tl;
-      float fQ = __uint2float_rn(Q);
-      float pm = __fadd_rn(__uint2float_rn(pad), __fdiv_rn(__int2float_rn(Sp), fQ));
-      float tm = __fadd_rn(__int2float_rn(t), __fdiv_rn(__int2float_rn(St), fQ));
-      float sp = __fdiv_rn(__fsqrt_rn(__int2float_rn(Vp)), fQ);
-      float st = __fdiv_rn(__fsqrt_rn(__int2float_rn(Vt)), fQ);
+      const int Vp = (int)(Q * Spp) - Sp * Sp, Vt = (int)(Q * Stt) - St * St;
+      const u32 qc = c[0] & 0x3FFu;
+      const int t = t_base + (int)tl;
+      const float fQ = __uint2float_rn(Q);
+      const float pm = __fadd_rn(__uint2float_rn(pad), __fdiv_rn(__int2float_rn(Sp), fQ));
+      const float tm = __fadd_rn(__int2float_rn(t), __fdiv_rn(__int2float_rn(St), fQ));
+      const float sp = __fdiv_rn(__fsqrt_rn(__int2float_rn(Vp)), fQ);
+      const float st = __fdiv_rn(__fsqrt_rn(__int2float_rn(Vt)), fQ);
       u32 fl = 0u;
       if (pad < 2u || pad + 2u >= npads) fl |= 1u;
       if (t < 2 || (u32)t + 2u >= PRM(n_time)) fl |= 2u;
       if (qc == 1023u) fl |= 4u;
-      u64 slot = base + rank;
+      const u64 slot = base + rank;
       if (slot < a.capacity) {
         a.out[slot * 2u] = make_uint4(__float_as_uint(pm), __float_as_uint(tm), __float_as_uint(sp), __float_as_uint(st));
         a.out[slot * 2u + 1u] = make_uint4(Q, qc | ((u32)t << 16), pad | (row << 8) | (sector << 16) | (fl << 24), 0u);
@@ -786,19 +896,19 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
   }
 }
 
-extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, 4) k_cluster_tiles_fast(K6Args a) {
+extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, 3) k_cluster_tiles_fast(K6Args a) {
   extern __shared__ __align__(16) u32 smem_u32[];
   k6_body<TPC_MODE_FAST>(a, smem_u32);
 }
-extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, 4) k_cluster_tiles_det_count(K6Args a) {
+extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, 3) k_cluster_tiles_det_count(K6Args a) {
   extern __shared__ __align__(16) u32 smem_u32[];
   k6_body<TPC_MODE_DET_COUNT>(a, smem_u32);
 }
-extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, 4) k_cluster_tiles_det_emit(K6Args a) {
+extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, 3) k_cluster_tiles_det_emit(K6Args a) {
   extern __shared__ __align__(16) u32 smem_u32[];
   k6_body<TPC_MODE_DET_EMIT>(a, smem_u32);
 }
-extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, 4) k_cluster_tiles_dump_map(K6Args a) {
+extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, 3) k_cluster_tiles_dump_map(K6Args a) {
   extern __shared__ __align__(16) u32 smem_u32[];
   k6_body<TPC_MODE_DUMP_MAP>(a, smem_u32);
 }
