@@ -175,7 +175,7 @@ __device__ __forceinline__ void k1_insert(const K1Smem& s, const u32 (&bin)[K], 
 extern "C" __global__ void __launch_bounds__(TPC_K1_THREADS, 1)
 k_partition_coarse(const uint2* __restrict__ digits, u64 n, u64 per_cta, uint4* __restrict__ pool,
                    u32* __restrict__ dir, u32* __restrict__ used, u32 slice_cap, u32* __restrict__ status) {
-  extern __shared__ __align__(16) u32 smem_u32[];
+  extern __shared__ __align__(128) u32 smem_u32[];
   const u32 nb = PRM(n_bins);
   const K1Smem s = k1_smem(smem_u32, nb);
   for (u32 i = threadIdx.x; i < nb; i += TPC_K1_THREADS) s.pos[i] = 8u;
@@ -394,7 +394,7 @@ extern "C" __global__ void __launch_bounds__(TPC_K5_THREADS, 2)
 k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, const u32* __restrict__ chunk_list,
                  const u32* __restrict__ bin_chunk_start, const u32* __restrict__ batch_start,
                  u32* __restrict__ blob, u64* __restrict__ blob_cursor, u64* __restrict__ idx) {
-  extern __shared__ __align__(16) u32 smem_u32[];
+  extern __shared__ __align__(128) u32 smem_u32[];
   u32* buf = smem_u32;                       // [TPC_K5_BUF]
   u32* s_cnt = buf + TPC_K5_BUF;             // [128] primaries per slab
   u32* s_dcnt = s_cnt + 128;                 // [128] halo copies per slab
@@ -555,6 +555,15 @@ __device__ __forceinline__ void mbar_wait(u64* bar, u32 parity) {
                  : "=r"(ok) : "r"(smem_addr(bar)), "r"(parity) : "memory");
   } while (!ok);
 }
+__device__ __forceinline__ void mbar_wait_backoff(u64* bar, u32 parity) {   // the producer's wait: do not steal issue slots
+  u32 ok;
+  for (;;) {
+    asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+                 : "=r"(ok) : "r"(smem_addr(bar)), "r"(parity) : "memory");
+    if (ok) break;
+    asm volatile("nanosleep.u32 200;" ::: "memory");
+  }
+}
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, u32 bytes, u64* bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                ::"r"(smem_addr(dst)), "l"(src), "r"(bytes), "r"(smem_addr(bar)) : "memory");
@@ -582,7 +591,6 @@ __host__ __device__ inline u32 tpc_k6_smem_bytes(u32 pitch, u32 max_peaks) {
 }
 __device__ __forceinline__ K6Smem k6_smem(u32* p) {
   K6Smem s;
-  p = (u32*)(((u64)p + 127ull) & ~127ull);   // bulk copies need 16-byte aligned destinations
   s.rec = p; p += TPC_K6_CAP;
   s.tile32 = p; s.tile = (u16*)p; p += TPC_TT * PRM(pitch) / 2u;
   s.bar = (u64*)p; p += 4;
@@ -650,7 +658,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       const u64 ib = (u64)nsl * bs0 + (u64)sl * nbatch;
       u32 round = 0u, total;
       do {
-        mbar_wait(&s.bar[1], ph); ph ^= 1u;
+        mbar_wait_backoff(&s.bar[1], ph); ph ^= 1u;
         total = k6_stage(s, a, ib, nbatch, round);
         ++round;
       } while (round * TPC_K6_CAPU < total);
@@ -740,7 +748,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
     // a rolling window.  For the word C of row r: L / R = the same two cells shifted one pad left /
     // right, H(r) = max(L, C, R).  A cell is a peak iff q > the 4 neighbours earlier in (t,p) order
     // and q >= the 4 later ones (O1), i.e. q >= max(max(H(r-1), L(r)) + 1, H(r+1), R(r)); an empty
-    // cell never passes (the bound is >= 1).  Rows 1..TT-2 are tested: owned rows plus the halo
+    // cell never passes (the bound is >= 1); thr_peak joins the same max.  Rows 1..TT-2 are tested: owned rows plus the halo
     // rows whose peak flags O2 needs.
     {
       const u32 nW = pitch >> 1;
@@ -748,6 +756,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       const u32 strips = TPC_K6_CONSUMERS / nc;         // >= 1: npads <= 256
       const u32 rp = (TPC_TT - 2u + strips - 1u) / strips;
       const u32 si = tid / nc, col = tid - si * nc + 1u;
+      const u32 thr2 = thr | (thr << 16);               // q >= thr_peak folded into the same bound
       if (si < strips) {
         const u32 r0 = 1u + si * rp;
         u32 r1 = r0 + rp;
@@ -764,13 +773,12 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
           A = p[-1]; const u32 C2 = p[0]; B = p[1];
           const u32 L2 = __funnelshift_l(A, C2, 16), R2 = __funnelshift_l(C2, B, 16);
           const u32 H2 = vmax2(vmax2(L2, C2), R2);
-          const u32 M = vmax2(vmax2(vmax2(H0, L1) + 0x00010001u, H2), R1);
+          const u32 M = vmax2(vmax2(vmax2(H0, L1) + 0x00010001u, H2), vmax2(R1, thr2));
           const u32 X = vmax2(C1, M) ^ C1;              // a zero half = that cell beats its 8 neighbours
           if ((X & 0xFFFFu) == 0u || (X >> 16) == 0u) {
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
-              const u32 q = (C1 >> (16 * h)) & 0xFFFFu;
-              if (((X >> (16 * h)) & 0xFFFFu) == 0u && q >= thr) {
+              if (((X >> (16 * h)) & 0xFFFFu) == 0u) {
                 const u32 i = atomicAdd(&s.misc[0], 1u);
                 s.peaks[i] = (u16)((r << 8) | (2u * col + (u32)h - TPC_HALO));
               }
@@ -897,18 +905,18 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
 }
 
 extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, 3) k_cluster_tiles_fast(K6Args a) {
-  extern __shared__ __align__(16) u32 smem_u32[];
+  extern __shared__ __align__(128) u32 smem_u32[];
   k6_body<TPC_MODE_FAST>(a, smem_u32);
 }
 extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, 3) k_cluster_tiles_det_count(K6Args a) {
-  extern __shared__ __align__(16) u32 smem_u32[];
+  extern __shared__ __align__(128) u32 smem_u32[];
   k6_body<TPC_MODE_DET_COUNT>(a, smem_u32);
 }
 extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, 3) k_cluster_tiles_det_emit(K6Args a) {
-  extern __shared__ __align__(16) u32 smem_u32[];
+  extern __shared__ __align__(128) u32 smem_u32[];
   k6_body<TPC_MODE_DET_EMIT>(a, smem_u32);
 }
 extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, 3) k_cluster_tiles_dump_map(K6Args a) {
-  extern __shared__ __align__(16) u32 smem_u32[];
+  extern __shared__ __align__(128) u32 smem_u32[];
   k6_body<TPC_MODE_DUMP_MAP>(a, smem_u32);
 }
