@@ -135,7 +135,7 @@ TPCCLUS_API int tpcclus_create(const tpcclus_params* params, tpcclus_handle** ou
 
 /* Clusterizes one time frame: enqueues every step of the path (NS (1)..(5)) on
  * `cuda_stream` (a cudaStream_t; NULL = legacy default stream) and returns without
- * synchronising.  d_digits: DEVICE, 8-byte aligned, n <= max_digits records, any order,
+ * synchronising.  d_digits: DEVICE, 16-byte aligned, n <= max_digits records, any order,
  * not modified.  out: HOST struct of DEVICE pointers.  The result depends only on
  * (params, digit multiset, mode), never on earlier runs (Q17).  One run at a time per
  * handle (the workspace is per handle).  The caller synchronises the stream before

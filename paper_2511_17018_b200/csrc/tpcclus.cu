@@ -23,7 +23,7 @@ extern "C" const char tpcclus_kernel_source[];   // generated from tpcclus_kerne
 
 namespace {
 
-constexpr uint32_t kMaxBins = 5632;   // K1 shared memory: 5632 * 38 B + 528 B <= 227 KB
+constexpr uint32_t kMaxSmem = 232448;  // 227 KB: K1 needs 40 B per coarse bin + 12.8 KB (5472 bins at the full geometry)
 constexpr int kMaxKernels = 12;
 
 thread_local std::string g_create_error;
@@ -78,7 +78,7 @@ int make_geometry(const tpcclus_params* p, Geometry* g) {
   }
   q.n_tc = (p->n_time + TPC_TC - 1) / TPC_TC;
   uint64_t nb = (uint64_t)p->n_sectors * p->n_rows * q.n_tc;
-  if (nb > kMaxBins) return TPCCLUS_ERR_UNSUPPORTED_GEOMETRY;
+  if (nb > 65535 || tpc_k1_smem_bytes((uint32_t)nb) > kMaxSmem) return TPCCLUS_ERR_UNSUPPORTED_GEOMETRY;
   q.n_bins = (uint32_t)nb;
   uint32_t tmin = p->n_time < TPC_TC ? p->n_time : TPC_TC;
   q.n_sl = (tmin + TPC_TS - 1) / TPC_TS;
@@ -469,7 +469,7 @@ int tpcclus_run(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n, co
   if (!h) return TPCCLUS_ERR_INVALID_ARG;
   h->err.clear();
   if (!out || !out->n_clusters || (!out->clusters && out->capacity) || (!d_digits && n) || n > h->g.max_digits ||
-      (mode != TPCCLUS_MODE_FAST && mode != TPCCLUS_MODE_DETERMINISTIC) || ((uintptr_t)d_digits & 7u) ||
+      (mode != TPCCLUS_MODE_FAST && mode != TPCCLUS_MODE_DETERMINISTIC) || ((uintptr_t)d_digits & 15u) ||
       ((uintptr_t)out->clusters & 15u) || ((uintptr_t)out->n_clusters & 7u))
     return fail(h, TPCCLUS_ERR_INVALID_ARG, "tpcclus_run: bad argument");
   cudaStream_t st = (cudaStream_t)cuda_stream;

@@ -62,9 +62,6 @@ __constant__ TpcParams c_prm;
 #endif
 
 // ---- shared-memory sizes (bytes); the host launches with exactly these --------------------
-__host__ __device__ inline u32 tpc_k1_smem_bytes(u32 nb) {
-  return (nb * TPC_STAGE + nb + ((nb + 1u) >> 1) + 4u) * 4u + 512u;
-}
 
 // ---- small PTX helpers -------------------------------------------------------------------
 __device__ __forceinline__ uint2 ld_stream_u2(const uint2* p) {   // read-once input: keep out of L1
@@ -97,79 +94,144 @@ __device__ __forceinline__ u32 lane_id() { return threadIdx.x & 31u; }
 // is private to (CTA, bin), so there is no global atomic and no histogram pre-pass.
 // The chunk directory dir[] (bin<<8 | records) is turned into per-bin lists by K2..K4.
 //
+// A round = 4096 digits, two block barriers:
+//   insert : slot = atomicAdd(cnt[bin]); slot < 8 -> the record goes into the stage; the
+//            writer of slot 7 queues the bin for flushing; slot >= 8 (the stage is full until
+//            the flush) -> the record is parked in a small spill list, its slot stays reserved
+//            and it is written at the head of the next round (slot - 8).
+//   flush  : the queue is worked off densely, two lanes per 32-byte stage, cnt[bin] -= 8.
+// Any skew is legal: when the spill list or the flush queue is full a thread keeps its
+// record in registers and the round repeats (flush, slot -= 8) until everything is placed.
+//
 // record (4 B):  pad[0:8) | u[8:22) | q[22:32)   with u = time - tc*TPC_TC + 3  (14 bit)
 // ==========================================================================================
-struct K1Smem {   // layout computed identically on the host (tpcclus.cu)
+#define TPC_K1_FQ 2048u      // flush-queue entries (u16 bin ids)
+#define TPC_K1_SPILL 512u    // spill entries per buffer (2 x u32)
+
+struct K1Smem {   // layout computed identically on the host (tpc_k1_smem_bytes)
   u32* stage;     // [NB][8]
+  u32* cnt;       // [NB]  records reserved in the stage (may exceed 8 until the flush)
   u32* pos;       // [NB]  (chunk_local << 4) | sectors_filled(0..8)
-  u32* cnt;       // [(NB+1)/2] two 16-bit counters per word
-  u32* misc;      // [0] next chunk, [1] bad flag
+  u32* spill;     // [2][TPC_K1_SPILL][2]  {rec, bin | slot << 16}
+  u32* misc;      // [0] next chunk  [1] flush-queue length  [2],[3] spill lengths
+  u16* fq;        // [TPC_K1_FQ]
   u16* npads;     // [256]
 };
+__host__ __device__ inline u32 tpc_k1_smem_bytes(u32 nb) {
+  return (nb * (TPC_STAGE + 2u) + 4u * TPC_K1_SPILL + 8u) * 4u + TPC_K1_FQ * 2u + 512u;
+}
 __device__ __forceinline__ K1Smem k1_smem(u32* base, u32 nb) {
   K1Smem s;
   s.stage = base;
-  s.pos = s.stage + (u64)nb * TPC_STAGE;
-  s.cnt = s.pos + nb;
-  s.misc = s.cnt + ((nb + 1u) >> 1);
-  s.npads = (u16*)(s.misc + 4);
+  s.cnt = s.stage + nb * TPC_STAGE;
+  s.pos = s.cnt + nb;
+  s.spill = s.pos + nb;
+  s.misc = s.spill + 4u * TPC_K1_SPILL;
+  s.fq = (u16*)(s.misc + 8);
+  s.npads = s.fq + TPC_K1_FQ;
   return s;
 }
 
-__device__ __forceinline__ void k1_flush(const K1Smem& s, u32 bin, u32 slice_base, u32 slice_cap,
-                                         uint4* pool, u32* dir) {
-  u32 p = s.pos[bin];
+// Moves the full stage of `bin` into the pool: lane pair (even, odd) = the two 16-byte halves.
+// Called with all 32 lanes; `act` marks the pairs that carry a bin.
+__device__ __forceinline__ void k1_flush_pair(const K1Smem& s, bool act, u32 bin, u32 slice_base, u32 slice_cap,
+                                              uint4* pool, u32* dir) {
+  const u32 half = threadIdx.x & 1u;
+  u32 sector = 0xFFFFFFFFu;   // index of the 32-byte sector inside this CTA's slice
+  if (act && half == 0u) {
+    const u32 p = s.pos[bin];
+    u32 fill = p & 15u, c = p >> 4;
+    if (fill == 8u) {
+      c = atomicAdd(&s.misc[0], 1u);
+      fill = 0u;
+      if (c < slice_cap) dir[slice_base + c] = (bin << 8) | TPC_CHUNK;
+    }
+    s.pos[bin] = (c << 4) | (fill + 1u);
+    s.cnt[bin] -= 8u;   // one flush per bin and phase: no other thread touches cnt[bin] here
+    if (c < slice_cap) sector = c * 8u + fill;
+  }
+  sector = __shfl_sync(0xFFFFFFFFu, sector, (int)(lane_id() & ~1u));
+  if (act && sector != 0xFFFFFFFFu) {
+    const uint4 v = ((const uint4*)s.stage)[bin * 2u + half];
+    pool[((u64)slice_base * 8u + sector) * 2u + half] = v;
+  }
+}
+__device__ __forceinline__ void k1_flush_single(const K1Smem& s, u32 bin, u32 slice_base, u32 slice_cap, uint4* pool, u32* dir) {
+  const u32 p = s.pos[bin];
   u32 fill = p & 15u, c = p >> 4;
   if (fill == 8u) {
     c = atomicAdd(&s.misc[0], 1u);
     fill = 0u;
     if (c < slice_cap) dir[slice_base + c] = (bin << 8) | TPC_CHUNK;
   }
-  const uint4* st = (const uint4*)(s.stage + (u64)bin * TPC_STAGE);
-  uint4 a = st[0], b = st[1];
-  if (c < slice_cap) st_256(pool + ((u64)(slice_base + c) * 16u + fill * 2u), a, b);
   s.pos[bin] = (c << 4) | (fill + 1u);
-  atomicSub(&s.cnt[bin >> 1], 8u << ((bin & 1u) * 16u));
+  s.cnt[bin] -= 8u;
+  const uint4* st = (const uint4*)(s.stage + bin * TPC_STAGE);
+  if (c < slice_cap) st_256(pool + ((u64)(slice_base + c) * 16u + fill * 2u), st[0], st[1]);
 }
 
-// Inserts up to K records per thread into the stages; block-synchronous.  bin == 0xFFFFFFFF
-// means "no record".  Handles any skew: a round in which one bin receives more than 8
-// records loops, flushing 8 at a time.
+// Queues `bin` for the flush phase; when the queue is full the caller flushes it itself (bit in lf).
+__device__ __forceinline__ bool k1_queue_flush(const K1Smem& s, u32 par, u32 bin) {
+  const u32 j = atomicAdd(&s.misc[4u + par], 1u);
+  if (j < TPC_K1_FQ) { s.fq[j] = (u16)bin; return true; }
+  return false;
+}
+
+// One pass = insert phase + flush phase (two block barriers).  Entries k with bit k of `pend`
+// set are still to be placed; bit k of `have` = entry k holds a reserved slot already.
+// Returns (block-uniform) whether any thread still has a pending entry.
 template <int K>
-__device__ __forceinline__ void k1_insert(const K1Smem& s, const u32 (&bin)[K], const u32 (&rec)[K],
-                                          u32 slice_base, u32 slice_cap, uint4* pool, u32* dir) {
-  u32 slot[K];
-  u32 pending = 0u, flush = 0u;
+__device__ __forceinline__ bool k1_pass(const K1Smem& s, u32& cur, u32& par, const u32 (&bin)[K], const u32 (&rec)[K],
+                                        u32 (&slot)[K], u32& pend, u32& have, u32 slice_base, u32 slice_cap,
+                                        uint4* pool, u32* dir) {
+  u32 lf = 0u, drain_bin = 0u;
+  u32* sp_in = s.spill + cur * 2u * TPC_K1_SPILL;
+  u32* sp_out = s.spill + (cur ^ 1u) * 2u * TPC_K1_SPILL;
+  u32 nsp = s.misc[2u + cur];
+  if (nsp > TPC_K1_SPILL) nsp = TPC_K1_SPILL;
+  if (threadIdx.x < nsp) {   // records parked in the previous pass: their bin was flushed since, slot - 8 < 8
+    const u32 r = sp_in[2u * threadIdx.x], w = sp_in[2u * threadIdx.x + 1u];
+    const u32 b = w & 0xFFFFu, sl = (w >> 16) - 8u;
+    s.stage[b * TPC_STAGE + sl] = r;
+    if (sl == TPC_STAGE - 1u && !k1_queue_flush(s, par, b)) { lf |= 1u << K; drain_bin = b; }
+  }
 #pragma unroll
   for (int k = 0; k < K; ++k) {
-    if (bin[k] != 0xFFFFFFFFu) {
-      u32 sh = (bin[k] & 1u) * 16u;
-      slot[k] = (atomicAdd(&s.cnt[bin[k] >> 1], 1u << sh) >> sh) & 0xFFFFu;
-      pending |= 1u << k;
-    } else {
-      slot[k] = 0u;
-    }
-  }
-  for (;;) {
-#pragma unroll
-    for (int k = 0; k < K; ++k) {
-      if (pending & (1u << k)) {
-        if (slot[k] < TPC_STAGE) {
-          s.stage[(u64)bin[k] * TPC_STAGE + slot[k]] = rec[k];
-          pending &= ~(1u << k);
-          if (slot[k] == TPC_STAGE - 1u) flush |= 1u << k;
-        } else {
-          slot[k] -= TPC_STAGE;
+    if (pend & (1u << k)) {
+      if (have & (1u << k)) slot[k] -= 8u;
+      else { slot[k] = atomicAdd(&s.cnt[bin[k]], 1u); have |= 1u << k; }
+      if (slot[k] < TPC_STAGE) {
+        s.stage[bin[k] * TPC_STAGE + slot[k]] = rec[k];
+        pend &= ~(1u << k);
+        if (slot[k] == TPC_STAGE - 1u && !k1_queue_flush(s, par, bin[k])) lf |= 1u << k;
+      } else if (slot[k] < 2u * TPC_STAGE) {
+        const u32 j = atomicAdd(&s.misc[2u + (cur ^ 1u)], 1u);
+        if (j < TPC_K1_SPILL) {
+          sp_out[2u * j] = rec[k];
+          sp_out[2u * j + 1u] = bin[k] | (slot[k] << 16);
+          pend &= ~(1u << k);
         }
       }
     }
-    __syncthreads();
+  }
+  __syncthreads();
+  // ---- flush phase ---------------------------------------------------------------------------
+  u32 nf = s.misc[4u + par];
+  if (nf > TPC_K1_FQ) nf = TPC_K1_FQ;
+  const u32 lim = (2u * nf + 31u) & ~31u;
+  for (u32 j = threadIdx.x; j < lim; j += TPC_K1_THREADS) {
+    const bool act = j < 2u * nf;
+    k1_flush_pair(s, act, act ? (u32)s.fq[j >> 1] : 0u, slice_base, slice_cap, pool, dir);
+  }
+  if (lf) {   // the queue was full
 #pragma unroll
     for (int k = 0; k < K; ++k)
-      if (flush & (1u << k)) k1_flush(s, bin[k], slice_base, slice_cap, pool, dir);
-    flush = 0u;
-    if (!__syncthreads_or((int)pending)) break;
+      if (lf & (1u << k)) k1_flush_single(s, bin[k], slice_base, slice_cap, pool, dir);
+    if (lf & (1u << K)) k1_flush_single(s, drain_bin, slice_base, slice_cap, pool, dir);
   }
+  if (threadIdx.x == 0) { s.misc[2u + cur] = 0u; s.misc[4u + (par ^ 1u)] = 0u; }
+  cur ^= 1u; par ^= 1u;
+  return __syncthreads_or((int)pend) != 0;
 }
 
 extern "C" __global__ void __launch_bounds__(TPC_K1_THREADS, 1)
@@ -178,79 +240,93 @@ k_partition_coarse(const uint2* __restrict__ digits, u64 n, u64 per_cta, uint4* 
   extern __shared__ __align__(128) u32 smem_u32[];
   const u32 nb = PRM(n_bins);
   const K1Smem s = k1_smem(smem_u32, nb);
-  for (u32 i = threadIdx.x; i < nb; i += TPC_K1_THREADS) s.pos[i] = 8u;
-  for (u32 i = threadIdx.x; i < ((nb + 1u) >> 1); i += TPC_K1_THREADS) s.cnt[i] = 0u;
-  if (threadIdx.x < 4) s.misc[threadIdx.x] = 0u;
+  for (u32 i = threadIdx.x; i < nb; i += TPC_K1_THREADS) { s.pos[i] = 8u; s.cnt[i] = 0u; }
+  if (threadIdx.x < 8) s.misc[threadIdx.x] = 0u;
   if (threadIdx.x < 256) s.npads[threadIdx.x] = threadIdx.x < PRM(n_rows) ? PRM_NPADS(threadIdx.x) : (u16)0;
   __syncthreads();
 
   const u32 slice_base = blockIdx.x * slice_cap;
-  const u64 begin = (u64)blockIdx.x * per_cta;
+  const u64 begin = (u64)blockIdx.x * per_cta;   // a multiple of the round: 16-byte aligned loads
   u64 end = begin + per_cta;
   if (end > n) end = n;
   const u32 ROUND = TPC_K1_THREADS * TPC_K1_DPT;
   const u32 S = PRM(n_sectors), R = PRM(n_rows), T = PRM(n_time), NTC = PRM(n_tc);
+  u32 cur = 0u, par = 0u;
 
-  uint2 nxt[TPC_K1_DPT];
+  // thread t of a round owns digits 2t, 2t+1 of each half of the round (two 16-byte loads)
+  auto fetch = [&](u64 base, uint4 (&d)[TPC_K1_DPT / 2]) {
 #pragma unroll
-  for (int k = 0; k < TPC_K1_DPT; ++k) {
-    u64 i = begin + (u64)k * TPC_K1_THREADS + threadIdx.x;
-    nxt[k] = (begin < end && i < end) ? ld_stream_u2(digits + i) : make_uint2(0u, 0u);
-  }
+    for (int h = 0; h < TPC_K1_DPT / 2; ++h) {
+      const u64 i = base + (u64)h * (ROUND / (TPC_K1_DPT / 2)) + 2u * threadIdx.x;
+      if (i + 1u < end) d[h] = ld_stream_u4((const uint4*)(digits + i));
+      else if (i < end) { const uint2 v = ld_stream_u2(digits + i); d[h] = make_uint4(v.x, v.y, 0u, 0u); }
+      else d[h] = make_uint4(0u, 0u, 0u, 0u);
+    }
+  };
+  uint4 nxt[TPC_K1_DPT / 2];
+  fetch(begin, nxt);
   bool bad = false;
   for (u64 base = begin; base < end; base += ROUND) {
-    uint2 cur[TPC_K1_DPT];
+    uint4 curd[TPC_K1_DPT / 2];
 #pragma unroll
-    for (int k = 0; k < TPC_K1_DPT; ++k) cur[k] = nxt[k];
-#pragma unroll
-    for (int k = 0; k < TPC_K1_DPT; ++k) {   // prefetch the next round while this one is binned
-      u64 i = base + ROUND + (u64)k * TPC_K1_THREADS + threadIdx.x;
-      nxt[k] = (i < end) ? ld_stream_u2(digits + i) : make_uint2(0u, 0u);
-    }
-    u32 bin[TPC_K1_DPT], rec[TPC_K1_DPT], dbin[TPC_K1_DPT], drec[TPC_K1_DPT];
-    bool anydup = false;
+    for (int h = 0; h < TPC_K1_DPT / 2; ++h) curd[h] = nxt[h];
+    fetch(base + ROUND, nxt);   // prefetch the next round while this one is binned
+    u32 bin[TPC_K1_DPT], rec[TPC_K1_DPT], slot[TPC_K1_DPT], dbin[TPC_K1_DPT], drec[TPC_K1_DPT];
+    u32 pend = 0u, dpend = 0u;
 #pragma unroll
     for (int k = 0; k < TPC_K1_DPT; ++k) {
-      u64 i = base + (u64)k * TPC_K1_THREADS + threadIdx.x;
-      bin[k] = 0xFFFFFFFFu; rec[k] = 0u; dbin[k] = 0xFFFFFFFFu; drec[k] = 0u;
+      const u64 i = base + (u64)(k >> 1) * (ROUND / (TPC_K1_DPT / 2)) + 2u * threadIdx.x + (u32)(k & 1);
+      const u32 w0 = (k & 1) ? curd[k >> 1].z : curd[k >> 1].x, w1 = (k & 1) ? curd[k >> 1].w : curd[k >> 1].y;
+      bin[k] = 0u; rec[k] = 0u; dbin[k] = 0u; drec[k] = 0u;
       if (i < end) {
-        u32 w0 = cur[k].x, w1 = cur[k].y;
-        u32 q = w0 & 0xFFFFu, t = w0 >> 16, pad = w1 & 0xFFu, row = (w1 >> 8) & 0xFFu, sec = (w1 >> 16) & 0xFFu;
+        u32 q = w0 & 0xFFFFu;
+        const u32 t = w0 >> 16, pad = w1 & 0xFFu, row = (w1 >> 8) & 0xFFu, sec = (w1 >> 16) & 0xFFu;
         if (sec >= S || row >= R || t >= T || pad >= (u32)s.npads[row]) {   // O0 / Q4: ignore + flag
           bad = true;
         } else if (q != 0u) {                                               // Q4: zero charge ignored
           q = q > 1023u ? 1023u : q;                                        // Q4: clamp
-          u32 tc = (NTC > 1u) ? t / TPC_TC : 0u;
-          u32 v = t - tc * TPC_TC;
-          u32 b0 = (sec * R + row) * NTC + tc;
+          const u32 tc = (NTC > 1u) ? t / TPC_TC : 0u;
+          const u32 v = t - tc * TPC_TC;
+          const u32 b0 = (sec * R + row) * NTC + tc;
           bin[k] = b0;
           rec[k] = pad | ((v + TPC_HALO) << 8) | (q << 22);
+          pend |= 1u << k;
           if (NTC > 1u) {   // halo copy into the neighbouring time-chunk's bin
             if (v < TPC_HALO && tc > 0u) {
-              dbin[k] = b0 - 1u; drec[k] = pad | ((v + TPC_TC + TPC_HALO) << 8) | (q << 22); anydup = true;
+              dbin[k] = b0 - 1u; drec[k] = pad | ((v + TPC_TC + TPC_HALO) << 8) | (q << 22); dpend |= 1u << k;
             } else if (v + TPC_HALO >= TPC_TC && tc + 1u < NTC) {
-              dbin[k] = b0 + 1u; drec[k] = pad | ((v + TPC_HALO - TPC_TC) << 8) | (q << 22); anydup = true;
+              dbin[k] = b0 + 1u; drec[k] = pad | ((v + TPC_HALO - TPC_TC) << 8) | (q << 22); dpend |= 1u << k;
             }
           }
         }
       }
     }
-    k1_insert<TPC_K1_DPT>(s, bin, rec, slice_base, slice_cap, pool, dir);
+    u32 have = 0u;
+    while (k1_pass<TPC_K1_DPT>(s, cur, par, bin, rec, slot, pend, have, slice_base, slice_cap, pool, dir)) {}
     if (NTC > 1u) {
-      if (__syncthreads_or((int)anydup)) k1_insert<TPC_K1_DPT>(s, dbin, drec, slice_base, slice_cap, pool, dir);
+      if (__syncthreads_or((int)dpend)) {
+        have = 0u;
+        while (k1_pass<TPC_K1_DPT>(s, cur, par, dbin, drec, slot, dpend, have, slice_base, slice_cap, pool, dir)) {}
+      }
     }
   }
   if (bad) atomicOr(status, TPC_STATUS_BAD_DIGITS);
+  {   // records still parked in the spill list (block-uniform: misc is stable after a pass)
+    u32 bin[1] = {0u}, rec[1] = {0u}, slot[1] = {0u}, pend = 0u, have = 0u;
+    while (s.misc[2u + cur] != 0u) k1_pass<1>(s, cur, par, bin, rec, slot, pend, have, slice_base, slice_cap, pool, dir);
+  }
   __syncthreads();
-  // drain: every bin's partial stage goes to its current (or a fresh) chunk; fix the
-  // record count of that last chunk in the directory.
+  // drain: every bin's partial stage goes to its current (or a fresh) chunk, unused slots zeroed;
+  // fix the record count of that last chunk in the directory.
   for (u32 b = threadIdx.x; b < nb; b += TPC_K1_THREADS) {
-    u32 m = (s.cnt[b >> 1] >> ((b & 1u) * 16u)) & 0xFFFFu;   // 0..7 staged
-    u32 p = s.pos[b];
+    const u32 m = s.cnt[b];   // 0..7 staged
+    const u32 p = s.pos[b];
     u32 fill = p & 15u, c = p >> 4;
     if (m != 0u) {
       if (fill == 8u) { c = atomicAdd(&s.misc[0], 1u); fill = 0u; }
-      const uint4* st = (const uint4*)(s.stage + (u64)b * TPC_STAGE);
+      u32* stw = s.stage + b * TPC_STAGE;
+      for (u32 k = m; k < TPC_STAGE; ++k) stw[k] = 0u;
+      const uint4* st = (const uint4*)stw;
       if (c < slice_cap) {
         st_256(pool + ((u64)(slice_base + c) * 16u + fill * 2u), st[0], st[1]);
         dir[slice_base + c] = (b << 8) | (fill * 8u + m);
@@ -744,47 +820,63 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
     }
 
     // ---- O1: 3x3 peaks, dense scan on packed u16x2 words ----------------------------------
-    // A thread owns one word column (2 pads) of a strip of rows and walks down the time axis with
-    // a rolling window.  For the word C of row r: L / R = the same two cells shifted one pad left /
-    // right, H(r) = max(L, C, R).  A cell is a peak iff q > the 4 neighbours earlier in (t,p) order
-    // and q >= the 4 later ones (O1), i.e. q >= max(max(H(r-1), L(r)) + 1, H(r+1), R(r)); an empty
-    // cell never passes (the bound is >= 1); thr_peak joins the same max.  Rows 1..TT-2 are tested: owned rows plus the halo
-    // rows whose peak flags O2 needs.
+    // A thread owns a group of 4 word columns (8 pads, one 128-bit load per row) of a strip of
+    // rows and walks down the time axis with a rolling 3-row window.  For the word C of row r:
+    // L / R = the same two cells shifted one pad left / right, H(r) = max(L, C, R).  A cell is a
+    // peak iff q > the 4 neighbours earlier in (t,p) order and q >= the 4 later ones (O1), i.e.
+    // q >= max(max(H(r-1), L(r)) + 1, H(r+1), R(r)); an empty cell never passes (the bound is
+    // >= 1) and thr_peak joins the same max.  Rows 1..TT-2 are tested: the owned rows plus the
+    // halo rows whose peak flags O2 needs.  Guard cells are 0 and can never be flagged.
     {
       const u32 nW = pitch >> 1;
-      const u32 nc = (npads + 2u) >> 1;                 // word columns 1..nc hold cells 3..npads+2
-      const u32 strips = TPC_K6_CONSUMERS / nc;         // >= 1: npads <= 256
+      const u32 ng = (((npads + 2u) >> 1) >> 2) + 1u;    // word groups covering cells 0..npads+2
+      const u32 strips = TPC_K6_CONSUMERS / ng;          // >= 1: npads <= 256 -> ng <= 33
       const u32 rp = (TPC_TT - 2u + strips - 1u) / strips;
-      const u32 si = tid / nc, col = tid - si * nc + 1u;
-      const u32 thr2 = thr | (thr << 16);               // q >= thr_peak folded into the same bound
-      if (si < strips) {
-        const u32 r0 = 1u + si * rp;
-        u32 r1 = r0 + rp;
-        if (r1 > TPC_TT - 1u) r1 = TPC_TT - 1u;
-        const u32* p = s.tile32 + (r0 - 1u) * nW + col;
-        u32 A = p[-1], C0 = p[0], B = p[1];
-        u32 H0 = vmax2(vmax2(__funnelshift_l(A, C0, 16), C0), __funnelshift_l(C0, B, 16));
-        p += nW;
-        A = p[-1]; u32 C1 = p[0]; B = p[1];
-        u32 L1 = __funnelshift_l(A, C1, 16), R1 = __funnelshift_l(C1, B, 16);
-        u32 H1 = vmax2(vmax2(L1, C1), R1);
-        for (u32 r = r0; r < r1; ++r) {
-          p += nW;
-          A = p[-1]; const u32 C2 = p[0]; B = p[1];
-          const u32 L2 = __funnelshift_l(A, C2, 16), R2 = __funnelshift_l(C2, B, 16);
-          const u32 H2 = vmax2(vmax2(L2, C2), R2);
-          const u32 M = vmax2(vmax2(vmax2(H0, L1) + 0x00010001u, H2), vmax2(R1, thr2));
-          const u32 X = vmax2(C1, M) ^ C1;              // a zero half = that cell beats its 8 neighbours
-          if ((X & 0xFFFFu) == 0u || (X >> 16) == 0u) {
+      const u32 si = tid / ng, g = tid - si * ng;
+      const u32 thr2 = thr | (thr << 16);
+      const u32 r0 = 1u + si * rp;
+      u32 r1 = r0 + rp;
+      if (r1 > TPC_TT - 1u) r1 = TPC_TT - 1u;
+      if (si < strips && r0 < r1) {
+        const bool hasl = g != 0u, hasr = 4u * g + 4u < nW;
+        struct Row { u32 C[4], S[5], H[4]; };
+        auto load = [&](const u32* q, Row& w) {
+          const uint4 v = *(const uint4*)q;
+          const u32 a = hasl ? q[-1] : 0u, b = hasr ? q[4] : 0u;
+          w.C[0] = v.x; w.C[1] = v.y; w.C[2] = v.z; w.C[3] = v.w;
+          w.S[0] = __funnelshift_l(a, v.x, 16); w.S[1] = __funnelshift_l(v.x, v.y, 16);
+          w.S[2] = __funnelshift_l(v.y, v.z, 16); w.S[3] = __funnelshift_l(v.z, v.w, 16);
+          w.S[4] = __funnelshift_l(v.w, b, 16);
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-              if (((X >> (16 * h)) & 0xFFFFu) == 0u) {
-                const u32 i = atomicAdd(&s.misc[0], 1u);
-                s.peaks[i] = (u16)((r << 8) | (2u * col + (u32)h - TPC_HALO));
-              }
-            }
+          for (int k = 0; k < 4; ++k) w.H[k] = vmax2(vmax2(w.S[k], w.C[k]), w.S[k + 1]);
+        };
+        auto test = [&](const Row& up, const Row& mid, const Row& dn, u32 r) {
+          u32 X[4], any = 0u;
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            const u32 M = vmax2(vmax2(vmax2(up.H[k], mid.S[k]) + 0x00010001u, dn.H[k]), vmax2(mid.S[k + 1], thr2));
+            X[k] = vmax2(mid.C[k], M) ^ mid.C[k];        // a zero half = that cell beats its 8 neighbours
+            any |= (X[k] - 0x00010001u) & ~X[k] & 0x80008000u;   // pre-filter: some half may be zero
           }
-          H0 = H1; H1 = H2; L1 = L2; C1 = C2; R1 = R2;
+          if (any) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+#pragma unroll
+              for (int h = 0; h < 2; ++h)
+                if (((X[k] >> (16 * h)) & 0xFFFFu) == 0u) {
+                  const u32 i = atomicAdd(&s.misc[0], 1u);
+                  s.peaks[i] = (u16)((r << 8) | (8u * g + 2u * (u32)k + (u32)h - TPC_HALO));
+                }
+          }
+        };
+        const u32* q = s.tile32 + (r0 - 1u) * nW + 4u * g;
+        Row ra, rb, rc;
+        load(q, ra); q += nW;
+        load(q, rb); q += nW;
+        for (u32 r = r0;;) {   // unrolled by 3 so the window rotates by renaming, not by moves
+          load(q, rc); test(ra, rb, rc, r); if (++r >= r1) break; q += nW;
+          load(q, ra); test(rb, rc, ra, r); if (++r >= r1) break; q += nW;
+          load(q, rb); test(rc, ra, rb, r); if (++r >= r1) break; q += nW;
         }
       }
     }
