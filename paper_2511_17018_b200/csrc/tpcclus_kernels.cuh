@@ -120,15 +120,15 @@ struct K1Smem {   // layout computed identically on the host (tpc_k1_smem_bytes)
 __host__ __device__ inline u32 tpc_k1_smem_bytes(u32 nb) {
   return (nb * (TPC_STAGE + 2u) + 4u * TPC_K1_SPILL + 8u) * 4u + TPC_K1_FQ * 2u + 512u;
 }
-__device__ __forceinline__ K1Smem k1_smem(u32* base, u32 nb) {
+__device__ __forceinline__ K1Smem k1_smem(u32* base, u32 nb) {   // fixed-size arrays first: constant offsets
   K1Smem s;
-  s.stage = base;
+  s.misc = base;
+  s.spill = s.misc + 8;
+  s.fq = (u16*)(s.spill + 4u * TPC_K1_SPILL);
+  s.npads = s.fq + TPC_K1_FQ;
+  s.stage = (u32*)(s.npads + 256);
   s.cnt = s.stage + nb * TPC_STAGE;
   s.pos = s.cnt + nb;
-  s.spill = s.pos + nb;
-  s.misc = s.spill + 4u * TPC_K1_SPILL;
-  s.fq = (u16*)(s.misc + 8);
-  s.npads = s.fq + TPC_K1_FQ;
   return s;
 }
 
@@ -178,11 +178,11 @@ __device__ __forceinline__ bool k1_queue_flush(const K1Smem& s, u32 par, u32 bin
 }
 
 // One pass = insert phase + flush phase (two block barriers).  Entries k with bit k of `pend`
-// set are still to be placed; bit k of `have` = entry k holds a reserved slot already.
+// set are still to be placed; FIRST = they have no reserved slot yet.
 // Returns (block-uniform) whether any thread still has a pending entry.
-template <int K>
+template <int K, bool FIRST>
 __device__ __forceinline__ bool k1_pass(const K1Smem& s, u32& cur, u32& par, const u32 (&bin)[K], const u32 (&rec)[K],
-                                        u32 (&slot)[K], u32& pend, u32& have, u32 slice_base, u32 slice_cap,
+                                        u32 (&slot)[K], u32& pend, u32 slice_base, u32 slice_cap,
                                         uint4* pool, u32* dir) {
   u32 lf = 0u, drain_bin = 0u;
   u32* sp_in = s.spill + cur * 2u * TPC_K1_SPILL;
@@ -198,8 +198,8 @@ __device__ __forceinline__ bool k1_pass(const K1Smem& s, u32& cur, u32& par, con
 #pragma unroll
   for (int k = 0; k < K; ++k) {
     if (pend & (1u << k)) {
-      if (have & (1u << k)) slot[k] -= 8u;
-      else { slot[k] = atomicAdd(&s.cnt[bin[k]], 1u); have |= 1u << k; }
+      if (FIRST) slot[k] = atomicAdd(&s.cnt[bin[k]], 1u);   // reserve; later passes: the bin was flushed once since
+      else slot[k] -= 8u;
       if (slot[k] < TPC_STAGE) {
         s.stage[bin[k] * TPC_STAGE + slot[k]] = rec[k];
         pend &= ~(1u << k);
@@ -234,6 +234,73 @@ __device__ __forceinline__ bool k1_pass(const K1Smem& s, u32& cur, u32& par, con
   return __syncthreads_or((int)pend) != 0;
 }
 
+template <bool MULTI_TC>
+__device__ __forceinline__ void k1_rounds(const K1Smem& s, const uint2* __restrict__ digits, u64 begin, u64 end, u32 slice_base,
+                                          u32 slice_cap, uint4* pool, u32* dir, u32& cur, u32& par, bool& bad) {
+  const u32 ROUND = TPC_K1_THREADS * TPC_K1_DPT, HALF = ROUND / (TPC_K1_DPT / 2);
+  const u32 S = PRM(n_sectors), R = PRM(n_rows), T = PRM(n_time), NTC = PRM(n_tc);
+  // thread t of a round owns digits 2t, 2t+1 of each half of the round (16-byte loads); digits
+  // past the end read as 0 = "charge 0, ignored", so the decode needs no bounds checks
+  auto fetch = [&](u64 base, uint4 (&d)[TPC_K1_DPT / 2]) {
+    const uint2* p = digits + base + 2u * threadIdx.x;
+    if (base + ROUND <= end) {
+#pragma unroll
+      for (int h = 0; h < TPC_K1_DPT / 2; ++h) d[h] = ld_stream_u4((const uint4*)(p + h * HALF));
+    } else {
+#pragma unroll
+      for (int h = 0; h < TPC_K1_DPT / 2; ++h) {
+        const u64 i = base + (u64)h * HALF + 2u * threadIdx.x;
+        if (i + 1u < end) d[h] = ld_stream_u4((const uint4*)(p + h * HALF));
+        else if (i < end) { const uint2 v = ld_stream_u2(p + h * HALF); d[h] = make_uint4(v.x, v.y, 0u, 0u); }
+        else d[h] = make_uint4(0u, 0u, 0u, 0u);
+      }
+    }
+  };
+  uint4 nxt[TPC_K1_DPT / 2];
+  fetch(begin, nxt);
+  for (u64 base = begin; base < end; base += ROUND) {
+    uint4 curd[TPC_K1_DPT / 2];
+#pragma unroll
+    for (int h = 0; h < TPC_K1_DPT / 2; ++h) curd[h] = nxt[h];
+    fetch(base + ROUND, nxt);   // prefetch the next round while this one is binned
+    u32 bin[TPC_K1_DPT], rec[TPC_K1_DPT], slot[TPC_K1_DPT], dbin[TPC_K1_DPT], drec[TPC_K1_DPT];
+    u32 pend = 0u, dpend = 0u;
+#pragma unroll
+    for (int k = 0; k < TPC_K1_DPT; ++k) {
+      const u32 w0 = (k & 1) ? curd[k >> 1].z : curd[k >> 1].x, w1 = (k & 1) ? curd[k >> 1].w : curd[k >> 1].y;
+      u32 q = w0 & 0xFFFFu;
+      const u32 t = w0 >> 16, pad = w1 & 0xFFu, row = (w1 >> 8) & 0xFFu, sec = (w1 >> 16) & 0xFFu;
+      // O0 / Q4: out of range -> ignored + flagged (npads[row] is 0 for row >= n_rows)
+      const bool valid = sec < S && t < T && pad < (u32)s.npads[row];
+      bad |= !valid;
+      q = q > 1023u ? 1023u : q;                                  // Q4: clamp
+      const bool ok = valid && q != 0u;                           // Q4: zero charge ignored
+      u32 tc = 0u, v = t;
+      if (MULTI_TC) { tc = t / TPC_TC; v = t - tc * TPC_TC; }
+      const u32 b0 = MULTI_TC ? (sec * R + row) * NTC + tc : sec * R + row;
+      bin[k] = ok ? b0 : 0u;
+      rec[k] = pad | ((v + TPC_HALO) << 8) | (q << 22);
+      pend |= ok ? (1u << k) : 0u;
+      if (MULTI_TC) {   // halo copy into the neighbouring time-chunk's bin
+        dbin[k] = 0u; drec[k] = 0u;
+        if (ok && v < TPC_HALO && tc > 0u) {
+          dbin[k] = b0 - 1u; drec[k] = pad | ((v + TPC_TC + TPC_HALO) << 8) | (q << 22); dpend |= 1u << k;
+        } else if (ok && v + TPC_HALO >= TPC_TC && tc + 1u < NTC) {
+          dbin[k] = b0 + 1u; drec[k] = pad | ((v + TPC_HALO - TPC_TC) << 8) | (q << 22); dpend |= 1u << k;
+        }
+      }
+    }
+    if (k1_pass<TPC_K1_DPT, true>(s, cur, par, bin, rec, slot, pend, slice_base, slice_cap, pool, dir))
+      while (k1_pass<TPC_K1_DPT, false>(s, cur, par, bin, rec, slot, pend, slice_base, slice_cap, pool, dir)) {}
+    if (MULTI_TC) {
+      if (__syncthreads_or((int)dpend)) {
+        if (k1_pass<TPC_K1_DPT, true>(s, cur, par, dbin, drec, slot, dpend, slice_base, slice_cap, pool, dir))
+          while (k1_pass<TPC_K1_DPT, false>(s, cur, par, dbin, drec, slot, dpend, slice_base, slice_cap, pool, dir)) {}
+      }
+    }
+  }
+}
+
 extern "C" __global__ void __launch_bounds__(TPC_K1_THREADS, 1)
 k_partition_coarse(const uint2* __restrict__ digits, u64 n, u64 per_cta, uint4* __restrict__ pool,
                    u32* __restrict__ dir, u32* __restrict__ used, u32 slice_cap, u32* __restrict__ status) {
@@ -249,71 +316,14 @@ k_partition_coarse(const uint2* __restrict__ digits, u64 n, u64 per_cta, uint4* 
   const u64 begin = (u64)blockIdx.x * per_cta;   // a multiple of the round: 16-byte aligned loads
   u64 end = begin + per_cta;
   if (end > n) end = n;
-  const u32 ROUND = TPC_K1_THREADS * TPC_K1_DPT;
-  const u32 S = PRM(n_sectors), R = PRM(n_rows), T = PRM(n_time), NTC = PRM(n_tc);
   u32 cur = 0u, par = 0u;
-
-  // thread t of a round owns digits 2t, 2t+1 of each half of the round (two 16-byte loads)
-  auto fetch = [&](u64 base, uint4 (&d)[TPC_K1_DPT / 2]) {
-#pragma unroll
-    for (int h = 0; h < TPC_K1_DPT / 2; ++h) {
-      const u64 i = base + (u64)h * (ROUND / (TPC_K1_DPT / 2)) + 2u * threadIdx.x;
-      if (i + 1u < end) d[h] = ld_stream_u4((const uint4*)(digits + i));
-      else if (i < end) { const uint2 v = ld_stream_u2(digits + i); d[h] = make_uint4(v.x, v.y, 0u, 0u); }
-      else d[h] = make_uint4(0u, 0u, 0u, 0u);
-    }
-  };
-  uint4 nxt[TPC_K1_DPT / 2];
-  fetch(begin, nxt);
   bool bad = false;
-  for (u64 base = begin; base < end; base += ROUND) {
-    uint4 curd[TPC_K1_DPT / 2];
-#pragma unroll
-    for (int h = 0; h < TPC_K1_DPT / 2; ++h) curd[h] = nxt[h];
-    fetch(base + ROUND, nxt);   // prefetch the next round while this one is binned
-    u32 bin[TPC_K1_DPT], rec[TPC_K1_DPT], slot[TPC_K1_DPT], dbin[TPC_K1_DPT], drec[TPC_K1_DPT];
-    u32 pend = 0u, dpend = 0u;
-#pragma unroll
-    for (int k = 0; k < TPC_K1_DPT; ++k) {
-      const u64 i = base + (u64)(k >> 1) * (ROUND / (TPC_K1_DPT / 2)) + 2u * threadIdx.x + (u32)(k & 1);
-      const u32 w0 = (k & 1) ? curd[k >> 1].z : curd[k >> 1].x, w1 = (k & 1) ? curd[k >> 1].w : curd[k >> 1].y;
-      bin[k] = 0u; rec[k] = 0u; dbin[k] = 0u; drec[k] = 0u;
-      if (i < end) {
-        u32 q = w0 & 0xFFFFu;
-        const u32 t = w0 >> 16, pad = w1 & 0xFFu, row = (w1 >> 8) & 0xFFu, sec = (w1 >> 16) & 0xFFu;
-        if (sec >= S || row >= R || t >= T || pad >= (u32)s.npads[row]) {   // O0 / Q4: ignore + flag
-          bad = true;
-        } else if (q != 0u) {                                               // Q4: zero charge ignored
-          q = q > 1023u ? 1023u : q;                                        // Q4: clamp
-          const u32 tc = (NTC > 1u) ? t / TPC_TC : 0u;
-          const u32 v = t - tc * TPC_TC;
-          const u32 b0 = (sec * R + row) * NTC + tc;
-          bin[k] = b0;
-          rec[k] = pad | ((v + TPC_HALO) << 8) | (q << 22);
-          pend |= 1u << k;
-          if (NTC > 1u) {   // halo copy into the neighbouring time-chunk's bin
-            if (v < TPC_HALO && tc > 0u) {
-              dbin[k] = b0 - 1u; drec[k] = pad | ((v + TPC_TC + TPC_HALO) << 8) | (q << 22); dpend |= 1u << k;
-            } else if (v + TPC_HALO >= TPC_TC && tc + 1u < NTC) {
-              dbin[k] = b0 + 1u; drec[k] = pad | ((v + TPC_HALO - TPC_TC) << 8) | (q << 22); dpend |= 1u << k;
-            }
-          }
-        }
-      }
-    }
-    u32 have = 0u;
-    while (k1_pass<TPC_K1_DPT>(s, cur, par, bin, rec, slot, pend, have, slice_base, slice_cap, pool, dir)) {}
-    if (NTC > 1u) {
-      if (__syncthreads_or((int)dpend)) {
-        have = 0u;
-        while (k1_pass<TPC_K1_DPT>(s, cur, par, dbin, drec, slot, dpend, have, slice_base, slice_cap, pool, dir)) {}
-      }
-    }
-  }
+  if (PRM(n_tc) > 1u) k1_rounds<true>(s, digits, begin, end, slice_base, slice_cap, pool, dir, cur, par, bad);
+  else k1_rounds<false>(s, digits, begin, end, slice_base, slice_cap, pool, dir, cur, par, bad);
   if (bad) atomicOr(status, TPC_STATUS_BAD_DIGITS);
   {   // records still parked in the spill list (block-uniform: misc is stable after a pass)
-    u32 bin[1] = {0u}, rec[1] = {0u}, slot[1] = {0u}, pend = 0u, have = 0u;
-    while (s.misc[2u + cur] != 0u) k1_pass<1>(s, cur, par, bin, rec, slot, pend, have, slice_base, slice_cap, pool, dir);
+    u32 bin[1] = {0u}, rec[1] = {0u}, slot[1] = {0u}, pend = 0u;
+    while (s.misc[2u + cur] != 0u) k1_pass<1, false>(s, cur, par, bin, rec, slot, pend, slice_base, slice_cap, pool, dir);
   }
   __syncthreads();
   // drain: every bin's partial stage goes to its current (or a fresh) chunk, unused slots zeroed;
