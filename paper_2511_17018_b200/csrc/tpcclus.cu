@@ -33,7 +33,7 @@ inline uint64_t align_up(uint64_t x, uint64_t a) { return (x + a - 1) / a * a; }
 struct Layout {   // byte offsets into the workspace
   uint64_t counters, counters_bytes;   // zeroed at the head of every run
   uint64_t status, blob_cursor, bin_nchunks, bin_fill;
-  uint64_t used, bin_chunk_start, batch_start, dir, chunk_list, pool, blob, idx;
+  uint64_t used, bin_chunk_start, batch_start, batch_bin, dir, chunk_list, pool, blob, idx;
   uint64_t tile_cnt, tile_local, block_sum, block_prefix, row_off;
   uint64_t total;        // device-path workspace
   uint64_t host_digits;  // staging of run_host (beyond `total`)
@@ -115,6 +115,7 @@ int make_geometry(const tpcclus_params* p, Geometry* g) {
   L.used = take(4ull * g->g1);
   L.bin_chunk_start = take(4ull * (nb + 1));
   L.batch_start = take(4ull * (nb + 1));
+  L.batch_bin = take(4ull * g->n_batches_max);
   L.dir = take(4ull * g->n_chunks_max);
   L.chunk_list = take(4ull * g->n_chunks_max);
   L.pool = take(256ull * g->n_chunks_max);
@@ -331,10 +332,10 @@ int tpcclus_create(const tpcclus_params* p, tpcclus_handle** out) {
   h->params.n_pads = h->g.prm.n_pads;
   h->ws = (char*)p->workspace;
   h->smem_k1 = tpc_k1_smem_bytes(g.prm.n_bins);
-  h->smem_k5 = (TPC_K5_BUF + 128u * 3u + 132u + 8u) * 4u;
+  h->smem_k5 = tpc_k5_smem_bytes();
   h->smem_k6 = tpc_k6_smem_bytes(g.prm.pitch, g.prm.max_peaks);
   h->grid_k5 = g.g1 * 2u;
-  h->grid_k6 = g.g1 * 3u < g.n_tiles ? g.g1 * 3u : g.n_tiles;
+  h->grid_k6 = g.g1 * TPC_K6_CTAS < g.n_tiles ? g.g1 * TPC_K6_CTAS : g.n_tiles;
   auto bail = [&](int code) { std::string e = h->err.empty() ? g_create_error : h->err; delete h; g_create_error = e; return code; };
   // static table for the debug map hook
   std::vector<uint64_t> ro(p->n_rows + 1, 0);
@@ -412,7 +413,7 @@ double tpcclus_rtc_build_ms(const tpcclus_handle* h) { return h ? h->rtc_ms : 0.
 namespace {
 
 struct RunPtrs {
-  u32 *status, *bin_nchunks, *bin_fill, *used, *bin_chunk_start, *batch_start, *dir, *chunk_list, *blob;
+  u32 *status, *bin_nchunks, *bin_fill, *used, *bin_chunk_start, *batch_start, *batch_bin, *dir, *chunk_list, *blob;
   u32 *tile_cnt, *tile_local, *block_sum;
   u64 *blob_cursor, *idx, *block_prefix, *row_off;
   uint4* pool;
@@ -423,7 +424,7 @@ RunPtrs ptrs(tpcclus_handle* h) {
   RunPtrs p;
   p.status = (u32*)(w + L.status); p.blob_cursor = (u64*)(w + L.blob_cursor);
   p.bin_nchunks = (u32*)(w + L.bin_nchunks); p.bin_fill = (u32*)(w + L.bin_fill); p.used = (u32*)(w + L.used);
-  p.bin_chunk_start = (u32*)(w + L.bin_chunk_start); p.batch_start = (u32*)(w + L.batch_start);
+  p.bin_chunk_start = (u32*)(w + L.bin_chunk_start); p.batch_start = (u32*)(w + L.batch_start); p.batch_bin = (u32*)(w + L.batch_bin);
   p.dir = (u32*)(w + L.dir); p.chunk_list = (u32*)(w + L.chunk_list); p.pool = (uint4*)(w + L.pool);
   p.blob = (u32*)(w + L.blob); p.idx = (u64*)(w + L.idx);
   p.tile_cnt = (u32*)(w + L.tile_cnt); p.tile_local = (u32*)(w + L.tile_local);
@@ -451,11 +452,11 @@ int enqueue_binning(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n
   u32 gx = (slice_cap + 255u) / 256u; if (gx > 32u) gx = 32u;
   { void* a[] = {&p.dir, &p.used, &slice_cap, &p.bin_nchunks};
     if ((rc = launch(h, K_DIR_COUNT, dim3(gx, g.g1), dim3(256), 0, st, a))) return rc; }
-  { void* a[] = {&p.bin_nchunks, &p.bin_chunk_start, &p.batch_start};
+  { void* a[] = {&p.bin_nchunks, &p.bin_chunk_start, &p.batch_start, &p.batch_bin};
     if ((rc = launch(h, K_DIR_SCAN, dim3(1), dim3(TPC_SCAN_THREADS), 0, st, a))) return rc; }
   { void* a[] = {&p.dir, &p.used, &slice_cap, &p.bin_chunk_start, &p.bin_fill, &p.chunk_list};
     if ((rc = launch(h, K_DIR_FILL, dim3(gx, g.g1), dim3(256), 0, st, a))) return rc; }
-  { void* a[] = {&p.pool, &p.dir, &p.chunk_list, &p.bin_chunk_start, &p.batch_start, &p.blob, &p.blob_cursor, &p.idx};
+  { void* a[] = {&p.pool, &p.dir, &p.chunk_list, &p.bin_chunk_start, &p.batch_start, &p.batch_bin, &p.blob, &p.blob_cursor, &p.idx};
     if ((rc = launch(h, K_PART_FINE, dim3(h->grid_k5), dim3(TPC_K5_THREADS), h->smem_k5, st, a))) return rc; }
   return TPCCLUS_OK;
 }

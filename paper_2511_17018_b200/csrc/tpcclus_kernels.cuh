@@ -112,21 +112,19 @@ struct K1Smem {   // layout computed identically on the host (tpc_k1_smem_bytes)
   u32* stage;     // [NB][8]
   u32* cnt;       // [NB]  records reserved in the stage (may exceed 8 until the flush)
   u32* pos;       // [NB]  (chunk_local << 4) | sectors_filled(0..8)
-  u32* spill;     // [2][TPC_K1_SPILL][2]  {rec, bin | slot << 16}
-  u32* misc;      // [0] next chunk  [1] flush-queue length  [2],[3] spill lengths
-  u16* fq;        // [TPC_K1_FQ]
-  u16* npads;     // [256]
+  u32* spill;     // [2][warps][TPC_K1_WSP][2]  {rec, bin | slot << 16}
+  u32* misc;      // [0] next chunk
+  u16* fq;        // [warps][TPC_K1_WFQ]
 };
 __host__ __device__ inline u32 tpc_k1_smem_bytes(u32 nb) {
-  return (nb * (TPC_STAGE + 2u) + 4u * TPC_K1_SPILL + 8u) * 4u + TPC_K1_FQ * 2u + 512u;
+  return (nb * (TPC_STAGE + 2u) + 4u * TPC_K1_SPILL + 8u) * 4u + TPC_K1_FQ * 2u;
 }
 __device__ __forceinline__ K1Smem k1_smem(u32* base, u32 nb) {   // fixed-size arrays first: constant offsets
   K1Smem s;
   s.misc = base;
   s.spill = s.misc + 8;
   s.fq = (u16*)(s.spill + 4u * TPC_K1_SPILL);
-  s.npads = s.fq + TPC_K1_FQ;
-  s.stage = (u32*)(s.npads + 256);
+  s.stage = (u32*)(s.fq + TPC_K1_FQ);
   s.cnt = s.stage + nb * TPC_STAGE;
   s.pos = s.cnt + nb;
   return s;
@@ -170,58 +168,70 @@ __device__ __forceinline__ void k1_flush_single(const K1Smem& s, u32 bin, u32 sl
   if (c < slice_cap) st_256(pool + ((u64)(slice_base + c) * 16u + fill * 2u), st[0], st[1]);
 }
 
-// Queues `bin` for the flush phase; when the queue is full the caller flushes it itself (bit in lf).
-__device__ __forceinline__ bool k1_queue_flush(const K1Smem& s, u32 par, u32 bin) {
-  const u32 j = atomicAdd(&s.misc[4u + par], 1u);
-  if (j < TPC_K1_FQ) { s.fq[j] = (u16)bin; return true; }
-  return false;
-}
+#define TPC_K1_WFQ (TPC_K1_FQ / (TPC_K1_THREADS / 32))        // flush-queue entries per warp (64)
+#define TPC_K1_WSP (TPC_K1_SPILL / (TPC_K1_THREADS / 32))     // spill entries per warp and buffer (16)
 
 // One pass = insert phase + flush phase (two block barriers).  Entries k with bit k of `pend`
-// set are still to be placed; FIRST = they have no reserved slot yet.
+// set are still to be placed; FIRST = they have no reserved slot yet.  The flush queue and
+// the spill list are private to the warp and filled with ballots, so the only shared-memory
+// atomics are the slot reservations.  `nsp` = entries this warp parked in the previous pass.
 // Returns (block-uniform) whether any thread still has a pending entry.
 template <int K, bool FIRST>
-__device__ __forceinline__ bool k1_pass(const K1Smem& s, u32& cur, u32& par, const u32 (&bin)[K], const u32 (&rec)[K],
+__device__ __forceinline__ bool k1_pass(const K1Smem& s, u32& cur, u32& nsp, const u32 (&bin)[K], const u32 (&rec)[K],
                                         u32 (&slot)[K], u32& pend, u32 slice_base, u32 slice_cap,
                                         uint4* pool, u32* dir) {
-  u32 lf = 0u, drain_bin = 0u;
-  u32* sp_in = s.spill + cur * 2u * TPC_K1_SPILL;
-  u32* sp_out = s.spill + (cur ^ 1u) * 2u * TPC_K1_SPILL;
-  u32 nsp = s.misc[2u + cur];
-  if (nsp > TPC_K1_SPILL) nsp = TPC_K1_SPILL;
-  if (threadIdx.x < nsp) {   // records parked in the previous pass: their bin was flushed since, slot - 8 < 8
-    const u32 r = sp_in[2u * threadIdx.x], w = sp_in[2u * threadIdx.x + 1u];
-    const u32 b = w & 0xFFFFu, sl = (w >> 16) - 8u;
-    s.stage[b * TPC_STAGE + sl] = r;
-    if (sl == TPC_STAGE - 1u && !k1_queue_flush(s, par, b)) { lf |= 1u << K; drain_bin = b; }
+  const u32 lane = lane_id(), warp = threadIdx.x >> 5, lt = (1u << lane) - 1u;
+  u16* fq = s.fq + warp * TPC_K1_WFQ;
+  u32* sp_in = s.spill + ((cur * (TPC_K1_THREADS / 32) + warp) * TPC_K1_WSP) * 2u;
+  u32* sp_out = s.spill + (((cur ^ 1u) * (TPC_K1_THREADS / 32) + warp) * TPC_K1_WSP) * 2u;
+  u32 lf = 0u, drain_bin = 0u, nfq = 0u, nout = 0u;
+  auto queue = [&](bool fl, u32 b, int bit) {   // warp-wide: every lane calls it
+    const u32 m = __ballot_sync(0xFFFFFFFFu, fl);
+    if (fl) {
+      const u32 i = nfq + __popc(m & lt);
+      if (i < TPC_K1_WFQ) fq[i] = (u16)b;
+      else { lf |= 1u << bit; if (bit == K) drain_bin = b; }   // queue full: flush it myself
+    }
+    nfq += __popc(m);
+  };
+  {   // records parked in the previous pass: their bin was flushed since, slot - 8 < 8
+    bool fl = false;
+    u32 b = 0u;
+    if (lane < nsp) {
+      const u32 r = sp_in[2u * lane], w = sp_in[2u * lane + 1u];
+      b = w & 0xFFFFu;
+      const u32 sl = (w >> 16) - 8u;
+      s.stage[b * TPC_STAGE + sl] = r;
+      fl = sl == TPC_STAGE - 1u;
+    }
+    queue(fl, b, K);
+  }
+#pragma unroll
+  for (int k = 0; k < K; ++k) {   // reserve: independent atomics first
+    if (FIRST) slot[k] = (pend & (1u << k)) ? atomicAdd(&s.cnt[bin[k]], 1u) : 0xFFFFFFFFu;
+    else slot[k] = (pend & (1u << k)) ? slot[k] - 8u : 0xFFFFFFFFu;
   }
 #pragma unroll
   for (int k = 0; k < K; ++k) {
-    if (pend & (1u << k)) {
-      if (FIRST) slot[k] = atomicAdd(&s.cnt[bin[k]], 1u);   // reserve; later passes: the bin was flushed once since
-      else slot[k] -= 8u;
-      if (slot[k] < TPC_STAGE) {
-        s.stage[bin[k] * TPC_STAGE + slot[k]] = rec[k];
-        pend &= ~(1u << k);
-        if (slot[k] == TPC_STAGE - 1u && !k1_queue_flush(s, par, bin[k])) lf |= 1u << k;
-      } else if (slot[k] < 2u * TPC_STAGE) {
-        const u32 j = atomicAdd(&s.misc[2u + (cur ^ 1u)], 1u);
-        if (j < TPC_K1_SPILL) {
-          sp_out[2u * j] = rec[k];
-          sp_out[2u * j + 1u] = bin[k] | (slot[k] << 16);
-          pend &= ~(1u << k);
-        }
-      }
+    const u32 sl = slot[k];
+    if (sl < TPC_STAGE) { s.stage[bin[k] * TPC_STAGE + sl] = rec[k]; pend &= ~(1u << k); }
+    queue(sl == TPC_STAGE - 1u, bin[k], k);
+    const bool sp = sl >= TPC_STAGE && sl < 2u * TPC_STAGE;   // the stage is full until the flush: park it
+    const u32 m = __ballot_sync(0xFFFFFFFFu, sp);
+    if (sp) {
+      const u32 i = nout + __popc(m & lt);
+      if (i < TPC_K1_WSP) { sp_out[2u * i] = rec[k]; sp_out[2u * i + 1u] = bin[k] | (sl << 16); pend &= ~(1u << k); }
     }
+    nout += __popc(m);
   }
+  nsp = nout < TPC_K1_WSP ? nout : TPC_K1_WSP;
   __syncthreads();
-  // ---- flush phase ---------------------------------------------------------------------------
-  u32 nf = s.misc[4u + par];
-  if (nf > TPC_K1_FQ) nf = TPC_K1_FQ;
-  const u32 lim = (2u * nf + 31u) & ~31u;
-  for (u32 j = threadIdx.x; j < lim; j += TPC_K1_THREADS) {
-    const bool act = j < 2u * nf;
-    k1_flush_pair(s, act, act ? (u32)s.fq[j >> 1] : 0u, slice_base, slice_cap, pool, dir);
+  // ---- flush phase: every warp works off its own queue, one lane pair per 32-byte stage ----
+  if (nfq > TPC_K1_WFQ) nfq = TPC_K1_WFQ;
+  for (u32 j0 = 0u; j0 < nfq; j0 += 16u) {
+    const u32 j = j0 + (lane >> 1);
+    const bool act = j < nfq;
+    k1_flush_pair(s, act, act ? (u32)fq[j] : 0u, slice_base, slice_cap, pool, dir);
   }
   if (lf) {   // the queue was full
 #pragma unroll
@@ -229,14 +239,13 @@ __device__ __forceinline__ bool k1_pass(const K1Smem& s, u32& cur, u32& par, con
       if (lf & (1u << k)) k1_flush_single(s, bin[k], slice_base, slice_cap, pool, dir);
     if (lf & (1u << K)) k1_flush_single(s, drain_bin, slice_base, slice_cap, pool, dir);
   }
-  if (threadIdx.x == 0) { s.misc[2u + cur] = 0u; s.misc[4u + (par ^ 1u)] = 0u; }
-  cur ^= 1u; par ^= 1u;
+  cur ^= 1u;
   return __syncthreads_or((int)pend) != 0;
 }
 
 template <bool MULTI_TC>
 __device__ __forceinline__ void k1_rounds(const K1Smem& s, const uint2* __restrict__ digits, u64 begin, u64 end, u32 slice_base,
-                                          u32 slice_cap, uint4* pool, u32* dir, u32& cur, u32& par, bool& bad) {
+                                          u32 slice_cap, uint4* pool, u32* dir, u32& cur, u32& nsp, bool& bad) {
   const u32 ROUND = TPC_K1_THREADS * TPC_K1_DPT, HALF = ROUND / (TPC_K1_DPT / 2);
   const u32 S = PRM(n_sectors), R = PRM(n_rows), T = PRM(n_time), NTC = PRM(n_tc);
   // thread t of a round owns digits 2t, 2t+1 of each half of the round (16-byte loads); digits
@@ -270,8 +279,8 @@ __device__ __forceinline__ void k1_rounds(const K1Smem& s, const uint2* __restri
       const u32 w0 = (k & 1) ? curd[k >> 1].z : curd[k >> 1].x, w1 = (k & 1) ? curd[k >> 1].w : curd[k >> 1].y;
       u32 q = w0 & 0xFFFFu;
       const u32 t = w0 >> 16, pad = w1 & 0xFFu, row = (w1 >> 8) & 0xFFu, sec = (w1 >> 16) & 0xFFu;
-      // O0 / Q4: out of range -> ignored + flagged (npads[row] is 0 for row >= n_rows)
-      const bool valid = sec < S && t < T && pad < (u32)s.npads[row];
+      // O0 / Q4: out of range -> ignored + flagged (pad >= n_pads[row] is caught by K6, where the row is uniform)
+      const bool valid = sec < S && row < R && t < T;
       bad |= !valid;
       q = q > 1023u ? 1023u : q;                                  // Q4: clamp
       const bool ok = valid && q != 0u;                           // Q4: zero charge ignored
@@ -290,12 +299,12 @@ __device__ __forceinline__ void k1_rounds(const K1Smem& s, const uint2* __restri
         }
       }
     }
-    if (k1_pass<TPC_K1_DPT, true>(s, cur, par, bin, rec, slot, pend, slice_base, slice_cap, pool, dir))
-      while (k1_pass<TPC_K1_DPT, false>(s, cur, par, bin, rec, slot, pend, slice_base, slice_cap, pool, dir)) {}
+    if (k1_pass<TPC_K1_DPT, true>(s, cur, nsp, bin, rec, slot, pend, slice_base, slice_cap, pool, dir))
+      while (k1_pass<TPC_K1_DPT, false>(s, cur, nsp, bin, rec, slot, pend, slice_base, slice_cap, pool, dir)) {}
     if (MULTI_TC) {
       if (__syncthreads_or((int)dpend)) {
-        if (k1_pass<TPC_K1_DPT, true>(s, cur, par, dbin, drec, slot, dpend, slice_base, slice_cap, pool, dir))
-          while (k1_pass<TPC_K1_DPT, false>(s, cur, par, dbin, drec, slot, dpend, slice_base, slice_cap, pool, dir)) {}
+        if (k1_pass<TPC_K1_DPT, true>(s, cur, nsp, dbin, drec, slot, dpend, slice_base, slice_cap, pool, dir))
+          while (k1_pass<TPC_K1_DPT, false>(s, cur, nsp, dbin, drec, slot, dpend, slice_base, slice_cap, pool, dir)) {}
       }
     }
   }
@@ -309,21 +318,20 @@ k_partition_coarse(const uint2* __restrict__ digits, u64 n, u64 per_cta, uint4* 
   const K1Smem s = k1_smem(smem_u32, nb);
   for (u32 i = threadIdx.x; i < nb; i += TPC_K1_THREADS) { s.pos[i] = 8u; s.cnt[i] = 0u; }
   if (threadIdx.x < 8) s.misc[threadIdx.x] = 0u;
-  if (threadIdx.x < 256) s.npads[threadIdx.x] = threadIdx.x < PRM(n_rows) ? PRM_NPADS(threadIdx.x) : (u16)0;
   __syncthreads();
 
   const u32 slice_base = blockIdx.x * slice_cap;
   const u64 begin = (u64)blockIdx.x * per_cta;   // a multiple of the round: 16-byte aligned loads
   u64 end = begin + per_cta;
   if (end > n) end = n;
-  u32 cur = 0u, par = 0u;
+  u32 cur = 0u, nsp = 0u;
   bool bad = false;
-  if (PRM(n_tc) > 1u) k1_rounds<true>(s, digits, begin, end, slice_base, slice_cap, pool, dir, cur, par, bad);
-  else k1_rounds<false>(s, digits, begin, end, slice_base, slice_cap, pool, dir, cur, par, bad);
+  if (PRM(n_tc) > 1u) k1_rounds<true>(s, digits, begin, end, slice_base, slice_cap, pool, dir, cur, nsp, bad);
+  else k1_rounds<false>(s, digits, begin, end, slice_base, slice_cap, pool, dir, cur, nsp, bad);
   if (bad) atomicOr(status, TPC_STATUS_BAD_DIGITS);
-  {   // records still parked in the spill list (block-uniform: misc is stable after a pass)
+  {   // records still parked in the spill lists
     u32 bin[1] = {0u}, rec[1] = {0u}, slot[1] = {0u}, pend = 0u;
-    while (s.misc[2u + cur] != 0u) k1_pass<1, false>(s, cur, par, bin, rec, slot, pend, slice_base, slice_cap, pool, dir);
+    while (__syncthreads_or((int)nsp)) k1_pass<1, false>(s, cur, nsp, bin, rec, slot, pend, slice_base, slice_cap, pool, dir);
   }
   __syncthreads();
   // drain: every bin's partial stage goes to its current (or a fresh) chunk, unused slots zeroed;
@@ -369,8 +377,10 @@ k_dir_count(const u32* __restrict__ dir, const u32* __restrict__ used, u32 slice
 // single CTA: exclusive scans over the bins.
 //   bin_chunk_start[b] = sum_{b'<b} nchunks[b']          (NB+1 entries)
 //   batch_start[b]     = sum_{b'<b} ceil(nchunks[b']/CPB) (NB+1 entries; [NB] = total batches)
+//   batch_bin[k]       = the bin batch k belongs to
 extern "C" __global__ void __launch_bounds__(TPC_SCAN_THREADS)
-k_dir_scan(const u32* __restrict__ bin_nchunks, u32* __restrict__ bin_chunk_start, u32* __restrict__ batch_start) {
+k_dir_scan(const u32* __restrict__ bin_nchunks, u32* __restrict__ bin_chunk_start, u32* __restrict__ batch_start,
+           u32* __restrict__ batch_bin) {
   __shared__ u32 s_a[TPC_SCAN_THREADS], s_b[TPC_SCAN_THREADS];
   const u32 nb = PRM(n_bins);
   const u32 per = (nb + TPC_SCAN_THREADS - 1u) / TPC_SCAN_THREADS;
@@ -392,7 +402,9 @@ k_dir_scan(const u32* __restrict__ bin_nchunks, u32* __restrict__ bin_chunk_star
   for (u32 b = lo; b < hi; ++b) {
     u32 c = bin_nchunks[b];
     bin_chunk_start[b] = ea; batch_start[b] = eb;
-    ea += c; eb += (c + TPC_CPB - 1u) / TPC_CPB;
+    const u32 nbt = (c + TPC_CPB - 1u) / TPC_CPB;
+    for (u32 k = 0u; k < nbt; ++k) batch_bin[eb + k] = b;   // batch -> its bin, for K5
+    ea += c; eb += nbt;
   }
   if (threadIdx.x == TPC_SCAN_THREADS - 1u) { bin_chunk_start[nb] = s_a[threadIdx.x]; batch_start[nb] = s_b[threadIdx.x]; }
 }
@@ -474,36 +486,35 @@ k_scan_sums(const u32* __restrict__ block_sum, u64* __restrict__ block_prefix, u
 // tile record (4 B):  pad[0:8) | tl[8:16) | q[16:26)   tl = row of the tile, 0..TPC_TT-1
 // tile sl of a bin holds u in [sl*TS, sl*TS + TS + 6);  it OWNS tl in [3, TS+3).
 // ==========================================================================================
-#define TPC_K5_BUF (2u * TPC_CPB * TPC_CHUNK + 8u * 128u)   // u32 words: records + halo copies + run padding
+#define TPC_NSLMAX 128u   // >= slabs per bin: TPC_TC / TPC_TS = 127
+#define TPC_K5_BUF (2u * TPC_CPB * TPC_CHUNK + 8u * TPC_NSLMAX)   // u32 words: records + halo copies + run padding
+__host__ __device__ inline u32 tpc_k5_smem_bytes() { return (TPC_K5_BUF + 4u * TPC_NSLMAX + 8u) * 4u; }
 
 extern "C" __global__ void __launch_bounds__(TPC_K5_THREADS, 2)
 k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, const u32* __restrict__ chunk_list,
                  const u32* __restrict__ bin_chunk_start, const u32* __restrict__ batch_start,
-                 u32* __restrict__ blob, u64* __restrict__ blob_cursor, u64* __restrict__ idx) {
+                 const u32* __restrict__ batch_bin, u32* __restrict__ blob, u64* __restrict__ blob_cursor,
+                 u64* __restrict__ idx) {
   extern __shared__ __align__(128) u32 smem_u32[];
   u32* buf = smem_u32;                       // [TPC_K5_BUF]
-  u32* s_cnt = buf + TPC_K5_BUF;             // [128] primaries per slab
-  u32* s_dcnt = s_cnt + 128;                 // [128] halo copies per slab
-  u32* s_off = s_dcnt + 128;                 // [129] run start (multiple of 8)
-  u32* s_dcur = s_off + 132;                 // [128]
+  u32* s_cnt = buf + TPC_K5_BUF;             // [NSLMAX] primaries per slab
+  u32* s_dcnt = s_cnt + TPC_NSLMAX;          // [NSLMAX] halo copies per slab
+  u32* s_off = s_dcnt + TPC_NSLMAX;          // [NSLMAX + 1] run start (multiple of 8)
+  u32* s_dcur = s_off + TPC_NSLMAX + 4u;     // [NSLMAX]
   __shared__ u64 s_gbase;
   const u32 nb = PRM(n_bins), nsl = PRM(n_sl);
   const u32 n_batches = batch_start[nb];
 
   for (u32 batch = blockIdx.x; batch < n_batches; batch += gridDim.x) {
-    // bin of this batch: last b with batch_start[b] <= batch
-    u32 lo = 0u, hi = nb;
-    while (hi - lo > 1u) { u32 mid = (lo + hi) >> 1; if (batch_start[mid] <= batch) lo = mid; else hi = mid; }
-    const u32 b = lo;
+    const u32 b = batch_bin[batch];
+    if (threadIdx.x < TPC_NSLMAX) { s_cnt[threadIdx.x] = 0u; s_dcnt[threadIdx.x] = 0u; s_dcur[threadIdx.x] = 0u; }
+    __syncthreads();
     const u32 kb = batch - batch_start[b];
     const u32 nbatch_b = batch_start[b + 1] - batch_start[b];
     const u32 c0 = bin_chunk_start[b] + kb * TPC_CPB;
     u32 c1 = c0 + TPC_CPB;
     if (c1 > bin_chunk_start[b + 1]) c1 = bin_chunk_start[b + 1];
     const u32 nch = c1 - c0;
-
-    if (threadIdx.x < 128) { s_cnt[threadIdx.x] = 0u; s_dcnt[threadIdx.x] = 0u; s_dcur[threadIdx.x] = 0u; }
-    __syncthreads();
 
     // ---- load <= 16 records per thread, count per slab, remember the rank ------------------
     u32 rec[16];
@@ -513,16 +524,18 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
       u32 q4 = threadIdx.x + (u32)i * TPC_K5_THREADS;   // 16-byte piece of the batch
       u32 ch = q4 >> 4, sub = q4 & 15u;
       uint4 v = make_uint4(0u, 0u, 0u, 0u);
-      u32 nrec = 0u;
       if (ch < nch) {
         u32 cid = chunk_list[c0 + ch];
-        nrec = dir[cid] & 0xFFu;
+        // K1 writes whole 32-byte sectors and zero-fills the last one: a piece is valid or not as a
+        // whole.  Both loads are issued before the test (a chunk is always 256 allocated bytes).
+        const u32 nrec = dir[cid] & 0xFFu;
         v = ld_stream_u4(pool + (u64)cid * 16u + sub);
+        if (sub * 4u >= nrec) v = make_uint4(0u, 0u, 0u, 0u);
       }
       u32 r4[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
-        u32 r = (sub * 4u + (u32)j < nrec) ? r4[j] : 0u;   // q >= 1 in every valid record, so 0 = none
+        u32 r = r4[j];   // q >= 1 in every valid record, so 0 = none
         u32 rk = 0u;
         if (r != 0u) {
           u32 u = (r >> 8) & 0x3FFFu;
@@ -535,12 +548,12 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
       }
     }
     __syncthreads();
-    // ---- exclusive scan of padded run lengths (one warp, 4 slabs per lane) -----------------
+    // ---- exclusive scan of padded run lengths (one warp, NSLMAX/32 slabs per lane) ---------
     if (threadIdx.x < 32) {
-      u32 len[4], t = 0u;
+      u32 len[TPC_NSLMAX / 32u], t = 0u;
 #pragma unroll
-      for (int k = 0; k < 4; ++k) {
-        u32 sl = threadIdx.x * 4u + (u32)k;
+      for (int k = 0; k < (int)(TPC_NSLMAX / 32u); ++k) {
+        u32 sl = threadIdx.x * (TPC_NSLMAX / 32u) + (u32)k;
         len[k] = sl < nsl ? ((s_cnt[sl] + s_dcnt[sl] + 7u) & ~7u) : 0u;
         t += len[k];
       }
@@ -549,9 +562,9 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
       for (int d = 1; d < 32; d <<= 1) { u32 o = __shfl_up_sync(0xFFFFFFFFu, inc, d); if ((int)threadIdx.x >= d) inc += o; }
       u32 e = inc - t;
 #pragma unroll
-      for (int k = 0; k < 4; ++k) { s_off[threadIdx.x * 4u + (u32)k] = e; e += len[k]; }
+      for (int k = 0; k < (int)(TPC_NSLMAX / 32u); ++k) { s_off[threadIdx.x * (TPC_NSLMAX / 32u) + (u32)k] = e; e += len[k]; }
       if (threadIdx.x == 31) {
-        s_off[128] = inc;
+        s_off[TPC_NSLMAX] = inc;
         s_gbase = atomicAdd(blob_cursor, (u64)inc);
       }
     }
@@ -572,14 +585,14 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
         }
       }
     }
-    if (threadIdx.x >= 128u && threadIdx.x < 128u + nsl) {   // zero the padding of every run (K6 skips record 0)
-      const u32 sl = threadIdx.x - 128u;
+    if (threadIdx.x >= TPC_NSLMAX && threadIdx.x < TPC_NSLMAX + nsl) {   // zero the padding of every run (K6 skips record 0)
+      const u32 sl = threadIdx.x - TPC_NSLMAX;
       for (u32 k = s_off[sl] + s_cnt[sl] + s_dcnt[sl]; k < s_off[sl + 1u]; ++k) buf[k] = 0u;
     }
     __syncthreads();
     // ---- dump the sorted batch + its index entries -----------------------------------------
     const u64 gbase = s_gbase;
-    const u32 total = s_off[128];
+    const u32 total = s_off[TPC_NSLMAX];
     uint4* dst = (uint4*)(blob + gbase);       // gbase is a multiple of 8 records (32 B)
     const uint4* src = (const uint4*)buf;
     for (u32 i = threadIdx.x; i < (total >> 2); i += TPC_K5_THREADS) dst[i] = src[i];
@@ -615,6 +628,7 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
 #define TPC_K6_THREADS (TPC_K6_CONSUMERS + 32u)  // + the producer warp
 #define TPC_K6_CAP 4096u                         // records staged per round (16 KB)
 #define TPC_K6_CAPU (TPC_K6_CAP / 4u)            // ... in 16-byte units
+#define TPC_K6_CTAS 3                            // resident CTAs per SM (shared memory and registers)
 
 struct K6Args {
   const u32* blob; const u64* idx; const u32* batch_start;
@@ -655,12 +669,12 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, u32 bytes, 
                ::"r"(smem_addr(dst)), "l"(src), "r"(bytes), "r"(smem_addr(bar)) : "memory");
 }
 __device__ __forceinline__ u32 vmax2(u32 a, u32 b) { u32 d; asm("max.u16x2 %0, %1, %2;" : "=r"(d) : "r"(a), "r"(b)); return d; }
-// barrier 1 = the 256 consumer threads only (the producer warp never joins it)
-__device__ __forceinline__ void csync() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
+// barrier 1 = the consumer threads only (the producer warp never joins it)
+__device__ __forceinline__ void csync() { asm volatile("bar.sync 1, %0;" ::"n"(TPC_K6_CONSUMERS) : "memory"); }
 __device__ __forceinline__ u32 csync_or(u32 v) {
   u32 r;
-  asm volatile("{\n.reg .pred p, q;\nsetp.ne.u32 p, %1, 0;\nbar.red.or.pred q, 1, 256, p;\nselp.u32 %0, 1, 0, q;\n}"
-               : "=r"(r) : "r"(v) : "memory");
+  asm volatile("{\n.reg .pred p, q;\nsetp.ne.u32 p, %1, 0;\nbar.red.or.pred q, 1, %2, p;\nselp.u32 %0, 1, 0, q;\n}"
+               : "=r"(r) : "r"(v), "n"(TPC_K6_CONSUMERS) : "memory");
   return r;
 }
 
@@ -754,6 +768,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
 
   // ---- consumers -------------------------------------------------------------------------------
   u32 ph = 0u;
+  bool bad = false;
   for (u32 tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
     const u32 b = tile / nsl, sl = tile - b * nsl;
     mbar_wait(&s.bar[0], ph); ph ^= 1u;
@@ -764,6 +779,10 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       if (MODE == TPC_MODE_DET_COUNT && tid == 0) a.tile_cnt[tile] = 0u;
       continue;
     }
+    const u32 tc = b % PRM(n_tc), sr = b / PRM(n_tc);
+    const u32 row = sr % PRM(n_rows), sector = sr / PRM(n_rows);
+    const u32 npads = PRM_NPADS(row);
+    const int t_base = (int)(tc * TPC_TC + sl * TPC_TS) - (int)TPC_HALO;   // time of tile row 0
     // ---- O0: zero the map, scatter the tile's records -------------------------------------
     csync();   // every consumer is done with the previous tile's map
     {
@@ -782,8 +801,11 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
         const u32 rr[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
         for (int k = 0; k < 4; ++k)
-          if (rr[k] != 0u)   // 0 = run padding (every real record has q >= 1)
-            s.tile[((rr[k] >> 8) & 0xFFu) * pitch + (rr[k] & 0xFFu) + TPC_HALO] = (u16)((rr[k] >> 16) & 0x3FFu);
+          if (rr[k] != 0u) {   // 0 = run padding (every real record has q >= 1)
+            const u32 pad = rr[k] & 0xFFu;
+            if (pad < npads) s.tile[((rr[k] >> 8) & 0xFFu) * pitch + pad + TPC_HALO] = (u16)((rr[k] >> 16) & 0x3FFu);
+            else bad = true;   // O0 / Q4: pad out of range for this row -> ignored + flagged
+          }
       }
       if (MODE != TPC_MODE_FAST) {
         // Q5, deterministic: two digits on one cell -> the maximum, whatever the order.  Re-check
@@ -796,7 +818,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
             const u32 rr[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
             for (int k = 0; k < 4; ++k)
-              if (rr[k] != 0u) {
+              if (rr[k] != 0u && (rr[k] & 0xFFu) < npads) {
                 const u32 cell = ((rr[k] >> 8) & 0xFFu) * pitch + (rr[k] & 0xFFu) + TPC_HALO;
                 const u16 q = (u16)((rr[k] >> 16) & 0x3FFu);
                 if (s.tile[cell] < q) { s.tile[cell] = q; any = 1u; }
@@ -813,10 +835,6 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
     }
     csync();
 
-    const u32 tc = b % PRM(n_tc), sr = b / PRM(n_tc);
-    const u32 row = sr % PRM(n_rows), sector = sr / PRM(n_rows);
-    const u32 npads = PRM_NPADS(row);
-    const int t_base = (int)(tc * TPC_TC + sl * TPC_TS) - (int)TPC_HALO;   // time of tile row 0
 
     if (MODE == TPC_MODE_DUMP_MAP) {
       const u64 sector_cells = a.row_off[PRM(n_rows)];
@@ -1004,21 +1022,22 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       }
     }
   }
+  if (bad) atomicOr(a.status, TPC_STATUS_BAD_DIGITS);
 }
 
-extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, 3) k_cluster_tiles_fast(K6Args a) {
+extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, TPC_K6_CTAS) k_cluster_tiles_fast(K6Args a) {
   extern __shared__ __align__(128) u32 smem_u32[];
   k6_body<TPC_MODE_FAST>(a, smem_u32);
 }
-extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, 3) k_cluster_tiles_det_count(K6Args a) {
+extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, TPC_K6_CTAS) k_cluster_tiles_det_count(K6Args a) {
   extern __shared__ __align__(128) u32 smem_u32[];
   k6_body<TPC_MODE_DET_COUNT>(a, smem_u32);
 }
-extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, 3) k_cluster_tiles_det_emit(K6Args a) {
+extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, TPC_K6_CTAS) k_cluster_tiles_det_emit(K6Args a) {
   extern __shared__ __align__(128) u32 smem_u32[];
   k6_body<TPC_MODE_DET_EMIT>(a, smem_u32);
 }
-extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, 3) k_cluster_tiles_dump_map(K6Args a) {
+extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, TPC_K6_CTAS) k_cluster_tiles_dump_map(K6Args a) {
   extern __shared__ __align__(128) u32 smem_u32[];
   k6_body<TPC_MODE_DUMP_MAP>(a, smem_u32);
 }
