@@ -53,7 +53,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
             return LIB
     _embed_source()
     tmp = LIB + ".tmp%d" % os.getpid()
-    cmd = [_nvcc(), *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", tmp,
+    cmd = [_nvcc(), *NVCC_FLAGS, *os.environ.get("TPC_EXTRA", "").split(), *(["-Xptxas", "-v"] if verbose else []), "-o", tmp,
            os.path.join(CSRC, "tpcclus.cu"), GEN, "-ldl"]
     subprocess.check_call(cmd)
     os.replace(tmp, LIB)

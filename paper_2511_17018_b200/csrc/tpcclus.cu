@@ -456,7 +456,7 @@ int enqueue_binning(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n
     if ((rc = launch(h, K_DIR_SCAN, dim3(1), dim3(TPC_SCAN_THREADS), 0, st, a))) return rc; }
   { void* a[] = {&p.dir, &p.used, &slice_cap, &p.bin_chunk_start, &p.bin_fill, &p.chunk_list};
     if ((rc = launch(h, K_DIR_FILL, dim3(gx, g.g1), dim3(256), 0, st, a))) return rc; }
-  { void* a[] = {&p.pool, &p.dir, &p.chunk_list, &p.bin_chunk_start, &p.batch_start, &p.batch_bin, &p.blob, &p.blob_cursor, &p.idx};
+  { void* a[] = {&p.pool, &p.dir, &p.chunk_list, &p.bin_chunk_start, &p.batch_start, &p.batch_bin, &p.blob, &p.blob_cursor, &p.idx, &status};
     if ((rc = launch(h, K_PART_FINE, dim3(h->grid_k5), dim3(TPC_K5_THREADS), h->smem_k5, st, a))) return rc; }
   return TPCCLUS_OK;
 }

@@ -494,7 +494,7 @@ extern "C" __global__ void __launch_bounds__(TPC_K5_THREADS, 2)
 k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, const u32* __restrict__ chunk_list,
                  const u32* __restrict__ bin_chunk_start, const u32* __restrict__ batch_start,
                  const u32* __restrict__ batch_bin, u32* __restrict__ blob, u64* __restrict__ blob_cursor,
-                 u64* __restrict__ idx) {
+                 u64* __restrict__ idx, u32* __restrict__ status) {
   extern __shared__ __align__(128) u32 smem_u32[];
   u32* buf = smem_u32;                       // [TPC_K5_BUF]
   u32* s_cnt = buf + TPC_K5_BUF;             // [NSLMAX] primaries per slab
@@ -504,9 +504,11 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
   __shared__ u64 s_gbase;
   const u32 nb = PRM(n_bins), nsl = PRM(n_sl);
   const u32 n_batches = batch_start[nb];
+  bool bad = false;
 
   for (u32 batch = blockIdx.x; batch < n_batches; batch += gridDim.x) {
     const u32 b = batch_bin[batch];
+    const u32 npads = PRM_NPADS((b / PRM(n_tc)) % PRM(n_rows));   // one bin = one pad row
     if (threadIdx.x < TPC_NSLMAX) { s_cnt[threadIdx.x] = 0u; s_dcnt[threadIdx.x] = 0u; s_dcur[threadIdx.x] = 0u; }
     __syncthreads();
     const u32 kb = batch - batch_start[b];
@@ -536,6 +538,7 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
         u32 r = r4[j];   // q >= 1 in every valid record, so 0 = none
+        if ((r & 0xFFu) >= npads && r != 0u) { r = 0u; bad = true; }   // O0 / Q4: pad out of range -> ignored + flagged
         u32 rk = 0u;
         if (r != 0u) {
           u32 u = (r >> 8) & 0x3FFFu;
@@ -603,6 +606,7 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
     }
     __syncthreads();
   }
+  if (bad) atomicOr(status, TPC_STATUS_BAD_DIGITS);
 }
 
 // ==========================================================================================
@@ -683,11 +687,14 @@ struct K6Smem {
   u16* tile; u32* tile32;
   u64* bar;        // [0] full (producer -> consumers), [1] empty (consumers -> producer)
   u64* base;
-  u32* rowmask; u32* rowpre; u32* misc; u16* peaks;
+  u32* pmask;      // [TT][9]  O1 peaks, bit = pad + 2 (so pad - 2 of a 5x5 ring is bit >= 0)
+  u32* rowmask;    // [TT][8]  O2 survivors, bit = pad
+  u32* rowpre; u32* misc; u16* peaks;
 };
-// misc: [0] n_peaks  [1] survivors  [2] total 16-byte units of the tile being staged
+// misc: [0] n_peaks  [2] total 16-byte units of the tile being staged
+#define TPC_K6_PMW 9u
 __host__ __device__ inline u32 tpc_k6_smem_bytes(u32 pitch, u32 max_peaks) {
-  return (TPC_K6_CAP + TPC_TT * pitch / 2u + 4u + 2u + TPC_TT * 8u + TPC_TT + 2u + 8u + (max_peaks + 1u) / 2u) * 4u + 128u;
+  return (TPC_K6_CAP + TPC_TT * pitch / 2u + 4u + 2u + TPC_TT * (8u + TPC_K6_PMW) + TPC_TT + 2u + 8u + (max_peaks + 1u) / 2u) * 4u + 128u;
 }
 __device__ __forceinline__ K6Smem k6_smem(u32* p) {
   K6Smem s;
@@ -695,6 +702,7 @@ __device__ __forceinline__ K6Smem k6_smem(u32* p) {
   s.tile32 = p; s.tile = (u16*)p; p += TPC_TT * PRM(pitch) / 2u;
   s.bar = (u64*)p; p += 4;
   s.base = (u64*)p; p += 2;
+  s.pmask = p; p += TPC_TT * TPC_K6_PMW;   // pmask and rowmask are contiguous: zeroed together
   s.rowmask = p; p += TPC_TT * 8u;
   s.rowpre = p; p += TPC_TT + 2u;
   s.misc = p; p += 8;
@@ -767,13 +775,22 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
   }
 
   // ---- consumers -------------------------------------------------------------------------------
+  // Per tile, five block barriers (A..G below).  The map, pmask and rowmask are zeroed at the
+  // tail of the previous tile, so barrier A doubles as "zeroing done".
   u32 ph = 0u;
-  bool bad = false;
+  const u32 zero_words = tile_words / 4u;
+  auto zero_tile = [&]() {
+    uint4* z = (uint4*)s.tile32;
+    for (u32 i = tid; i < zero_words; i += TPC_K6_CONSUMERS) z[i] = make_uint4(0u, 0u, 0u, 0u);
+    for (u32 i = tid; i < TPC_TT * (8u + TPC_K6_PMW); i += TPC_K6_CONSUMERS) s.pmask[i] = 0u;
+    if (tid == 0) s.misc[0] = 0u;
+  };
+  zero_tile();
   for (u32 tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
     const u32 b = tile / nsl, sl = tile - b * nsl;
     mbar_wait(&s.bar[0], ph); ph ^= 1u;
     const u32 total = s.misc[2];
-    if (total == 0u) {   // block-uniform: nothing in this tile
+    if (total == 0u) {   // block-uniform: nothing in this tile; the map stays zero
       __syncwarp();
       if (lane_id() == 0u) mbar_arrive(&s.bar[1]);
       if (MODE == TPC_MODE_DET_COUNT && tid == 0) a.tile_cnt[tile] = 0u;
@@ -783,15 +800,11 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
     const u32 row = sr % PRM(n_rows), sector = sr / PRM(n_rows);
     const u32 npads = PRM_NPADS(row);
     const int t_base = (int)(tc * TPC_TC + sl * TPC_TS) - (int)TPC_HALO;   // time of tile row 0
-    // ---- O0: zero the map, scatter the tile's records -------------------------------------
-    csync();   // every consumer is done with the previous tile's map
-    {
-      uint4* z = (uint4*)s.tile32;
-      for (u32 i = tid; i < tile_words / 4u; i += TPC_K6_CONSUMERS) z[i] = make_uint4(0u, 0u, 0u, 0u);
-      for (u32 i = tid; i < TPC_TT * 8u; i += TPC_K6_CONSUMERS) s.rowmask[i] = 0u;
-      if (tid < 2) s.misc[tid] = 0u;
-    }
-    csync();
+#if defined(TPC_ABL) && TPC_ABL == 9
+    { for (u32 round = 0u;;) { __syncwarp(); if (lane_id() == 0u) mbar_arrive(&s.bar[1]); ++round; if (round * TPC_K6_CAPU >= total) break; mbar_wait(&s.bar[0], ph); ph ^= 1u; } continue; }
+#endif
+    csync();   // A: the previous tile is done with the map, and the map is zero
+    // ---- O0: scatter the tile's records ------------------------------------------------------
     for (u32 round = 0u;;) {
       u32 nu = total - round * TPC_K6_CAPU;
       if (nu > TPC_K6_CAPU) nu = TPC_K6_CAPU;
@@ -801,11 +814,8 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
         const u32 rr[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
         for (int k = 0; k < 4; ++k)
-          if (rr[k] != 0u) {   // 0 = run padding (every real record has q >= 1)
-            const u32 pad = rr[k] & 0xFFu;
-            if (pad < npads) s.tile[((rr[k] >> 8) & 0xFFu) * pitch + pad + TPC_HALO] = (u16)((rr[k] >> 16) & 0x3FFu);
-            else bad = true;   // O0 / Q4: pad out of range for this row -> ignored + flagged
-          }
+          if (rr[k] != 0u)   // 0 = run padding (every real record has q >= 1)
+            s.tile[((rr[k] >> 8) & 0xFFu) * pitch + (rr[k] & 0xFFu) + TPC_HALO] = (u16)((rr[k] >> 16) & 0x3FFu);
       }
       if (MODE != TPC_MODE_FAST) {
         // Q5, deterministic: two digits on one cell -> the maximum, whatever the order.  Re-check
@@ -818,7 +828,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
             const u32 rr[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
             for (int k = 0; k < 4; ++k)
-              if (rr[k] != 0u && (rr[k] & 0xFFu) < npads) {
+              if (rr[k] != 0u) {
                 const u32 cell = ((rr[k] >> 8) & 0xFFu) * pitch + (rr[k] & 0xFFu) + TPC_HALO;
                 const u16 q = (u16)((rr[k] >> 16) & 0x3FFu);
                 if (s.tile[cell] < q) { s.tile[cell] = q; any = 1u; }
@@ -827,14 +837,19 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
           if (!csync_or(any)) break;
         }
       }
-      __syncwarp();
-      if (lane_id() == 0u) mbar_arrive(&s.bar[1]);   // this warp is done with the staged records
       ++round;
       if (round * TPC_K6_CAPU >= total) break;
+      __syncwarp();
+      if (lane_id() == 0u) mbar_arrive(&s.bar[1]);   // this warp is done with the staged records
       mbar_wait(&s.bar[0], ph); ph ^= 1u;
     }
-    csync();
-
+    // a tile staged in one round (the usual case) keeps its records for the peak test below
+    const bool sparse = total <= TPC_K6_CAPU && MODE != TPC_MODE_DUMP_MAP;
+    if (!sparse) { __syncwarp(); if (lane_id() == 0u) mbar_arrive(&s.bar[1]); }
+    csync();   // C: the map is complete
+#if defined(TPC_ABL) && TPC_ABL == 1
+    zero_tile(); continue;
+#endif
 
     if (MODE == TPC_MODE_DUMP_MAP) {
       const u64 sector_cells = a.row_off[PRM(n_rows)];
@@ -844,9 +859,51 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
         if (t < (int)PRM(n_time))
           a.dmap[(u64)sector * sector_cells + a.row_off[row] + (u64)t * npads + p] = s.tile[tl * pitch + p + TPC_HALO];
       }
+      csync();
+      zero_tile();
       continue;
     }
 
+    // ---- O1: 3x3 peaks, record-driven (the tile's records are still staged) -----------------
+    // Every record with q >= thr_peak in rows 1..TT-2 tests its own cell: the two words holding
+    // (x-1, x, x+1) of the rows above, at and below are loaded and aligned with a funnel shift;
+    // q > the 4 neighbours earlier in (t,p) order and q >= the 4 later ones (O1).  Cost follows
+    // the occupancy, not the tile area; a tile that needed several staging rounds takes the
+    // dense scan below instead.  A peak sets its bit in pmask (which also removes duplicates of
+    // one cell); the peaks of owned rows go into the list the later phases walk.
+    if (sparse) {
+      const u32 nW = pitch >> 1;
+      const uint4* r4 = (const uint4*)s.rec;
+      for (u32 u = tid; u < total; u += TPC_K6_CONSUMERS) {
+        const uint4 v = r4[u];
+        const u32 rr[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          const u32 q = (rr[k] >> 16) & 0x3FFu, tl = (rr[k] >> 8) & 0xFFu, pad = rr[k] & 0xFFu;
+          if (q < thr || tl - 1u >= TPC_TT - 2u) continue;   // (q = 0 for run padding)
+          const u32 x = pad + TPC_HALO, h = x & 1u, sh = 16u - 16u * h;
+          const u32* w = s.tile32 + (tl - 1u) * nW + (x >> 1) - 1u + h;
+          const u32 pu = __funnelshift_r(w[0], w[1], sh), nu = (w[1] >> sh) & 0xFFFFu;
+          w += nW;
+          const u32 pm = __funnelshift_r(w[0], w[1], sh), nm = (w[1] >> sh) & 0xFFFFu;
+          w += nW;
+          const u32 pd = __funnelshift_r(w[0], w[1], sh), nd = (w[1] >> sh) & 0xFFFFu;
+          if ((pm >> 16) != q) continue;   // a smaller duplicate of this cell
+          const u32 e = max(max(pu & 0xFFFFu, pu >> 16), max(nu, pm & 0xFFFFu));
+          const u32 l = max(max(pd & 0xFFFFu, pd >> 16), max(nd, nm));
+          if (q > e && q >= l) {
+            const u32 bit = 1u << ((pad + 2u) & 31u);
+            const u32 old = atomicOr(&s.pmask[tl * TPC_K6_PMW + ((pad + 2u) >> 5)], bit);
+            if (!(old & bit) && tl >= TPC_HALO && tl < TPC_TS + TPC_HALO) {   // a halo-row peak is emitted by its own tile
+              const u32 i = atomicAdd(&s.misc[0], 1u);
+              s.peaks[i] = (u16)((tl << 8) | pad);
+            }
+          }
+        }
+      }
+      __syncwarp();
+      if (lane_id() == 0u) mbar_arrive(&s.bar[1]);   // this warp is done with the staged records
+    } else
     // ---- O1: 3x3 peaks, dense scan on packed u16x2 words ----------------------------------
     // A thread owns a group of 4 word columns (8 pads, one 128-bit load per row) of a strip of
     // rows and walks down the time axis with a rolling 3-row window.  For the word C of row r:
@@ -854,7 +911,8 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
     // peak iff q > the 4 neighbours earlier in (t,p) order and q >= the 4 later ones (O1), i.e.
     // q >= max(max(H(r-1), L(r)) + 1, H(r+1), R(r)); an empty cell never passes (the bound is
     // >= 1) and thr_peak joins the same max.  Rows 1..TT-2 are tested: the owned rows plus the
-    // halo rows whose peak flags O2 needs.  Guard cells are 0 and can never be flagged.
+    // halo rows whose peaks O2 needs.  Guard cells are 0 and can never be flagged.  A peak sets
+    // its bit in pmask; the peaks of owned rows also go into the list the later phases walk.
     {
       const u32 nW = pitch >> 1;
       const u32 ng = (((npads + 2u) >> 1) >> 2) + 1u;    // word groups covering cells 0..npads+2
@@ -892,8 +950,12 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
 #pragma unroll
               for (int h = 0; h < 2; ++h)
                 if (((X[k] >> (16 * h)) & 0xFFFFu) == 0u) {
-                  const u32 i = atomicAdd(&s.misc[0], 1u);
-                  s.peaks[i] = (u16)((r << 8) | (8u * g + 2u * (u32)k + (u32)h - TPC_HALO));
+                  const u32 pad = 8u * g + 2u * (u32)k + (u32)h - TPC_HALO;
+                  atomicOr(&s.pmask[r * TPC_K6_PMW + ((pad + 2u) >> 5)], 1u << ((pad + 2u) & 31u));
+                  if (r >= TPC_HALO && r < TPC_TS + TPC_HALO) {   // a halo-row peak is emitted by its own tile
+                    const u32 i = atomicAdd(&s.misc[0], 1u);
+                    s.peaks[i] = (u16)((r << 8) | pad);
+                  }
                 }
           }
         };
@@ -908,55 +970,71 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
         }
       }
     }
-    csync();
+    csync();   // D: peak set complete
     const u32 npk = s.misc[0];
-    for (u32 i = tid; i < npk; i += TPC_K6_CONSUMERS) {   // bit 15 of a cell = peak flag (distinct cells: plain stores)
-      const u32 e = s.peaks[i];
-      s.tile[(e >> 8) * pitch + (e & 0xFFu) + TPC_HALO] |= (u16)0x8000u;
-    }
-    csync();
+#if defined(TPC_ABL) && TPC_ABL == 2
+    zero_tile(); continue;
+#endif
 
     // ---- O2: suppression of the owned peaks against the un-updated peak set -----------------
     for (u32 i = tid; i < npk; i += TPC_K6_CONSUMERS) {
       const u32 e = s.peaks[i];
       const u32 tl = e >> 8, pad = e & 0xFFu;
-      if (tl < TPC_HALO || tl >= TPC_TS + TPC_HALO) continue;   // a halo row: its own tile emits it
-      const u16* c = s.tile + tl * pitch + pad + TPC_HALO;
-      const u32 qc = c[0] & 0x3FFu;
-      u32 nq[3][3];
+      // the 5x5 ring of peak bits around (tl, pad): 5 bits per row, bit k <-> dp = k - 2
+      const u32 w0 = pad >> 5, sh = pad & 31u;   // bit (pad + 2) - 2 = pad
+      u32 ring = 0u;
 #pragma unroll
-      for (int dt = -1; dt <= 1; ++dt)
-#pragma unroll
-        for (int dp = -1; dp <= 1; ++dp) nq[dt + 1][dp + 1] = c[dt * (int)pitch + dp] & 0x3FFu;
+      for (int dt = -2; dt <= 2; ++dt) {
+        const u32* pm = s.pmask + (tl + dt) * TPC_K6_PMW + w0;
+        const u32 win = __funnelshift_r(pm[0], pm[1], sh) & ((dt == -2 || dt == 2) ? 0x1Fu : 0x11u);
+        ring |= win << (5 * (dt + 2));
+      }
       bool dead = false;
+      if (ring) {   // some peak at Chebyshev distance exactly 2
+        const u16* c = s.tile + tl * pitch + pad + TPC_HALO;
+        const u32 qc = c[0];
+        u32 nq[3][3];
 #pragma unroll
-      for (int dt = -2; dt <= 2; ++dt)
+        for (int dt = -1; dt <= 1; ++dt)
 #pragma unroll
-        for (int dp = -2; dp <= 2; ++dp) {
-          if (dt != -2 && dt != 2 && dp != -2 && dp != 2) continue;
-          const u32 v = c[dt * (int)pitch + dp];
-          if (!(v & 0x8000u)) continue;
-          const u32 q2 = v & 0x3FFu;
-          const bool beats = q2 > qc || (q2 == qc && (dt < 0 || (dt == 0 && dp < 0)));   // P:36 total order
-          if (!beats) continue;
+          for (int dp = -1; dp <= 1; ++dp) nq[dt + 1][dp + 1] = c[dt * (int)pitch + dp];
 #pragma unroll
-          for (int mt = -1; mt <= 1; ++mt)
+        for (int dt = -2; dt <= 2; ++dt)
 #pragma unroll
-            for (int mp = -1; mp <= 1; ++mp) {
-              if (mt == 0 && mp == 0) continue;
-              if (mt - dt > 1 || dt - mt > 1 || mp - dp > 1 || dp - mp > 1) continue;
-              if (nq[mt + 1][mp + 1] + eps >= qc) dead = true;
-            }
-        }
+          for (int dp = -2; dp <= 2; ++dp) {
+            if (dt != -2 && dt != 2 && dp != -2 && dp != 2) continue;
+            if (!((ring >> (5 * (dt + 2) + dp + 2)) & 1u)) continue;
+            const u32 q2 = c[dt * (int)pitch + dp];
+            const bool beats = q2 > qc || (q2 == qc && (dt < 0 || (dt == 0 && dp < 0)));   // P:36 total order
+            if (!beats) continue;
+#pragma unroll
+            for (int mt = -1; mt <= 1; ++mt)
+#pragma unroll
+              for (int mp = -1; mp <= 1; ++mp) {
+                if (mt == 0 && mp == 0) continue;
+                if (mt - dt > 1 || dt - mt > 1 || mp - dp > 1 || dp - mp > 1) continue;
+                if (nq[mt + 1][mp + 1] + eps >= qc) dead = true;
+              }
+          }
+      }
       if (!dead) atomicOr(&s.rowmask[tl * 8u + (pad >> 5)], 1u << (pad & 31u));
     }
-    csync();
-    // ---- rank rows: rowpre[tl] = survivors in rows < tl --------------------------------------
-    if (tid < 32) {
+    csync();   // F: survivor set complete
+#if defined(TPC_ABL) && TPC_ABL == 3
+    zero_tile(); continue;
+#endif
+
+    // ---- rank (last warp) || O3 + O4 (everyone else first) ------------------------------------
+    // rowpre[tl] = survivors in rows < tl, which ranks every cluster in (time, pad) order inside
+    // the tile without a sort.  The last warp computes it and fetches the tile's base (FAST: one
+    // atomic; DET: the scanned count) while the other warps already do the 5x5 arithmetic; the
+    // results meet at barrier G.
+    if (tid >= TPC_K6_CONSUMERS - 32u) {
+      const u32 lane = lane_id();
       u32 cnt[5], t = 0u;
 #pragma unroll
       for (int k = 0; k < 5; ++k) {
-        const u32 tl = tid * 5u + (u32)k;
+        const u32 tl = lane * 5u + (u32)k;
         u32 n = 0u;
         if (tl < TPC_TT) {
 #pragma unroll
@@ -966,30 +1044,26 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       }
       u32 inc = t;
 #pragma unroll
-      for (int d = 1; d < 32; d <<= 1) { u32 o = __shfl_up_sync(0xFFFFFFFFu, inc, d); if ((int)tid >= d) inc += o; }
+      for (int d = 1; d < 32; d <<= 1) { u32 o = __shfl_up_sync(0xFFFFFFFFu, inc, d); if ((int)lane >= d) inc += o; }
       u32 ex = inc - t;
 #pragma unroll
-      for (int k = 0; k < 5; ++k) { const u32 tl = tid * 5u + (u32)k; if (tl < TPC_TT) s.rowpre[tl] = ex; ex += cnt[k]; }
-      if (tid == 31) {
-        s.misc[1] = inc;
+      for (int k = 0; k < 5; ++k) { const u32 tl = lane * 5u + (u32)k; if (tl < TPC_TT) s.rowpre[tl] = ex; ex += cnt[k]; }
+      if (lane == 31u) {
         if (MODE == TPC_MODE_DET_COUNT) a.tile_cnt[tile] = inc;
         if (MODE == TPC_MODE_FAST) s.base[0] = atomicAdd(a.n_clusters, (u64)inc);
         if (MODE == TPC_MODE_DET_EMIT) s.base[0] = a.block_prefix[tile / TPC_SCAN_PER_CTA] + a.tile_local[tile];
       }
     }
-    if (MODE == TPC_MODE_DET_COUNT) continue;
-    csync();
-    const u64 base = s.base[0];
-
-    // ---- O3 + O4 + O5: 5x5 sums, float32 finalisation (every op rounded once, no FMA), emit --
-    for (u32 i = tid; i < npk; i += TPC_K6_CONSUMERS) {
-      const u32 e = s.peaks[i];
+    // one cluster per thread held in registers across barrier G (further ones, npk > threads, after it)
+    uint4 o0 = make_uint4(0u, 0u, 0u, 0u), o1 = make_uint4(0u, 0u, 0u, 0u);
+    u32 inrow = 0xFFFFFFFFu, my_tl = 0u;
+    auto cog = [&](u32 e, uint4& c0, uint4& c1, u32& rk) -> bool {
       const u32 tl = e >> 8, pad = e & 0xFFu;
       const u32 w = pad >> 5, bitpos = pad & 31u;
       const u32 mword = s.rowmask[tl * 8u + w];
-      if (!((mword >> bitpos) & 1u)) continue;   // suppressed, or a halo-row peak (never marked)
-      u32 rank = s.rowpre[tl] + __popc(mword & ((1u << bitpos) - 1u));
-      for (u32 k = 0; k < w; ++k) rank += __popc(s.rowmask[tl * 8u + k]);
+      if (!((mword >> bitpos) & 1u)) return false;   // suppressed
+      rk = __popc(mword & ((1u << bitpos) - 1u));
+      for (u32 k = 0; k < w; ++k) rk += __popc(s.rowmask[tl * 8u + k]);
       const u16* c = s.tile + tl * pitch + pad + TPC_HALO;
       u32 Q = 0u, Spp = 0u, Stt = 0u;
       int Sp = 0, St = 0;
@@ -997,12 +1071,12 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       for (int dt = -2; dt <= 2; ++dt)
 #pragma unroll
         for (int dp = -2; dp <= 2; ++dp) {
-          const u32 q = c[dt * (int)pitch + dp] & 0x3FFu;
+          const u32 q = c[dt * (int)pitch + dp];
           Q += q; Sp += (int)q * dp; St += (int)q * dt;
           Spp += q * (u32)(dp * dp); Stt += q * (u32)(dt * dt);
         }
       const int Vp = (int)(Q * Spp) - Sp * Sp, Vt = (int)(Q * Stt) - St * St;
-      const u32 qc = c[0] & 0x3FFu;
+      const u32 qc = c[0];
       const int t = t_base + (int)tl;
       const float fQ = __uint2float_rn(Q);
       const float pm = __fadd_rn(__uint2float_rn(pad), __fdiv_rn(__int2float_rn(Sp), fQ));
@@ -1013,16 +1087,33 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       if (pad < 2u || pad + 2u >= npads) fl |= 1u;
       if (t < 2 || (u32)t + 2u >= PRM(n_time)) fl |= 2u;
       if (qc == 1023u) fl |= 4u;
-      const u64 slot = base + rank;
-      if (slot < a.capacity) {
-        a.out[slot * 2u] = make_uint4(__float_as_uint(pm), __float_as_uint(tm), __float_as_uint(sp), __float_as_uint(st));
-        a.out[slot * 2u + 1u] = make_uint4(Q, qc | ((u32)t << 16), pad | (row << 8) | (sector << 16) | (fl << 24), 0u);
-      } else {
-        atomicOr(a.status, TPC_STATUS_OVERFLOW);
-      }
+      c0 = make_uint4(__float_as_uint(pm), __float_as_uint(tm), __float_as_uint(sp), __float_as_uint(st));
+      c1 = make_uint4(Q, qc | ((u32)t << 16), pad | (row << 8) | (sector << 16) | (fl << 24), 0u);
+      return true;
+    };
+    auto emit = [&](u64 slot, const uint4& c0, const uint4& c1) {
+      if (slot < a.capacity) { a.out[slot * 2u] = c0; a.out[slot * 2u + 1u] = c1; }
+      else atomicOr(a.status, TPC_STATUS_OVERFLOW);
+    };
+    if (MODE != TPC_MODE_DET_COUNT && tid < npk) {
+      const u32 e = s.peaks[tid];
+      my_tl = e >> 8;
+      u32 rk;
+      if (cog(e, o0, o1, rk)) inrow = rk;
     }
+    csync();   // G: rowpre and base are there; nobody reads the map of this tile's first 256 peaks any more
+    if (MODE != TPC_MODE_DET_COUNT) {
+      const u64 base = s.base[0];
+      if (inrow != 0xFFFFFFFFu) emit(base + s.rowpre[my_tl] + inrow, o0, o1);
+      for (u32 i = tid + TPC_K6_CONSUMERS; i < npk; i += TPC_K6_CONSUMERS) {   // dense tiles only
+        const u32 e = s.peaks[i];
+        u32 rk;
+        if (cog(e, o0, o1, rk)) emit(base + s.rowpre[e >> 8] + rk, o0, o1);
+      }
+      if (npk > TPC_K6_CONSUMERS) csync();   // block-uniform: the extra clusters still read the map
+    }
+    zero_tile();   // for the next tile (barrier A orders it before the scatter)
   }
-  if (bad) atomicOr(a.status, TPC_STATUS_BAD_DIGITS);
 }
 
 extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, TPC_K6_CTAS) k_cluster_tiles_fast(K6Args a) {
