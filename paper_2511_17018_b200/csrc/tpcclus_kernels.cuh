@@ -713,13 +713,13 @@ __device__ __forceinline__ K6Smem k6_smem(u32* p) {
 // Producer warp: stages round `round` of a tile -- the 16-byte units [round*CAPU, (round+1)*CAPU)
 // of the concatenation of the tile's runs (one run per K5 batch of the bin, 32-byte aligned and
 // zero-padded by K5) -- and arrives on the full barrier.  Returns the tile's total units.
-__device__ __forceinline__ u32 k6_stage(const K6Smem& s, const K6Args& a, u64 ib, u32 nbatch, u32 round) {
+__device__ __forceinline__ u32 k6_stage(const K6Smem& s, const K6Args& a, u64 ib, u32 nbatch, u32 round, u64 e0) {
   const u32 lane = lane_id();
   const u32 lo = round * TPC_K6_CAPU, hi = lo + TPC_K6_CAPU;
   u32 pos = 0u;
   for (u32 g0 = 0u; g0 < nbatch; g0 += 32u) {
     const u32 g = g0 + lane;
-    u64 e = g < nbatch ? a.idx[ib + g] : 0ull;
+    u64 e = g0 == 0u ? e0 : (g < nbatch ? a.idx[ib + g] : 0ull);   // e0: the first 32 entries, loaded ahead
     const u32 units = ((u32)(e >> 40) + 3u) >> 2;
     const u64 src = e & ((1ull << 40) - 1ull);
     u32 inc = units;
@@ -758,18 +758,34 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
 
   if (tid >= TPC_K6_CONSUMERS) {
     // ---- producer warp -----------------------------------------------------------------------
+    // While the consumers work on tile k the producer already holds the index entries of tile
+    // k+1 and has asked L2 for its runs, so that once the buffer is released the bulk copies
+    // start at once and hit L2.
     u32 ph = 1u;   // a fresh barrier passes a wait on parity 1: the buffer starts out free
-    for (u32 tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    const u32 lane = lane_id();
+    u64 ib = 0ull, e0 = 0ull;
+    u32 nbatch = 0u;
+    auto look_ahead = [&](u32 tile) {
       const u32 b = tile / nsl, sl = tile - b * nsl;
       const u32 bs0 = a.batch_start[b];
-      const u32 nbatch = a.batch_start[b + 1] - bs0;
-      const u64 ib = (u64)nsl * bs0 + (u64)sl * nbatch;
-      u32 round = 0u, total;
-      do {
+      nbatch = a.batch_start[b + 1] - bs0;
+      ib = (u64)nsl * bs0 + (u64)sl * nbatch;
+      e0 = lane < nbatch ? a.idx[ib + lane] : 0ull;
+      const u32 bytes = (((u32)(e0 >> 40) + 3u) >> 2) * 16u;
+      if (bytes != 0u)
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(a.blob + (e0 & ((1ull << 40) - 1ull))), "r"(bytes) : "memory");
+    };
+    if (blockIdx.x < n_tiles) look_ahead(blockIdx.x);
+    for (u32 tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+      const u64 ib_c = ib, e0_c = e0;
+      const u32 nbatch_c = nbatch;
+      mbar_wait_backoff(&s.bar[1], ph); ph ^= 1u;
+      const u32 total = k6_stage(s, a, ib_c, nbatch_c, 0u, e0_c);
+      if (tile + gridDim.x < n_tiles) look_ahead(tile + gridDim.x);
+      for (u32 round = 1u; round * TPC_K6_CAPU < total; ++round) {
         mbar_wait_backoff(&s.bar[1], ph); ph ^= 1u;
-        total = k6_stage(s, a, ib, nbatch, round);
-        ++round;
-      } while (round * TPC_K6_CAPU < total);
+        k6_stage(s, a, ib_c, nbatch_c, round, e0_c);
+      }
     }
     return;
   }
