@@ -32,7 +32,7 @@ inline uint64_t align_up(uint64_t x, uint64_t a) { return (x + a - 1) / a * a; }
 
 struct Layout {   // byte offsets into the workspace
   uint64_t counters, counters_bytes;   // zeroed at the head of every run
-  uint64_t status, blob_cursor, bin_nchunks, bin_fill;
+  uint64_t status, blob_cursor, slice_cnt;
   uint64_t used, bin_chunk_start, batch_start, batch_bin, dir, chunk_list, pool, blob, idx;
   uint64_t tile_cnt, tile_local, block_sum, block_prefix, row_off;
   uint64_t total;        // device-path workspace
@@ -109,9 +109,8 @@ int make_geometry(const tpcclus_params* p, Geometry* g) {
   L.counters = o;
   L.status = take(4);
   L.blob_cursor = take(8);
-  L.bin_nchunks = take(4ull * nb);
-  L.bin_fill = take(4ull * nb);
   L.counters_bytes = o - L.counters;
+  L.slice_cnt = take(4ull * nb * g->g1);
   L.used = take(4ull * g->g1);
   L.bin_chunk_start = take(4ull * (nb + 1));
   L.batch_start = take(4ull * (nb + 1));
@@ -413,7 +412,7 @@ double tpcclus_rtc_build_ms(const tpcclus_handle* h) { return h ? h->rtc_ms : 0.
 namespace {
 
 struct RunPtrs {
-  u32 *status, *bin_nchunks, *bin_fill, *used, *bin_chunk_start, *batch_start, *batch_bin, *dir, *chunk_list, *blob;
+  u32 *status, *slice_cnt, *used, *bin_chunk_start, *batch_start, *batch_bin, *dir, *chunk_list, *blob;
   u32 *tile_cnt, *tile_local, *block_sum;
   u64 *blob_cursor, *idx, *block_prefix, *row_off;
   uint4* pool;
@@ -423,7 +422,7 @@ RunPtrs ptrs(tpcclus_handle* h) {
   char* w = h->ws;
   RunPtrs p;
   p.status = (u32*)(w + L.status); p.blob_cursor = (u64*)(w + L.blob_cursor);
-  p.bin_nchunks = (u32*)(w + L.bin_nchunks); p.bin_fill = (u32*)(w + L.bin_fill); p.used = (u32*)(w + L.used);
+  p.slice_cnt = (u32*)(w + L.slice_cnt); p.used = (u32*)(w + L.used);
   p.bin_chunk_start = (u32*)(w + L.bin_chunk_start); p.batch_start = (u32*)(w + L.batch_start); p.batch_bin = (u32*)(w + L.batch_bin);
   p.dir = (u32*)(w + L.dir); p.chunk_list = (u32*)(w + L.chunk_list); p.pool = (uint4*)(w + L.pool);
   p.blob = (u32*)(w + L.blob); p.idx = (u64*)(w + L.idx);
@@ -449,13 +448,13 @@ int enqueue_binning(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n
   int rc;
   { void* a[] = {&dig, &n64, &per_cta, &p.pool, &p.dir, &p.used, &slice_cap, &status};
     if ((rc = launch(h, K_PART_COARSE, dim3(g.g1), dim3(TPC_K1_THREADS), h->smem_k1, st, a))) return rc; }
-  u32 gx = (slice_cap + 255u) / 256u; if (gx > 32u) gx = 32u;
-  { void* a[] = {&p.dir, &p.used, &slice_cap, &p.bin_nchunks};
-    if ((rc = launch(h, K_DIR_COUNT, dim3(gx, g.g1), dim3(256), 0, st, a))) return rc; }
-  { void* a[] = {&p.bin_nchunks, &p.bin_chunk_start, &p.batch_start, &p.batch_bin};
-    if ((rc = launch(h, K_DIR_SCAN, dim3(1), dim3(TPC_SCAN_THREADS), 0, st, a))) return rc; }
-  { void* a[] = {&p.dir, &p.used, &slice_cap, &p.bin_chunk_start, &p.bin_fill, &p.chunk_list};
-    if ((rc = launch(h, K_DIR_FILL, dim3(gx, g.g1), dim3(256), 0, st, a))) return rc; }
+  u32 n_slices = g.g1, smem_nb = 4u * g.prm.n_bins;
+  { void* a[] = {&p.dir, &p.used, &slice_cap, &p.slice_cnt};
+    if ((rc = launch(h, K_DIR_COUNT, dim3(g.g1), dim3(TPC_SCAN_THREADS), smem_nb, st, a))) return rc; }
+  { void* a[] = {&p.slice_cnt, &n_slices, &p.bin_chunk_start, &p.batch_start, &p.batch_bin};
+    if ((rc = launch(h, K_DIR_SCAN, dim3(1), dim3(TPC_SCAN_THREADS), smem_nb, st, a))) return rc; }
+  { void* a[] = {&p.dir, &p.used, &slice_cap, &p.slice_cnt, &p.chunk_list};
+    if ((rc = launch(h, K_DIR_FILL, dim3(g.g1), dim3(TPC_SCAN_THREADS), smem_nb, st, a))) return rc; }
   { void* a[] = {&p.pool, &p.dir, &p.chunk_list, &p.bin_chunk_start, &p.batch_start, &p.batch_bin, &p.blob, &p.blob_cursor, &p.idx, &status};
     if ((rc = launch(h, K_PART_FINE, dim3(h->grid_k5), dim3(TPC_K5_THREADS), h->smem_k5, st, a))) return rc; }
   return TPCCLUS_OK;

@@ -363,32 +363,48 @@ k_partition_coarse(const uint2* __restrict__ digits, u64 n, u64 per_cta, uint4* 
 
 // ==========================================================================================
 // K2..K4  chunk directory -> per-bin chunk lists (bookkeeping of the scatter; ~2.6e7 chunks
-// at CFG[4], 4 bytes each).  The order of chunks inside a bin is whatever the atomics give:
-// nothing downstream depends on it (the map build is a max, O0/Q5).
+// at CFG[4], 4 bytes each).  One CTA per K1 slice with a shared-memory histogram, so there
+// are no global atomics: K2 counts chunks per (slice, bin), K3 turns the matrix into offsets
+// (slices of one bin follow each other), K4 places the chunk ids.  The order of chunks inside
+// a (slice, bin) group is whatever the shared atomics give: nothing downstream depends on
+// it (the map build is a max, O0/Q5).
 // ==========================================================================================
-extern "C" __global__ void __launch_bounds__(256)
-k_dir_count(const u32* __restrict__ dir, const u32* __restrict__ used, u32 slice_cap, u32* __restrict__ bin_nchunks) {
-  const u32 cta = blockIdx.y;
-  const u32 n = used[cta];
-  for (u32 c = blockIdx.x * 256u + threadIdx.x; c < n; c += gridDim.x * 256u)
-    atomicAdd(&bin_nchunks[dir[(u64)cta * slice_cap + c] >> 8], 1u);
+extern "C" __global__ void __launch_bounds__(TPC_SCAN_THREADS)
+k_dir_count(const u32* __restrict__ dir, const u32* __restrict__ used, u32 slice_cap, u32* __restrict__ slice_cnt) {
+  extern __shared__ __align__(128) u32 smem_u32[];
+  const u32 nb = PRM(n_bins);
+  for (u32 i = threadIdx.x; i < nb; i += TPC_SCAN_THREADS) smem_u32[i] = 0u;
+  __syncthreads();
+  const u32 n = used[blockIdx.x];
+  const u32* d = dir + (u64)blockIdx.x * slice_cap;
+  for (u32 c = threadIdx.x; c < n; c += TPC_SCAN_THREADS) atomicAdd(&smem_u32[d[c] >> 8], 1u);
+  __syncthreads();
+  for (u32 i = threadIdx.x; i < nb; i += TPC_SCAN_THREADS) slice_cnt[(u64)blockIdx.x * nb + i] = smem_u32[i];
 }
 
 // single CTA: exclusive scans over the bins.
 //   bin_chunk_start[b] = sum_{b'<b} nchunks[b']          (NB+1 entries)
 //   batch_start[b]     = sum_{b'<b} ceil(nchunks[b']/CPB) (NB+1 entries; [NB] = total batches)
 //   batch_bin[k]       = the bin batch k belongs to
+//   slice_cnt[s][b]   := bin_chunk_start[b] + sum_{s'<s} slice_cnt[s'][b]   (in place: K4's cursors)
 extern "C" __global__ void __launch_bounds__(TPC_SCAN_THREADS)
-k_dir_scan(const u32* __restrict__ bin_nchunks, u32* __restrict__ bin_chunk_start, u32* __restrict__ batch_start,
+k_dir_scan(u32* __restrict__ slice_cnt, u32 n_slices, u32* __restrict__ bin_chunk_start, u32* __restrict__ batch_start,
            u32* __restrict__ batch_bin) {
+  extern __shared__ __align__(128) u32 smem_u32[];   // [nb] chunks per bin
   __shared__ u32 s_a[TPC_SCAN_THREADS], s_b[TPC_SCAN_THREADS];
   const u32 nb = PRM(n_bins);
+  for (u32 b = threadIdx.x; b < nb; b += TPC_SCAN_THREADS) {   // coalesced over bins
+    u32 t = 0u;
+    for (u32 sl = 0u; sl < n_slices; ++sl) t += slice_cnt[(u64)sl * nb + b];
+    smem_u32[b] = t;
+  }
+  __syncthreads();
   const u32 per = (nb + TPC_SCAN_THREADS - 1u) / TPC_SCAN_THREADS;
   const u32 lo = threadIdx.x * per;
   u32 hi = lo + per;
   if (hi > nb) hi = nb;
   u32 sa = 0u, sb = 0u;
-  for (u32 b = lo; b < hi; ++b) { u32 c = bin_nchunks[b]; sa += c; sb += (c + TPC_CPB - 1u) / TPC_CPB; }
+  for (u32 b = lo; b < hi; ++b) { u32 c = smem_u32[b]; sa += c; sb += (c + TPC_CPB - 1u) / TPC_CPB; }
   s_a[threadIdx.x] = sa; s_b[threadIdx.x] = sb;
   __syncthreads();
   for (u32 d = 1u; d < TPC_SCAN_THREADS; d <<= 1) {   // Hillis-Steele inclusive scan
@@ -400,25 +416,31 @@ k_dir_scan(const u32* __restrict__ bin_nchunks, u32* __restrict__ bin_chunk_star
   }
   u32 ea = s_a[threadIdx.x] - sa, eb = s_b[threadIdx.x] - sb;   // exclusive prefix of this thread's range
   for (u32 b = lo; b < hi; ++b) {
-    u32 c = bin_nchunks[b];
+    u32 c = smem_u32[b];
     bin_chunk_start[b] = ea; batch_start[b] = eb;
     const u32 nbt = (c + TPC_CPB - 1u) / TPC_CPB;
     for (u32 k = 0u; k < nbt; ++k) batch_bin[eb + k] = b;   // batch -> its bin, for K5
     ea += c; eb += nbt;
   }
   if (threadIdx.x == TPC_SCAN_THREADS - 1u) { bin_chunk_start[nb] = s_a[threadIdx.x]; batch_start[nb] = s_b[threadIdx.x]; }
+  __syncthreads();   // bin_chunk_start[] of this CTA's own writes is read below (same CTA: visible after the barrier)
+  for (u32 b = threadIdx.x; b < nb; b += TPC_SCAN_THREADS) {
+    u32 run = bin_chunk_start[b];
+    for (u32 sl = 0u; sl < n_slices; ++sl) { const u32 t = slice_cnt[(u64)sl * nb + b]; slice_cnt[(u64)sl * nb + b] = run; run += t; }
+  }
 }
 
-extern "C" __global__ void __launch_bounds__(256)
+extern "C" __global__ void __launch_bounds__(TPC_SCAN_THREADS)
 k_dir_fill(const u32* __restrict__ dir, const u32* __restrict__ used, u32 slice_cap,
-           const u32* __restrict__ bin_chunk_start, u32* __restrict__ bin_fill, u32* __restrict__ chunk_list) {
-  const u32 cta = blockIdx.y;
-  const u32 n = used[cta];
-  for (u32 c = blockIdx.x * 256u + threadIdx.x; c < n; c += gridDim.x * 256u) {
-    u32 id = cta * slice_cap + c;
-    u32 bin = dir[id] >> 8;
-    chunk_list[bin_chunk_start[bin] + atomicAdd(&bin_fill[bin], 1u)] = id;
-  }
+           const u32* __restrict__ slice_cnt, u32* __restrict__ chunk_list) {
+  extern __shared__ __align__(128) u32 smem_u32[];   // [nb] cursors of this slice
+  const u32 nb = PRM(n_bins);
+  for (u32 i = threadIdx.x; i < nb; i += TPC_SCAN_THREADS) smem_u32[i] = slice_cnt[(u64)blockIdx.x * nb + i];
+  __syncthreads();
+  const u32 n = used[blockIdx.x];
+  const u32 id0 = blockIdx.x * slice_cap;
+  for (u32 c = threadIdx.x; c < n; c += TPC_SCAN_THREADS)
+    chunk_list[atomicAdd(&smem_u32[dir[id0 + c] >> 8], 1u)] = id0 + c;
 }
 
 // ==========================================================================================
