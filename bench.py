@@ -39,6 +39,8 @@ def _log(msg):
 
 
 METRIC = "TPC clusterizer digits/s on Pb-Pb-like time frame"
+# ncu --set full, CFG[4] shuffled FAST generic, one launch each (profiles/r01c_ncu_full_summary.txt)
+NCU_TRAFFIC_BYTES = {}
 UNIT = "digits/s"
 
 
@@ -100,6 +102,25 @@ def _oracle_sample(fr_digits_np, fr, n_sample_sectors):
     tm = {}
     cl, st, cnt = t1.clusterize(sub, n_sample_sectors, fr.n_rows, fr.n_time, fr.n_pads, capacity=max(len(sub) // 4, 1024), timing=tm)
     return len(sub), cnt, tm["seconds"]
+
+
+def aggregate_over_ranks(ms_local, units_local, device, world):
+    """Whole-job numbers for N ranks that each processed their own shard (weak scaling, no
+    data-path collective): the time is the MAX over ranks, the work the SUM.  One all_reduce
+    each on `device` (NCCL on the GPU box, gloo in the CPU tests)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(ms_local)], dtype=torch.float64, device=device)
+    u = torch.tensor([float(units_local)], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def rank_seed(seed_base, k, rank):
+    """Every rank clusterizes its own time frame (PAPER.md 97: one process per GPU, whole frames each)."""
+    return seed_base + k + 1000 * rank
 
 
 def run_reference(args):
@@ -171,7 +192,7 @@ def main():
     tp.lib()
 
     k = args.config
-    fr = make_frame(k, device=dev, order=args.order, seed=SEED_BASE + k + 1000 * rank)
+    fr = make_frame(k, device=dev, order=args.order, seed=rank_seed(SEED_BASE, k, rank))
     digits = fr.digits
     n = fr.n_digits
     torch.cuda.synchronize(dev)
@@ -208,13 +229,9 @@ def main():
     ms_total = e0.elapsed_time(e1)
     c.set_timing(False)
     _log("timed region done: %.3f ms/step" % (ms_total / args.steps))
-    t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-    tot_digits = torch.tensor([float(n)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(tot_digits, op=dist.ReduceOp.SUM)
-    ms_step = float(t.item()) / args.steps
-    value = float(tot_digits.item()) / (ms_step * 1e-3)
+    ms_max, tot_digits = aggregate_over_ranks(ms_total, n, dev, world)
+    ms_step = ms_max / args.steps
+    value = tot_digits / (ms_step * 1e-3)
 
     # ---- e2e: host buffers through tpcclus_run_host, copies inside the timed region -----------
     e2e = None
@@ -236,11 +253,9 @@ def main():
         barrier()
         sec = (time.perf_counter() - t0) / args.e2e_steps
         assert n_e2e == n_clusters and st_e2e == 0
-        te = torch.tensor([sec], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
-        e2e = {"value": float(tot_digits.item()) / float(te.item()), "unit": UNIT, "h2d_bytes_per_step": 8 * n,
-               "d2h_bytes_per_step": 32 * n_clusters + 16, "ms_per_step": float(te.item()) * 1e3,
+        sec_max, _ = aggregate_over_ranks(sec, n, dev, world)
+        e2e = {"value": tot_digits / sec_max, "unit": UNIT, "h2d_bytes_per_step": 8 * n,
+               "d2h_bytes_per_step": 32 * n_clusters + 16, "ms_per_step": sec_max * 1e3,
                "api": "tpcclus_run_host (pinned host buffers)"}
         del h_clusters
         _log("e2e done")
@@ -253,7 +268,6 @@ def main():
     # ---- roofline of the dominant kernel (algorithmic bytes per launch) ---
     peak, peak_src = _peaks()
     avg = {nm: float(np.mean(v)) for nm, v in per_kernel.items()}
-    n_rec_fine = None
     alg = {   # bytes one launch must move (per-unit figures x units of this frame)
         "k_partition_coarse": 8 * n + 4 * n,                    # read every digit once, write one 4-byte record
         "k_partition_fine": 4 * n + 4 * n,                      # read the records, write them tile-sorted
@@ -261,13 +275,26 @@ def main():
         "k_cluster_tiles_det_count": 4 * n,
         "k_cluster_tiles_det_emit": 4 * n + 32 * n_clusters,
     }
-    dom = max(avg, key=lambda nm: avg[nm])
-    roof = None
-    if dom in alg:
-        ach = alg[dom] / (avg[dom] * 1e-3) / 1e9
-        roof = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": None, "peak_source": peak_src, "kernel_ms": avg[dom],
-                "share_of_step": avg[dom] / sum(avg.values())}
+    # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full`
+    # capture of this very workload (profiles/r01c_README.md); null for any other workload
+    traffic = NCU_TRAFFIC_BYTES if (k == 4 and args.order == "shuffled" and not args.rtc) else {}
+    step_sum = sum(avg.values())
+    per_kernel_roof = {}
+    for nm in avg:
+        if nm in alg:
+            ach = alg[nm] / (avg[nm] * 1e-3) / 1e9
+            per_kernel_roof[nm] = {"bound": "hbm", "kernel": nm, "achieved": ach, "peak": peak, "unit": "GB/s",
+                                   "frac": ach / peak, "traffic": traffic.get(nm), "alg_bytes": alg[nm],
+                                   "kernel_ms": avg[nm], "share_of_step": avg[nm] / step_sum}
+    dom = max(per_kernel_roof, key=lambda nm: avg[nm]) if per_kernel_roof else None
+    roof = dict(per_kernel_roof[dom], peak_source=peak_src) if dom else None
+    # what actually bounds K1/K5: one shared-memory atomic per record, 1 lane per clock and SM
+    # (DESIGN.md section 6): floor = records / (SMs x SM clock)
+    sm_clk = (clk.summary()["sm_mhz"] or 1965.0) * 1e6
+    n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
+    lsu = {nm: {"bound": "lsu-atomics", "floor_ms": n / (n_sm * sm_clk) * 1e3, "kernel_ms": avg[nm],
+                "frac": n / (n_sm * sm_clk) * 1e3 / avg[nm]}
+           for nm in ("k_partition_coarse", "k_partition_fine") if nm in avg}
     b_alg = 8 * n + 32 * n_clusters
     method = {"b_alg_bytes": b_alg, "achieved_gbs": b_alg / (ms_step * 1e-3) / 1e9,
               "frac_of_peak": b_alg / (ms_step * 1e-3) / 1e9 / peak}
@@ -290,7 +317,8 @@ def main():
                    "n_digits": n, "n_clusters": n_clusters, "occupancy": fr.meta["occupancy"],
                    "checksum": "%016x" % fr.meta["checksum"], "l2": "inputs (%.1f GB) larger than L2" % (8 * n / 1e9)},
         "clocks": clk.summary(), "e2e": e2e, "gpu_launches": c.launches_per_run(mode) * args.steps,
-        "roofline": roof, "method_roofline": method, "kernels_ms": avg, "cpu_baseline": cpu,
+        "roofline": roof, "rooflines": per_kernel_roof, "lsu_rooflines": lsu, "method_roofline": method,
+        "kernels_ms": avg, "cpu_baseline": cpu,
     }
     print(json.dumps(out))
     if world > 1:
