@@ -534,34 +534,61 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
   const u32 n_batches = batch_start[nb];
   bool bad = false;
 
+  // The loads of a batch are issued one batch ahead, so that their latency (batch -> bin ->
+  // chunk list -> chunk: four dependent levels) hides behind the placing and dumping of the
+  // batch before: `look` fetches the scalars, `ids` the chunk ids, `pieces` the records.
+  struct Batch { u32 b, kb, nbatch_b, c0, nch; };
+  auto look = [&](u32 batch, Batch& t) {
+    t.nch = 0u;
+    if (batch >= n_batches) return;
+    t.b = batch_bin[batch];
+    const u32 bs = batch_start[t.b];
+    t.kb = batch - bs;
+    t.nbatch_b = batch_start[t.b + 1] - bs;
+    t.c0 = bin_chunk_start[t.b] + t.kb * TPC_CPB;
+    u32 c1 = t.c0 + TPC_CPB;
+    const u32 ce = bin_chunk_start[t.b + 1];
+    if (c1 > ce) c1 = ce;
+    t.nch = c1 - t.c0;
+  };
+  auto ids = [&](const Batch& t, u32 (&cid)[4]) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const u32 ch = (threadIdx.x + (u32)i * TPC_K5_THREADS) >> 4;
+      cid[i] = ch < t.nch ? chunk_list[t.c0 + ch] : 0xFFFFFFFFu;
+    }
+  };
+  auto pieces = [&](const u32 (&cid)[4], uint4 (&v)[4], u32 (&nrec)[4]) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const u32 sub = (threadIdx.x + (u32)i * TPC_K5_THREADS) & 15u;
+      v[i] = make_uint4(0u, 0u, 0u, 0u); nrec[i] = 0u;
+      if (cid[i] != 0xFFFFFFFFu) { nrec[i] = dir[cid[i]] & 0xFFu; v[i] = ld_stream_u4(pool + (u64)cid[i] * 16u + sub); }
+    }
+  };
+  Batch cur_b, nxt_b;
+  u32 cidn[4], nrecn[4];
+  uint4 vn[4];
+  look(blockIdx.x, cur_b);
+  ids(cur_b, cidn);
+  pieces(cidn, vn, nrecn);
+  look(blockIdx.x + gridDim.x, nxt_b);
+
   for (u32 batch = blockIdx.x; batch < n_batches; batch += gridDim.x) {
-    const u32 b = batch_bin[batch];
+    const u32 b = cur_b.b, kb = cur_b.kb, nbatch_b = cur_b.nbatch_b;
     const u32 npads = PRM_NPADS((b / PRM(n_tc)) % PRM(n_rows));   // one bin = one pad row
     if (threadIdx.x < TPC_NSLMAX) { s_cnt[threadIdx.x] = 0u; s_dcnt[threadIdx.x] = 0u; s_dcur[threadIdx.x] = 0u; }
     __syncthreads();
-    const u32 kb = batch - batch_start[b];
-    const u32 nbatch_b = batch_start[b + 1] - batch_start[b];
-    const u32 c0 = bin_chunk_start[b] + kb * TPC_CPB;
-    u32 c1 = c0 + TPC_CPB;
-    if (c1 > bin_chunk_start[b + 1]) c1 = bin_chunk_start[b + 1];
-    const u32 nch = c1 - c0;
 
-    // ---- load <= 16 records per thread, count per slab, remember the rank ------------------
+    // ---- <= 16 records per thread: count per slab, remember the rank -------------------------
     u32 rec[16];
     u32 rank[8];
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-      u32 q4 = threadIdx.x + (u32)i * TPC_K5_THREADS;   // 16-byte piece of the batch
-      u32 ch = q4 >> 4, sub = q4 & 15u;
-      uint4 v = make_uint4(0u, 0u, 0u, 0u);
-      if (ch < nch) {
-        u32 cid = chunk_list[c0 + ch];
-        // K1 writes whole 32-byte sectors and zero-fills the last one: a piece is valid or not as a
-        // whole.  Both loads are issued before the test (a chunk is always 256 allocated bytes).
-        const u32 nrec = dir[cid] & 0xFFu;
-        v = ld_stream_u4(pool + (u64)cid * 16u + sub);
-        if (sub * 4u >= nrec) v = make_uint4(0u, 0u, 0u, 0u);
-      }
+      const u32 sub = (threadIdx.x + (u32)i * TPC_K5_THREADS) & 15u;
+      // K1 writes whole 32-byte sectors and zero-fills the last one: a piece is valid or not as a whole
+      uint4 v = vn[i];
+      if (sub * 4u >= nrecn[i]) v = make_uint4(0u, 0u, 0u, 0u);
       u32 r4[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
@@ -578,6 +605,7 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
         if (j & 1) rank[i * 2 + (j >> 1)] |= rk << 16; else rank[i * 2 + (j >> 1)] = rk;
       }
     }
+    ids(nxt_b, cidn);   // chunk ids of the next batch: in flight during the scan and the placing
     __syncthreads();
     // ---- exclusive scan of padded run lengths (one warp, NSLMAX/32 slabs per lane) ---------
     if (threadIdx.x < 32) {
@@ -616,6 +644,9 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
         }
       }
     }
+    pieces(cidn, vn, nrecn);   // records of the next batch: in flight during the dump
+    cur_b = nxt_b;
+    look(batch + 2u * gridDim.x, nxt_b);
     if (threadIdx.x >= TPC_NSLMAX && threadIdx.x < TPC_NSLMAX + nsl) {   // zero the padding of every run (K6 skips record 0)
       const u32 sl = threadIdx.x - TPC_NSLMAX;
       for (u32 k = s_off[sl] + s_cnt[sl] + s_dcnt[sl]; k < s_off[sl + 1u]; ++k) buf[k] = 0u;
