@@ -40,7 +40,8 @@ def _log(msg):
 
 METRIC = "TPC clusterizer digits/s on Pb-Pb-like time frame"
 # ncu --set full, CFG[4] shuffled FAST generic, one launch each (profiles/r01c_ncu_full_summary.txt)
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {"k_partition_coarse": 12766551000 + 6479542000, "k_partition_fine": 9145850000 + 7143103000,
+                     "k_cluster_tiles_fast": 7338236000 + 1902622000}
 UNIT = "digits/s"
 
 
