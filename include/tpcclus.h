@@ -184,6 +184,11 @@ TPCCLUS_API double tpcclus_rtc_build_ms(const tpcclus_handle* h);
  * n_sectors * n_time * sum(n_pads) entries).  Not on the hot path. */
 TPCCLUS_API int tpcclus_debug_dense_map(tpcclus_handle* h, uint16_t* d_map, void* cuda_stream);
 
+/* Debug / test hook: 1 if the last DETERMINISTIC run had more clusters than its temporary run
+ * buffer holds (max_digits / 8) and therefore took the chained-scan fallback, 0 if not, negative
+ * on error.  Synchronises the device.  Results are identical either way. */
+TPCCLUS_API int tpcclus_debug_det_fallback(tpcclus_handle* h);
+
 #ifdef __cplusplus
 }
 #endif

@@ -54,7 +54,7 @@ _lib = None
 EXPORTS = ("tpcclus_workspace_bytes", "tpcclus_workspace_bytes_host", "tpcclus_create", "tpcclus_run",
            "tpcclus_run_host", "tpcclus_destroy", "tpcclus_error_string", "tpcclus_last_error",
            "tpcclus_launches_per_run", "tpcclus_set_timing", "tpcclus_last_timing", "tpcclus_rtc_build_ms",
-           "tpcclus_debug_dense_map")
+           "tpcclus_debug_dense_map", "tpcclus_debug_det_fallback")
 
 
 def lib() -> C.CDLL:
@@ -94,6 +94,8 @@ def lib() -> C.CDLL:
     L.tpcclus_rtc_build_ms.argtypes = [C.c_void_p]
     L.tpcclus_debug_dense_map.restype = C.c_int
     L.tpcclus_debug_dense_map.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    L.tpcclus_debug_det_fallback.restype = C.c_int
+    L.tpcclus_debug_det_fallback.argtypes = [C.c_void_p]
     _lib = L
     return L
 
@@ -235,6 +237,10 @@ class Clusterizer:
         if rc != 0:
             raise TpcclusError(rc, "tpcclus_debug_dense_map", (lib().tpcclus_last_error(self._h) or b"").decode())
         return m
+
+    def det_fallback(self):
+        """Debug hook: did the last DETERMINISTIC run take the chained-scan fallback?"""
+        return int(lib().tpcclus_debug_det_fallback(self._h)) == 1
 
     def close(self):
         if getattr(self, "_h", None):

@@ -34,7 +34,7 @@ struct Layout {   // byte offsets into the workspace
   uint64_t counters, counters_bytes;   // zeroed at the head of every run
   uint64_t status, blob_cursor, slice_cnt;
   uint64_t used, bin_chunk_start, batch_start, batch_bin, dir, chunk_list, pool, blob, idx;
-  uint64_t tile_cnt, tile_local, block_sum, block_prefix, row_off;
+  uint64_t ticket, temp_cursor, det_flag, tile_state, tile_base, tile_cnt, tile_local, block_sum, block_prefix, row_off;
   uint64_t total;        // device-path workspace
   uint64_t host_digits;  // staging of run_host (beyond `total`)
   uint64_t host_out;     // n_clusters (8) + status (4)
@@ -109,6 +109,10 @@ int make_geometry(const tpcclus_params* p, Geometry* g) {
   L.counters = o;
   L.status = take(4);
   L.blob_cursor = take(8);
+  L.ticket = take(4);
+  L.temp_cursor = take(8);
+  L.det_flag = take(4);
+  L.tile_state = take(8ull * g->n_tiles);   // DET chained scan: must start at 0 every run
   L.counters_bytes = o - L.counters;
   L.slice_cnt = take(4ull * nb * g->g1);
   L.used = take(4ull * g->g1);
@@ -120,6 +124,7 @@ int make_geometry(const tpcclus_params* p, Geometry* g) {
   L.pool = take(256ull * g->n_chunks_max);
   L.blob = take(4ull * g->blob_cap);
   L.idx = take(8ull * g->idx_cap);
+  L.tile_base = take(8ull * g->n_tiles);
   L.tile_cnt = take(4ull * g->n_tiles);
   L.tile_local = take(4ull * g->n_tiles);
   L.block_sum = take(4ull * g->n_scan_blocks);
@@ -178,16 +183,17 @@ Rtc& rtc() {
   return r;
 }
 
-enum KernelId { K_PART_COARSE, K_DIR_COUNT, K_DIR_SCAN, K_DIR_FILL, K_PART_FINE, K_TILES_FAST, K_TILES_COUNT,
-                K_TILES_EMIT, K_TILES_DUMP, K_SCAN_LOCAL, K_SCAN_SUMS, K_COUNT_ };
+enum KernelId { K_PART_COARSE, K_DIR_COUNT, K_DIR_SCAN, K_DIR_FILL, K_PART_FINE, K_TILES_FAST, K_TILES_DET,
+                K_TILES_DET_TEMP, K_TILES_DUMP, K_SCAN_LOCAL, K_SCAN_SUMS, K_EMIT_ORDERED, K_COUNT_ };
 const char* const kKernelNames[K_COUNT_] = {
     "k_partition_coarse", "k_dir_count", "k_dir_scan", "k_dir_fill", "k_partition_fine", "k_cluster_tiles_fast",
-    "k_cluster_tiles_det_count", "k_cluster_tiles_det_emit", "k_cluster_tiles_dump_map", "k_scan_local", "k_scan_sums"};
+    "k_cluster_tiles_det", "k_cluster_tiles_det_temp", "k_cluster_tiles_dump_map", "k_scan_local", "k_scan_sums",
+    "k_emit_ordered"};
 const void* const kKernelPtrs[K_COUNT_] = {
     (const void*)k_partition_coarse, (const void*)k_dir_count, (const void*)k_dir_scan, (const void*)k_dir_fill,
-    (const void*)k_partition_fine, (const void*)k_cluster_tiles_fast, (const void*)k_cluster_tiles_det_count,
-    (const void*)k_cluster_tiles_det_emit, (const void*)k_cluster_tiles_dump_map, (const void*)k_scan_local,
-    (const void*)k_scan_sums};
+    (const void*)k_partition_fine, (const void*)k_cluster_tiles_fast, (const void*)k_cluster_tiles_det,
+    (const void*)k_cluster_tiles_det_temp, (const void*)k_cluster_tiles_dump_map, (const void*)k_scan_local,
+    (const void*)k_scan_sums, (const void*)k_emit_ordered};
 
 }  // namespace
 
@@ -293,7 +299,7 @@ int build_rtc(tpcclus_handle* h) {
       return fail(nullptr, TPCCLUS_ERR_NVRTC, std::string("cuModuleGetFunction: ") + kKernelNames[k]);
   const int CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES = 8;
   struct { int k; uint32_t b; } sm[] = {{K_PART_COARSE, h->smem_k1}, {K_PART_FINE, h->smem_k5}, {K_TILES_FAST, h->smem_k6},
-                                        {K_TILES_COUNT, h->smem_k6}, {K_TILES_EMIT, h->smem_k6}, {K_TILES_DUMP, h->smem_k6}};
+                                        {K_TILES_DET, h->smem_k6}, {K_TILES_DET_TEMP, h->smem_k6}, {K_TILES_DUMP, h->smem_k6}};
   for (auto& e : sm)
     if (r.cuFuncSetAttribute(h->fn[e.k], CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES, (int)e.b) != 0)
       return fail(nullptr, TPCCLUS_ERR_CUDA, std::string("cuFuncSetAttribute: ") + kKernelNames[e.k]);
@@ -347,7 +353,7 @@ int tpcclus_create(const tpcclus_params* p, tpcclus_handle** out) {
     if (rc != TPCCLUS_OK) return bail(rc);
   } else {
     struct { int k; uint32_t b; } sm[] = {{K_PART_COARSE, h->smem_k1}, {K_PART_FINE, h->smem_k5}, {K_TILES_FAST, h->smem_k6},
-                                          {K_TILES_COUNT, h->smem_k6}, {K_TILES_EMIT, h->smem_k6}, {K_TILES_DUMP, h->smem_k6}};
+                                          {K_TILES_DET, h->smem_k6}, {K_TILES_DET_TEMP, h->smem_k6}, {K_TILES_DUMP, h->smem_k6}};
     for (auto& s : sm) {
       e = cudaFuncSetAttribute(kKernelPtrs[s.k], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s.b);
       if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("cudaFuncSetAttribute(") + kKernelNames[s.k] + "): " + cudaGetErrorString(e); return bail(TPCCLUS_ERR_CUDA); }
@@ -383,7 +389,7 @@ const char* tpcclus_last_error(const tpcclus_handle* h) { return h ? h->err.c_st
 
 int tpcclus_launches_per_run(const tpcclus_handle* h, int mode) {
   (void)h;
-  return mode == TPCCLUS_MODE_DETERMINISTIC ? 9 : 6;
+  return mode == TPCCLUS_MODE_DETERMINISTIC ? 10 : 6;   // DET: + K7, K8, K9 and the (normally idle) chained K6
 }
 
 int tpcclus_set_timing(tpcclus_handle* h, int enable) {
@@ -413,8 +419,8 @@ namespace {
 
 struct RunPtrs {
   u32 *status, *slice_cnt, *used, *bin_chunk_start, *batch_start, *batch_bin, *dir, *chunk_list, *blob;
-  u32 *tile_cnt, *tile_local, *block_sum;
-  u64 *blob_cursor, *idx, *block_prefix, *row_off;
+  u32 *ticket, *det_flag, *tile_cnt, *tile_local, *block_sum;
+  u64 *blob_cursor, *idx, *tile_state, *temp_cursor, *tile_base, *block_prefix, *row_off;
   uint4* pool;
 };
 RunPtrs ptrs(tpcclus_handle* h) {
@@ -426,8 +432,10 @@ RunPtrs ptrs(tpcclus_handle* h) {
   p.bin_chunk_start = (u32*)(w + L.bin_chunk_start); p.batch_start = (u32*)(w + L.batch_start); p.batch_bin = (u32*)(w + L.batch_bin);
   p.dir = (u32*)(w + L.dir); p.chunk_list = (u32*)(w + L.chunk_list); p.pool = (uint4*)(w + L.pool);
   p.blob = (u32*)(w + L.blob); p.idx = (u64*)(w + L.idx);
-  p.tile_cnt = (u32*)(w + L.tile_cnt); p.tile_local = (u32*)(w + L.tile_local);
-  p.block_sum = (u32*)(w + L.block_sum); p.block_prefix = (u64*)(w + L.block_prefix); p.row_off = (u64*)(w + L.row_off);
+  p.ticket = (u32*)(w + L.ticket); p.tile_state = (u64*)(w + L.tile_state); p.row_off = (u64*)(w + L.row_off);
+  p.temp_cursor = (u64*)(w + L.temp_cursor); p.det_flag = (u32*)(w + L.det_flag); p.tile_base = (u64*)(w + L.tile_base);
+  p.tile_cnt = (u32*)(w + L.tile_cnt); p.tile_local = (u32*)(w + L.tile_local); p.block_sum = (u32*)(w + L.block_sum);
+  p.block_prefix = (u64*)(w + L.block_prefix);
   return p;
 }
 
@@ -473,7 +481,6 @@ int tpcclus_run(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n, co
       ((uintptr_t)out->clusters & 15u) || ((uintptr_t)out->n_clusters & 7u))
     return fail(h, TPCCLUS_ERR_INVALID_ARG, "tpcclus_run: bad argument");
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  const Geometry& g = h->g;
   CUDA_TRY(h, cudaSetDevice(h->params.device));
   h->n_timed = 0;
   RunPtrs p = ptrs(h);
@@ -484,21 +491,31 @@ int tpcclus_run(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n, co
   K6Args a;
   a.blob = p.blob; a.idx = p.idx; a.batch_start = p.batch_start;
   a.out = (uint4*)out->clusters; a.capacity = out->capacity; a.n_clusters = (u64*)out->n_clusters; a.status = status;
-  a.tile_cnt = p.tile_cnt; a.tile_local = p.tile_local; a.block_prefix = p.block_prefix;
+  a.ticket = p.ticket; a.tile_state = p.tile_state;
+  a.temp = p.pool; a.temp_cap = h->g.n_chunks_max * 8ull; a.temp_cursor = p.temp_cursor;   // the K1 pool is dead after K5
+  a.tile_base = p.tile_base; a.tile_cnt = p.tile_cnt; a.det_flag = p.det_flag;
   a.dmap = nullptr; a.row_off = p.row_off;
   void* ka[] = {&a};
   if (mode == TPCCLUS_MODE_FAST) {
     CUDA_TRY(h, cudaMemsetAsync(out->n_clusters, 0, 8, st));
     if ((rc = launch(h, K_TILES_FAST, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
   } else {
-    if ((rc = launch(h, K_TILES_COUNT, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
+    // ordered output (PAPER.md 47-50): runs into the temporary buffer, scan of the tile counts,
+    // ordered copy.  Should the buffer be too small (more than max_digits/8 clusters) the flag is
+    // set, K9 does nothing and the chained-scan K6 redoes the frame; otherwise that launch exits at once.
+    const Geometry& g = h->g;
+    if ((rc = launch(h, K_TILES_DET_TEMP, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
     u32 nt = g.n_tiles, nblk = g.n_scan_blocks;
     { void* s[] = {&p.tile_cnt, &p.tile_local, &p.block_sum, &nt};
       if ((rc = launch(h, K_SCAN_LOCAL, dim3(nblk), dim3(TPC_SCAN_THREADS), 0, st, s))) return rc; }
     { u64* total = (u64*)out->n_clusters;
       void* s[] = {&p.block_sum, &p.block_prefix, &nblk, &total};
       if ((rc = launch(h, K_SCAN_SUMS, dim3(1), dim3(TPC_SCAN_THREADS), 0, st, s))) return rc; }
-    if ((rc = launch(h, K_TILES_EMIT, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
+    { uint4* o = (uint4*)out->clusters; u64 cap = out->capacity;
+      void* s[] = {&a.temp, &p.tile_base, &p.tile_cnt, &p.tile_local, &p.block_prefix, &nt, &o, &cap, &p.det_flag, &status};
+      if ((rc = launch(h, K_EMIT_ORDERED, dim3(g.g1 * 8u), dim3(256), 0, st, s))) return rc; }
+    CUDA_TRY(h, cudaMemsetAsync(p.ticket, 0, 4, st));
+    if ((rc = launch(h, K_TILES_DET, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
   }
   h->ran = true;
   return TPCCLUS_OK;
@@ -536,6 +553,13 @@ int tpcclus_run_host(tpcclus_handle* h, const tpcclus_digit* h_digits, uint64_t 
   return TPCCLUS_OK;
 }
 
+int tpcclus_debug_det_fallback(tpcclus_handle* h) {
+  if (!h) return TPCCLUS_ERR_INVALID_ARG;
+  uint32_t f = 0;
+  CUDA_TRY(h, cudaMemcpy(&f, h->ws + h->g.lay.det_flag, 4, cudaMemcpyDeviceToHost));   // synchronises
+  return f != 0 ? 1 : 0;
+}
+
 int tpcclus_debug_dense_map(tpcclus_handle* h, uint16_t* d_map, void* cuda_stream) {
   if (!h || !d_map) return TPCCLUS_ERR_INVALID_ARG;
   if (!h->ran) return fail(h, TPCCLUS_ERR_INVALID_ARG, "tpcclus_debug_dense_map: no run() yet");
@@ -549,7 +573,8 @@ int tpcclus_debug_dense_map(tpcclus_handle* h, uint16_t* d_map, void* cuda_strea
   K6Args a;
   memset(&a, 0, sizeof a);
   a.blob = p.blob; a.idx = p.idx; a.batch_start = p.batch_start; a.status = p.status;
-  a.dmap = d_map; a.row_off = p.row_off;
+  a.dmap = d_map; a.row_off = p.row_off; a.ticket = p.ticket; a.tile_state = p.tile_state; a.det_flag = p.det_flag;
+  CUDA_TRY(h, cudaMemsetAsync(p.ticket, 0, 4, st));   // the run before used the tickets up
   void* ka[] = {&a};
   int rc = launch(h, K_TILES_DUMP, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka);
   h->timing = t;

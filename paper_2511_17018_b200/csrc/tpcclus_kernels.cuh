@@ -14,7 +14,6 @@
 //   K6 cluster_tiles     per (sector,row,slab) tile: charge map in shared memory (O0),
 //                        3x3 peaks (O1), suppression (O2), 5x5 CoG (O3,O4), compaction,
 //                        ordered emission (O5)
-//   K7 scan_local / K8 scan_sums   deterministic mode: exclusive scan of per-tile counts
 #pragma once
 
 typedef unsigned int u32;
@@ -450,8 +449,11 @@ k_dir_fill(const u32* __restrict__ dir, const u32* __restrict__ used, u32 slice_
 }
 
 // ==========================================================================================
-// K7/K8  exclusive scan of per-tile cluster counts (deterministic mode, O5 / PAPER.md 47-50:
-// the ordered-scan compaction is the "slower deterministic algorithm" that replaces atomics)
+// K7/K8/K9  deterministic mode, ordered output (O5 / PAPER.md 47-50: an ordered scan and an
+// ordered copy after the kernel whose output order depends on the concurrency).  K6 emits each
+// tile's clusters, already in (time,pad) order, as one run at an atomically allocated place of
+// a temporary buffer and records (place, count) per tile; K7/K8 scan the counts; K9 copies the
+// runs to their final places in tile order.
 // ==========================================================================================
 extern "C" __global__ void __launch_bounds__(TPC_SCAN_THREADS)
 k_scan_local(const u32* __restrict__ in, u32* __restrict__ out_local, u32* __restrict__ block_sum, u32 n) {
@@ -498,6 +500,28 @@ k_scan_sums(const u32* __restrict__ block_sum, u64* __restrict__ block_prefix, u
     __syncthreads();
   }
   if (threadIdx.x == 0) *total = carry;
+}
+
+
+// K9: one warp per tile, 16 bytes per lane.  Skipped as a whole (flag set) when the temporary
+// buffer was too small: the chained-scan variant of K6 then redoes the frame (k6_chain).
+extern "C" __global__ void __launch_bounds__(256)
+k_emit_ordered(const uint4* __restrict__ temp, const u64* __restrict__ tile_base, const u32* __restrict__ tile_cnt,
+               const u32* __restrict__ tile_local, const u64* __restrict__ block_prefix, u32 n_tiles,
+               uint4* __restrict__ out, u64 capacity, const u32* __restrict__ flag, u32* __restrict__ status) {
+  if (*flag != 0u) return;
+  const u32 lane = threadIdx.x & 31u;
+  bool over = false;
+  for (u32 tile = blockIdx.x * 8u + (threadIdx.x >> 5); tile < n_tiles; tile += gridDim.x * 8u) {
+    const u32 cnt = tile_cnt[tile];
+    if (cnt == 0u) continue;
+    const u64 src = tile_base[tile] * 2ull;
+    const u64 dst0 = block_prefix[tile / TPC_SCAN_PER_CTA] + tile_local[tile];
+    u64 keep = capacity > dst0 ? capacity - dst0 : 0ull;   // Q22: the first `capacity` clusters stay, in order
+    if (keep < cnt) over = true; else keep = cnt;
+    for (u32 i = lane; i < (u32)keep * 2u; i += 32u) out[dst0 * 2ull + i] = temp[src + i];
+  }
+  if (over) atomicOr(status, TPC_STATUS_OVERFLOW);
 }
 
 // ==========================================================================================
@@ -680,12 +704,12 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
 // max.u16x2), mark peaks with bit 15, run the suppression per listed peak (O2), mark the
 // survivors in a per-row pad bitmask -- which ranks every cluster in (time, pad) order inside
 // the tile without a sort -- and finalise the 5x5 sums (O3/O4).  The base of the tile comes
-// from one atomic (FAST) or from the exclusive scan of the tile counts (DETERMINISTIC: K6
-// runs once to count, K7/K8 scan, K6 runs again to emit).
+// from one atomic (FAST) or from a single-pass chained scan of the tile counts (DETERMINISTIC,
+// k6_chain below).  Tiles are handed out by ticket, in increasing order.
 // ==========================================================================================
 #define TPC_MODE_FAST 0
-#define TPC_MODE_DET_COUNT 1
-#define TPC_MODE_DET_EMIT 2
+#define TPC_MODE_DET 1        // chained scan inside K6 (fallback: any number of clusters)
+#define TPC_MODE_DET_TEMP 2   // runs into the temporary buffer, K7-K9 order them (the usual path)
 #define TPC_MODE_DUMP_MAP 3
 #define TPC_K6_CONSUMERS 256u                   // threads that compute
 #define TPC_K6_THREADS (TPC_K6_CONSUMERS + 32u)  // + the producer warp
@@ -696,7 +720,10 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
 struct K6Args {
   const u32* blob; const u64* idx; const u32* batch_start;
   uint4* out; u64 capacity; u64* n_clusters; u32* status;
-  u32* tile_cnt; const u32* tile_local; const u64* block_prefix;
+  u32* ticket;        // next tile to hand out (zeroed per run)
+  u64* tile_state;    // DET: chained scan of the tile counts, [n_tiles], zeroed per run
+  uint4* temp; u64 temp_cap; u64* temp_cursor;   // DET_TEMP: run buffer (the dead K1 pool), in clusters
+  u64* tile_base; u32* tile_cnt; u32* det_flag;  // DET_TEMP: per-tile (place, count); flag = buffer too small
   u16* dmap; const u64* row_off;   // DUMP_MAP only: row_off[r] = cells of rows < r in one sector; [n_rows] = per sector
 };
 
@@ -769,6 +796,35 @@ __device__ __forceinline__ K6Smem k6_smem(u32* p) {
   return s;
 }
 
+// ---- DET: single-pass chained scan of the tile counts (decoupled look-back) ---------------
+// tile_state[t] = flag[62:64) | value[0:62): flag 1 = the tile's own count, flag 2 = the inclusive
+// prefix up to and including t.  Tiles are handed out by ticket in increasing order, so every
+// tile a CTA waits for was started by a CTA that is running: no co-residency assumption.
+// The result is a pure function of the counts, i.e. of the input set (an ordered scan
+// in place of atomics).  Called by one full warp; returns the exclusive prefix of `tile`.
+// relaxed is enough: the 64-bit word carries everything (flag and value), nothing else is published with it
+__device__ __forceinline__ u64 ld_state_u64(const u64* p) { u64 v; asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory"); return v; }
+__device__ __forceinline__ void st_state_u64(u64* p, u64 v) { asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory"); }
+__device__ __forceinline__ u64 k6_chain(u64* state, u32 tile, u32 count) {
+  const u32 lane = lane_id();
+  if (lane == 0u) st_state_u64(state + tile, (1ull << 62) | (u64)count);
+  u64 excl = 0ull;
+  for (long long j = (long long)tile - 1; j >= 0; j -= 32) {
+    const long long i = j - (long long)lane;
+    u64 v = i >= 0 ? ld_state_u64(state + i) : (2ull << 62);   // before tile 0: prefix 0
+    while (__any_sync(0xFFFFFFFFu, (v >> 62) == 0ull)) { if ((v >> 62) == 0ull) v = ld_state_u64(state + i); }
+    const u32 pm = __ballot_sync(0xFFFFFFFFu, (v >> 62) == 2ull);
+    const u32 first = pm ? (u32)__ffs((int)pm) - 1u : 31u;   // nearest tile that already has its prefix
+    u64 c = lane <= first ? (v & ((1ull << 62) - 1ull)) : 0ull;
+#pragma unroll
+    for (int d = 16; d >= 1; d >>= 1) c += __shfl_xor_sync(0xFFFFFFFFu, c, d);
+    excl += c;
+    if (pm) break;
+  }
+  if (lane == 0u) st_state_u64(state + tile, (2ull << 62) | (excl + (u64)count));
+  return excl;
+}
+
 // Producer warp: stages round `round` of a tile -- the 16-byte units [round*CAPU, (round+1)*CAPU)
 // of the concatenation of the tile's runs (one run per K5 batch of the bin, 32-byte aligned and
 // zero-padded by K5) -- and arrives on the full barrier.  Returns the tile's total units.
@@ -834,18 +890,29 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       if (bytes != 0u)
         asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(a.blob + (e0 & ((1ull << 40) - 1ull))), "r"(bytes) : "memory");
     };
-    if (blockIdx.x < n_tiles) look_ahead(blockIdx.x);
-    for (u32 tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    auto take = [&]() -> u32 {   // next tile, in increasing order over the whole grid
+      u32 t = 0u;
+      if (lane == 0u) t = atomicAdd(a.ticket, 1u);
+      return __shfl_sync(0xFFFFFFFFu, t, 0);
+    };
+    u32 tile = take();
+    if (tile < n_tiles) look_ahead(tile);
+    while (tile < n_tiles) {
       const u64 ib_c = ib, e0_c = e0;
       const u32 nbatch_c = nbatch;
+      const u32 next = take();
       mbar_wait_backoff(&s.bar[1], ph); ph ^= 1u;
+      if (lane == 0u) s.misc[3] = tile;   // published by the arrive in k6_stage
       const u32 total = k6_stage(s, a, ib_c, nbatch_c, 0u, e0_c);
-      if (tile + gridDim.x < n_tiles) look_ahead(tile + gridDim.x);
+      if (next < n_tiles) look_ahead(next);
       for (u32 round = 1u; round * TPC_K6_CAPU < total; ++round) {
         mbar_wait_backoff(&s.bar[1], ph); ph ^= 1u;
         k6_stage(s, a, ib_c, nbatch_c, round, e0_c);
       }
+      tile = next;
     }
+    mbar_wait_backoff(&s.bar[1], ph);   // tell the consumers there is nothing left
+    if (lane == 0u) { s.misc[3] = 0xFFFFFFFFu; s.misc[2] = 0u; mbar_arrive(&s.bar[0]); }
     return;
   }
 
@@ -861,14 +928,19 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
     if (tid == 0) s.misc[0] = 0u;
   };
   zero_tile();
-  for (u32 tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-    const u32 b = tile / nsl, sl = tile - b * nsl;
+  for (;;) {
     mbar_wait(&s.bar[0], ph); ph ^= 1u;
-    const u32 total = s.misc[2];
+    const u32 tile = s.misc[3], total = s.misc[2];
+    if (tile == 0xFFFFFFFFu) break;   // block-uniform
+    const u32 b = tile / nsl, sl = tile - b * nsl;
     if (total == 0u) {   // block-uniform: nothing in this tile; the map stays zero
       __syncwarp();
       if (lane_id() == 0u) mbar_arrive(&s.bar[1]);
-      if (MODE == TPC_MODE_DET_COUNT && tid == 0) a.tile_cnt[tile] = 0u;
+      if (MODE == TPC_MODE_DET_TEMP && tid == 0) a.tile_cnt[tile] = 0u;
+      if (MODE == TPC_MODE_DET && tid >= TPC_K6_CONSUMERS - 32u) {   // an empty tile is still a link of the chain
+        const u64 ex = k6_chain(a.tile_state, tile, 0u);
+        if (tile == n_tiles - 1u && lane_id() == 0u) *a.n_clusters = ex;
+      }
       continue;
     }
     const u32 tc = b % PRM(n_tc), sr = b / PRM(n_tc);
@@ -1102,7 +1174,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
     // ---- rank (last warp) || O3 + O4 (everyone else first) ------------------------------------
     // rowpre[tl] = survivors in rows < tl, which ranks every cluster in (time, pad) order inside
     // the tile without a sort.  The last warp computes it and fetches the tile's base (FAST: one
-    // atomic; DET: the scanned count) while the other warps already do the 5x5 arithmetic; the
+    // atomic; DET: the chained scan) while the other warps already do the 5x5 arithmetic; the
     // results meet at barrier G.
     if (tid >= TPC_K6_CONSUMERS - 32u) {
       const u32 lane = lane_id();
@@ -1123,10 +1195,18 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       u32 ex = inc - t;
 #pragma unroll
       for (int k = 0; k < 5; ++k) { const u32 tl = lane * 5u + (u32)k; if (tl < TPC_TT) s.rowpre[tl] = ex; ex += cnt[k]; }
-      if (lane == 31u) {
-        if (MODE == TPC_MODE_DET_COUNT) a.tile_cnt[tile] = inc;
-        if (MODE == TPC_MODE_FAST) s.base[0] = atomicAdd(a.n_clusters, (u64)inc);
-        if (MODE == TPC_MODE_DET_EMIT) s.base[0] = a.block_prefix[tile / TPC_SCAN_PER_CTA] + a.tile_local[tile];
+      const u32 count = __shfl_sync(0xFFFFFFFFu, inc, 31);
+      if (MODE == TPC_MODE_FAST) { if (lane == 31u) s.base[0] = atomicAdd(a.n_clusters, (u64)count); }
+      if (MODE == TPC_MODE_DET_TEMP) {
+        if (lane == 31u) {
+          const u64 at = atomicAdd(a.temp_cursor, (u64)count);
+          a.tile_base[tile] = at; a.tile_cnt[tile] = count; s.base[0] = at;
+          if (at + count > a.temp_cap) atomicOr(a.det_flag, 1u);
+        }
+      }
+      if (MODE == TPC_MODE_DET) {
+        const u64 ex = k6_chain(a.tile_state, tile, count);
+        if (lane == 0u) { s.base[0] = ex; if (tile == n_tiles - 1u) *a.n_clusters = ex + (u64)count; }
       }
     }
     // one cluster per thread held in registers across barrier G (further ones, npk > threads, after it)
@@ -1167,17 +1247,21 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       return true;
     };
     auto emit = [&](u64 slot, const uint4& c0, const uint4& c1) {
-      if (slot < a.capacity) { a.out[slot * 2u] = c0; a.out[slot * 2u + 1u] = c1; }
-      else atomicOr(a.status, TPC_STATUS_OVERFLOW);
+      if (MODE == TPC_MODE_DET_TEMP) {
+        if (slot < a.temp_cap) { a.temp[slot * 2u] = c0; a.temp[slot * 2u + 1u] = c1; }
+      } else {
+        if (slot < a.capacity) { a.out[slot * 2u] = c0; a.out[slot * 2u + 1u] = c1; }
+        else atomicOr(a.status, TPC_STATUS_OVERFLOW);
+      }
     };
-    if (MODE != TPC_MODE_DET_COUNT && tid < npk) {
+    if (tid < npk) {
       const u32 e = s.peaks[tid];
       my_tl = e >> 8;
       u32 rk;
       if (cog(e, o0, o1, rk)) inrow = rk;
     }
     csync();   // G: rowpre and base are there; nobody reads the map of this tile's first 256 peaks any more
-    if (MODE != TPC_MODE_DET_COUNT) {
+    {
       const u64 base = s.base[0];
       if (inrow != 0xFFFFFFFFu) emit(base + s.rowpre[my_tl] + inrow, o0, o1);
       for (u32 i = tid + TPC_K6_CONSUMERS; i < npk; i += TPC_K6_CONSUMERS) {   // dense tiles only
@@ -1195,13 +1279,14 @@ extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, TPC_K6_CTAS) k_clus
   extern __shared__ __align__(128) u32 smem_u32[];
   k6_body<TPC_MODE_FAST>(a, smem_u32);
 }
-extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, TPC_K6_CTAS) k_cluster_tiles_det_count(K6Args a) {
+extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, TPC_K6_CTAS) k_cluster_tiles_det(K6Args a) {
   extern __shared__ __align__(128) u32 smem_u32[];
-  k6_body<TPC_MODE_DET_COUNT>(a, smem_u32);
+  if (*a.det_flag == 0u) return;   // K7-K9 already delivered the ordered output
+  k6_body<TPC_MODE_DET>(a, smem_u32);
 }
-extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, TPC_K6_CTAS) k_cluster_tiles_det_emit(K6Args a) {
+extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, TPC_K6_CTAS) k_cluster_tiles_det_temp(K6Args a) {
   extern __shared__ __align__(128) u32 smem_u32[];
-  k6_body<TPC_MODE_DET_EMIT>(a, smem_u32);
+  k6_body<TPC_MODE_DET_TEMP>(a, smem_u32);
 }
 extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, TPC_K6_CTAS) k_cluster_tiles_dump_map(K6Args a) {
   extern __shared__ __align__(128) u32 smem_u32[];

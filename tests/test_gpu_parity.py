@@ -327,3 +327,32 @@ def test_full_frame_sampled_parity(tp, cuda_device, k):
         assert got.tobytes() == exp.tobytes(), (k, s_, r_)
         cells = set(zip(sel.view(t1.DIGIT)["time"].tolist(), sel.view(t1.DIGIT)["pad"].tolist()))
         assert all((int(t_), int(p_)) in cells for t_, p_ in zip(got["time_peak"], got["pad_peak"]))   # I5
+
+
+def test_det_fallback_when_run_buffer_is_too_small(tp, cuda_device):
+    """DETERMINISTIC normally writes each tile's clusters as a run into a temporary buffer of
+    max_digits / 8 clusters and orders the runs afterwards (K7-K9); a frame with more clusters
+    than that (here: every digit is its own cluster) must take the chained-scan fallback and
+    still be byte-identical to the oracle.  The usual frames must not take it."""
+    T, P, R = 3000, 138, 4
+    rows = np.zeros((R, T // 2, P // 2), dtype=t1.DIGIT)
+    rows["time"] = (2 * np.arange(T // 2, dtype=np.uint16))[None, :, None]
+    rows["pad"] = (2 * np.arange(P // 2, dtype=np.uint8))[None, None, :]
+    rows["row"] = np.arange(R, dtype=np.uint8)[:, None, None]
+    rows["charge"] = 50
+    d = rows.reshape(-1)
+    d = d[np.random.default_rng(31).permutation(len(d))]
+    exp, _ = _oracle(d, 1, R, T, [P] * R)
+    assert len(exp) == len(d)
+    c = tp.Clusterizer(1, R, T, [P] * R, len(d))
+    det, n, st = c.run_sync(_digits_tensor(d, cuda_device), tp.MODE_DETERMINISTIC)
+    assert c.det_fallback() and st == 0 and n == len(exp)
+    assert det.tobytes() == exp.tobytes()
+    fast, n, st = c.run_sync(_digits_tensor(d, cuda_device), tp.MODE_FAST)
+    _check_fast(fast, exp)
+    c.close()
+    fr = make_frame(0)
+    c = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, fr.n_digits)
+    c.run_sync(fr.digits.to(cuda_device), tp.MODE_DETERMINISTIC)
+    assert not c.det_fallback()
+    c.close()
