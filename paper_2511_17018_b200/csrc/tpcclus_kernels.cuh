@@ -777,10 +777,12 @@ struct K6Smem {
   u32* rowmask;    // [TT][8]  O2 survivors, bit = pad
   u32* rowpre; u32* misc; u16* peaks;
 };
-// misc: [0] n_peaks  [2] total 16-byte units of the tile being staged
+// misc: [0] n_peaks  [3] first tile of the stage  [4] tiles in the stage  [8+2m],[9+2m] offset and
+//       size (16-byte units) of tile m's records in `rec`
+#define TPC_K6_GROUP 4u   // tiles (consecutive slabs of one bin) a ticket covers
 #define TPC_K6_PMW 9u
 __host__ __device__ inline u32 tpc_k6_smem_bytes(u32 pitch, u32 max_peaks) {
-  return (TPC_K6_CAP + TPC_TT * pitch / 2u + 4u + 2u + TPC_TT * (8u + TPC_K6_PMW) + TPC_TT + 2u + 8u + (max_peaks + 1u) / 2u) * 4u + 128u;
+  return (TPC_K6_CAP + TPC_TT * pitch / 2u + 4u + 2u + TPC_TT * (8u + TPC_K6_PMW) + TPC_TT + 2u + 16u + (max_peaks + 1u) / 2u) * 4u + 128u;
 }
 __device__ __forceinline__ K6Smem k6_smem(u32* p) {
   K6Smem s;
@@ -791,7 +793,7 @@ __device__ __forceinline__ K6Smem k6_smem(u32* p) {
   s.pmask = p; p += TPC_TT * TPC_K6_PMW;   // pmask and rowmask are contiguous: zeroed together
   s.rowmask = p; p += TPC_TT * 8u;
   s.rowpre = p; p += TPC_TT + 2u;
-  s.misc = p; p += 8;
+  s.misc = p; p += 16;
   s.peaks = (u16*)p;
   return s;
 }
@@ -851,7 +853,7 @@ __device__ __forceinline__ u32 k6_stage(const K6Smem& s, const K6Args& a, u64 ib
     }
     pos += __shfl_sync(0xFFFFFFFFu, inc, 31);
   }
-  if (lane == 0u) { s.misc[2] = pos; mbar_arrive(&s.bar[0]); }
+  if (lane == 0u) { s.misc[8] = 0u; s.misc[9] = pos; mbar_arrive(&s.bar[0]); }
   return pos;
 }
 
@@ -873,46 +875,71 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
 
   if (tid >= TPC_K6_CONSUMERS) {
     // ---- producer warp -----------------------------------------------------------------------
-    // While the consumers work on tile k the producer already holds the index entries of tile
-    // k+1 and has asked L2 for its runs, so that once the buffer is released the bulk copies
-    // start at once and hit L2.
+    // A ticket = up to TPC_K6_GROUP consecutive slabs of one bin, handed out in increasing order.
+    // Small tiles (sparse frames) are staged together, one bulk copy per run and one barrier
+    // phase for the whole group, so that the staging latency is paid once per group; a tile
+    // that does not fit is staged alone, in as many rounds as it needs.  The loads for a stage
+    // (ticket, batch table, index entries, L2 prefetch of the runs) are issued before the wait
+    // for the buffer, i.e. while the consumers still work on the stage before.
     u32 ph = 1u;   // a fresh barrier passes a wait on parity 1: the buffer starts out free
     const u32 lane = lane_id();
-    u64 ib = 0ull, e0 = 0ull;
-    u32 nbatch = 0u;
-    auto look_ahead = [&](u32 tile) {
-      const u32 b = tile / nsl, sl = tile - b * nsl;
-      const u32 bs0 = a.batch_start[b];
-      nbatch = a.batch_start[b + 1] - bs0;
-      ib = (u64)nsl * bs0 + (u64)sl * nbatch;
-      e0 = lane < nbatch ? a.idx[ib + lane] : 0ull;
-      const u32 bytes = (((u32)(e0 >> 40) + 3u) >> 2) * 16u;
-      if (bytes != 0u)
-        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(a.blob + (e0 & ((1ull << 40) - 1ull))), "r"(bytes) : "memory");
-    };
-    auto take = [&]() -> u32 {   // next tile, in increasing order over the whole grid
+    const u32 gpb = (nsl + TPC_K6_GROUP - 1u) / TPC_K6_GROUP, n_tickets = nb * gpb;
+    for (;;) {
       u32 t = 0u;
       if (lane == 0u) t = atomicAdd(a.ticket, 1u);
-      return __shfl_sync(0xFFFFFFFFu, t, 0);
-    };
-    u32 tile = take();
-    if (tile < n_tiles) look_ahead(tile);
-    while (tile < n_tiles) {
-      const u64 ib_c = ib, e0_c = e0;
-      const u32 nbatch_c = nbatch;
-      const u32 next = take();
-      mbar_wait_backoff(&s.bar[1], ph); ph ^= 1u;
-      if (lane == 0u) s.misc[3] = tile;   // published by the arrive in k6_stage
-      const u32 total = k6_stage(s, a, ib_c, nbatch_c, 0u, e0_c);
-      if (next < n_tiles) look_ahead(next);
-      for (u32 round = 1u; round * TPC_K6_CAPU < total; ++round) {
-        mbar_wait_backoff(&s.bar[1], ph); ph ^= 1u;
-        k6_stage(s, a, ib_c, nbatch_c, round, e0_c);
+      t = __shfl_sync(0xFFFFFFFFu, t, 0);
+      if (t >= n_tickets) break;
+      const u32 b = t / gpb, sl0 = (t - b * gpb) * TPC_K6_GROUP;
+      const u32 cnt = nsl - sl0 < TPC_K6_GROUP ? nsl - sl0 : TPC_K6_GROUP;
+      const u32 bs0 = a.batch_start[b];
+      const u32 nbatch = a.batch_start[b + 1] - bs0;
+      const u64 ib0 = (u64)nsl * bs0 + (u64)sl0 * nbatch;
+      const u32 tile0 = b * nsl + sl0;
+      bool grouped = false;
+      u64 e = 0ull;
+      u32 units = 0u, inc = 0u;
+      const u32 m = lane >> 3, kb = lane & 7u;   // grouped: lane = (tile m of the group, batch kb)
+      if (nbatch <= 8u && cnt > 1u) {
+        if (m < cnt && kb < nbatch) e = a.idx[ib0 + (u64)m * nbatch + kb];
+        units = ((u32)(e >> 40) + 3u) >> 2;
+        inc = units;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { u32 o = __shfl_up_sync(0xFFFFFFFFu, inc, d); if ((int)lane >= d) inc += o; }
+        grouped = __shfl_sync(0xFFFFFFFFu, inc, 31) <= TPC_K6_CAPU;
       }
-      tile = next;
+      if (grouped) {
+        const u32 tot = __shfl_sync(0xFFFFFFFFu, inc, 31);
+        const void* src = a.blob + (e & ((1ull << 40) - 1ull));
+        if (units != 0u) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(units * 16u) : "memory");
+        const u32 off = inc - units;                                     // this run's place in rec
+        const u32 t_end = __shfl_sync(0xFFFFFFFFu, inc, (int)(lane | 7u));   // end of this tile's runs
+        const u32 t_beg = __shfl_sync(0xFFFFFFFFu, off, (int)(lane & ~7u));
+        mbar_wait_backoff(&s.bar[1], ph); ph ^= 1u;
+        if (kb == 0u && m < TPC_K6_GROUP) { s.misc[8u + 2u * m] = t_beg; s.misc[9u + 2u * m] = m < cnt ? t_end - t_beg : 0u; }
+        if (lane == 0u) { s.misc[3] = tile0; s.misc[4] = cnt; if (tot != 0u) mbar_expect_tx(&s.bar[0], tot * 16u); }
+        __syncwarp();
+        if (units != 0u) bulk_g2s(s.rec + off * 4u, src, units * 16u, &s.bar[0]);
+        __syncwarp();
+        if (lane == 0u) mbar_arrive(&s.bar[0]);
+      } else {
+        for (u32 k = 0u; k < cnt; ++k) {
+          const u64 ib = ib0 + (u64)k * nbatch;
+          const u64 e0 = lane < nbatch ? a.idx[ib + lane] : 0ull;
+          const u32 bytes = (((u32)(e0 >> 40) + 3u) >> 2) * 16u;
+          if (bytes != 0u)
+            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(a.blob + (e0 & ((1ull << 40) - 1ull))), "r"(bytes) : "memory");
+          mbar_wait_backoff(&s.bar[1], ph); ph ^= 1u;
+          if (lane == 0u) { s.misc[3] = tile0 + k; s.misc[4] = 1u; }   // published by the arrive in k6_stage
+          const u32 total = k6_stage(s, a, ib, nbatch, 0u, e0);
+          for (u32 round = 1u; round * TPC_K6_CAPU < total; ++round) {
+            mbar_wait_backoff(&s.bar[1], ph); ph ^= 1u;
+            k6_stage(s, a, ib, nbatch, round, e0);
+          }
+        }
+      }
     }
     mbar_wait_backoff(&s.bar[1], ph);   // tell the consumers there is nothing left
-    if (lane == 0u) { s.misc[3] = 0xFFFFFFFFu; s.misc[2] = 0u; mbar_arrive(&s.bar[0]); }
+    if (lane == 0u) { s.misc[3] = 0xFFFFFFFFu; s.misc[4] = 0u; mbar_arrive(&s.bar[0]); }
     return;
   }
 
@@ -930,12 +957,16 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
   zero_tile();
   for (;;) {
     mbar_wait(&s.bar[0], ph); ph ^= 1u;
-    const u32 tile = s.misc[3], total = s.misc[2];
-    if (tile == 0xFFFFFFFFu) break;   // block-uniform
+    const u32 tile0 = s.misc[3], ntl = s.misc[4];
+    if (tile0 == 0xFFFFFFFFu) break;   // block-uniform
+   for (u32 mt = 0u; mt < ntl; ++mt) {   // the tiles of this stage
+    const u32 tile = tile0 + mt, total = s.misc[9u + 2u * mt];
+    const u32* const rec = s.rec + s.misc[8u + 2u * mt] * 4u;
+    const bool last = mt + 1u == ntl;   // the staged records are released after the last tile's use of them
     const u32 b = tile / nsl, sl = tile - b * nsl;
     if (total == 0u) {   // block-uniform: nothing in this tile; the map stays zero
       __syncwarp();
-      if (lane_id() == 0u) mbar_arrive(&s.bar[1]);
+      if (last && lane_id() == 0u) mbar_arrive(&s.bar[1]);
       if (MODE == TPC_MODE_DET_TEMP && tid == 0) a.tile_cnt[tile] = 0u;
       if (MODE == TPC_MODE_DET && tid >= TPC_K6_CONSUMERS - 32u) {   // an empty tile is still a link of the chain
         const u64 ex = k6_chain(a.tile_state, tile, 0u);
@@ -947,15 +978,12 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
     const u32 row = sr % PRM(n_rows), sector = sr / PRM(n_rows);
     const u32 npads = PRM_NPADS(row);
     const int t_base = (int)(tc * TPC_TC + sl * TPC_TS) - (int)TPC_HALO;   // time of tile row 0
-#if defined(TPC_ABL) && TPC_ABL == 9
-    { for (u32 round = 0u;;) { __syncwarp(); if (lane_id() == 0u) mbar_arrive(&s.bar[1]); ++round; if (round * TPC_K6_CAPU >= total) break; mbar_wait(&s.bar[0], ph); ph ^= 1u; } continue; }
-#endif
     csync();   // A: the previous tile is done with the map, and the map is zero
     // ---- O0: scatter the tile's records ------------------------------------------------------
     for (u32 round = 0u;;) {
       u32 nu = total - round * TPC_K6_CAPU;
       if (nu > TPC_K6_CAPU) nu = TPC_K6_CAPU;
-      const uint4* r4 = (const uint4*)s.rec;
+      const uint4* r4 = (const uint4*)rec;
       for (u32 u = tid; u < nu; u += TPC_K6_CONSUMERS) {
         const uint4 v = r4[u];
         const u32 rr[4] = {v.x, v.y, v.z, v.w};
@@ -992,11 +1020,8 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
     }
     // a tile staged in one round (the usual case) keeps its records for the peak test below
     const bool sparse = total <= TPC_K6_CAPU && MODE != TPC_MODE_DUMP_MAP;
-    if (!sparse) { __syncwarp(); if (lane_id() == 0u) mbar_arrive(&s.bar[1]); }
+    if (!sparse) { __syncwarp(); if (last && lane_id() == 0u) mbar_arrive(&s.bar[1]); }
     csync();   // C: the map is complete
-#if defined(TPC_ABL) && TPC_ABL == 1
-    zero_tile(); continue;
-#endif
 
     if (MODE == TPC_MODE_DUMP_MAP) {
       const u64 sector_cells = a.row_off[PRM(n_rows)];
@@ -1020,7 +1045,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
     // one cell); the peaks of owned rows go into the list the later phases walk.
     if (sparse) {
       const u32 nW = pitch >> 1;
-      const uint4* r4 = (const uint4*)s.rec;
+      const uint4* r4 = (const uint4*)rec;
       for (u32 u = tid; u < total; u += TPC_K6_CONSUMERS) {
         const uint4 v = r4[u];
         const u32 rr[4] = {v.x, v.y, v.z, v.w};
@@ -1049,7 +1074,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
         }
       }
       __syncwarp();
-      if (lane_id() == 0u) mbar_arrive(&s.bar[1]);   // this warp is done with the staged records
+      if (last && lane_id() == 0u) mbar_arrive(&s.bar[1]);   // this warp is done with the staged records
     } else
     // ---- O1: 3x3 peaks, dense scan on packed u16x2 words ----------------------------------
     // A thread owns a group of 4 word columns (8 pads, one 128-bit load per row) of a strip of
@@ -1119,9 +1144,6 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
     }
     csync();   // D: peak set complete
     const u32 npk = s.misc[0];
-#if defined(TPC_ABL) && TPC_ABL == 2
-    zero_tile(); continue;
-#endif
 
     // ---- O2: suppression of the owned peaks against the un-updated peak set -----------------
     for (u32 i = tid; i < npk; i += TPC_K6_CONSUMERS) {
@@ -1167,9 +1189,6 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       if (!dead) atomicOr(&s.rowmask[tl * 8u + (pad >> 5)], 1u << (pad & 31u));
     }
     csync();   // F: survivor set complete
-#if defined(TPC_ABL) && TPC_ABL == 3
-    zero_tile(); continue;
-#endif
 
     // ---- rank (last warp) || O3 + O4 (everyone else first) ------------------------------------
     // rowpre[tl] = survivors in rows < tl, which ranks every cluster in (time, pad) order inside
@@ -1272,6 +1291,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       if (npk > TPC_K6_CONSUMERS) csync();   // block-uniform: the extra clusters still read the map
     }
     zero_tile();   // for the next tile (barrier A orders it before the scatter)
+   }
   }
 }
 
