@@ -356,3 +356,26 @@ def test_det_fallback_when_run_buffer_is_too_small(tp, cuda_device):
     c.run_sync(fr.digits.to(cuda_device), tp.MODE_DETERMINISTIC)
     assert not c.det_fallback()
     c.close()
+
+
+def test_order_and_build_invariance_at_scale(tp, cuda_device):
+    """I4 / I13 / I14 on a full-geometry frame (CFG[2], 1.1e8 digits): the deterministic output is
+    one byte string whatever the digit order (globally shuffled, readout-like, cell order),
+    whichever build (generic __constant__ / NVRTC literals) and however often it is run."""
+    import torch
+    ref = None
+    for order, rtc in (("shuffled", False), ("readout", False), ("cell", False), ("shuffled", True), ("shuffled", False)):
+        fr = make_frame(2, device=cuda_device, order=order)
+        c = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, fr.n_digits, rtc=rtc)
+        buf = torch.empty((fr.n_digits // 3, 32), dtype=torch.uint8, device=cuda_device)
+        _, nt, st = c.run(fr.digits, tp.MODE_DETERMINISTIC, clusters=buf)
+        torch.cuda.synchronize()
+        n = int(nt.item())
+        assert int(st.item()) == 0 and not c.det_fallback()
+        out = buf[:n].clone()
+        c.close()
+        del buf, fr
+        if ref is None:
+            ref = out
+        else:
+            assert out.shape == ref.shape and torch.equal(out, ref), (order, rtc)
