@@ -179,6 +179,15 @@ TPCCLUS_API int tpcclus_last_timing(tpcclus_handle* h, const char** names, float
 /* RTC build time in milliseconds (0 for non-RTC handles). */
 TPCCLUS_API double tpcclus_rtc_build_ms(const tpcclus_handle* h);
 
+/* On-disk cache of run-time-compiled kernels (section 5.1: processes of one node
+ * share one compilation, serialised by a file lock).  dir: HOST string, copied; NULL or "" turns
+ * the cache off again; if never called, $TPCCLUS_RTC_CACHE is used when set.  Process-wide, applies to
+ * handles created afterwards.  The key covers every baked parameter, the kernel text and the NVRTC
+ * version.  I/O errors are not errors: the handle is then compiled without caching. */
+TPCCLUS_API int tpcclus_set_rtc_cache_dir(const char* dir);
+/* 1 if this RTC handle's cubin came from the cache, else 0. */
+TPCCLUS_API int tpcclus_rtc_cache_hit(const tpcclus_handle* h);
+
 /* Debug/parity hook for step a1 (the charge map): after a run(), rebuilds the dense
  * [sector][row][time][pad] uint16 map (O0) from the binned digits into d_map (DEVICE,
  * n_sectors * n_time * sum(n_pads) entries).  Not on the hot path. */

@@ -54,7 +54,7 @@ _lib = None
 EXPORTS = ("tpcclus_workspace_bytes", "tpcclus_workspace_bytes_host", "tpcclus_create", "tpcclus_run",
            "tpcclus_run_host", "tpcclus_destroy", "tpcclus_error_string", "tpcclus_last_error",
            "tpcclus_launches_per_run", "tpcclus_set_timing", "tpcclus_last_timing", "tpcclus_rtc_build_ms",
-           "tpcclus_debug_dense_map", "tpcclus_debug_det_fallback")
+           "tpcclus_debug_dense_map", "tpcclus_debug_det_fallback", "tpcclus_set_rtc_cache_dir", "tpcclus_rtc_cache_hit")
 
 
 def lib() -> C.CDLL:
@@ -94,6 +94,10 @@ def lib() -> C.CDLL:
     L.tpcclus_rtc_build_ms.argtypes = [C.c_void_p]
     L.tpcclus_debug_dense_map.restype = C.c_int
     L.tpcclus_debug_dense_map.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    L.tpcclus_set_rtc_cache_dir.restype = C.c_int
+    L.tpcclus_set_rtc_cache_dir.argtypes = [C.c_char_p]
+    L.tpcclus_rtc_cache_hit.restype = C.c_int
+    L.tpcclus_rtc_cache_hit.argtypes = [C.c_void_p]
     L.tpcclus_debug_det_fallback.restype = C.c_int
     L.tpcclus_debug_det_fallback.argtypes = [C.c_void_p]
     _lib = L
@@ -131,6 +135,10 @@ def tpcclus_run(handle, d_digits_ptr, n, out: tpcclus_out, mode, stream_ptr) -> 
     rc = lib().tpcclus_run(handle, C.c_void_p(d_digits_ptr), int(n), C.byref(out), int(mode), C.c_void_p(stream_ptr))
     if rc != 0:
         raise TpcclusError(rc, "tpcclus_run", (lib().tpcclus_last_error(handle) or b"").decode())
+
+
+def tpcclus_set_rtc_cache_dir(path) -> None:
+    lib().tpcclus_set_rtc_cache_dir(None if path is None else os.fsencode(path))
 
 
 def tpcclus_destroy(handle) -> None:
@@ -225,6 +233,10 @@ class Clusterizer:
     @property
     def rtc_build_ms(self):
         return float(lib().tpcclus_rtc_build_ms(self._h))
+
+    @property
+    def rtc_cache_hit(self):
+        return int(lib().tpcclus_rtc_cache_hit(self._h)) == 1
 
     def dense_map(self, stream=None):
         """Debug hook (step a1): the O0 map of the last run as a flat uint16 CUDA tensor in

@@ -8,6 +8,9 @@
 // would compute returns TPCCLUS_ERR_CUDA.
 #include <cuda_runtime.h>
 #include <dlfcn.h>
+#include <fcntl.h>
+#include <sys/file.h>
+#include <unistd.h>
 
 #include <chrono>
 #include <cstdio>
@@ -153,6 +156,7 @@ struct Rtc {
   int (*nvrtcGetProgramLogSize)(void*, size_t*) = nullptr;
   int (*nvrtcGetProgramLog)(void*, char*) = nullptr;
   int (*nvrtcDestroyProgram)(void**) = nullptr;
+  int (*nvrtcVersion)(int*, int*) = nullptr;
   bool ok = false;
   std::string why;
 };
@@ -177,7 +181,7 @@ Rtc& rtc() {
   SYM(libcuda, cuFuncSetAttribute); SYM(libcuda, cuLaunchKernel); SYM(libcuda, cuGetErrorString);
   SYM(libnvrtc, nvrtcCreateProgram); SYM(libnvrtc, nvrtcCompileProgram); SYM(libnvrtc, nvrtcGetCUBINSize);
   SYM(libnvrtc, nvrtcGetCUBIN); SYM(libnvrtc, nvrtcGetProgramLogSize); SYM(libnvrtc, nvrtcGetProgramLog);
-  SYM(libnvrtc, nvrtcDestroyProgram);
+  SYM(libnvrtc, nvrtcDestroyProgram); SYM(libnvrtc, nvrtcVersion);
 #undef SYM
   r.ok = all;
   return r;
@@ -205,6 +209,7 @@ struct tpcclus_handle {
   void* module = nullptr;
   void* fn[K_COUNT_] = {};
   double rtc_ms = 0.0;
+  bool rtc_cache_hit = false;
   uint32_t smem_k1 = 0, smem_k5 = 0, smem_k6 = 0;
   uint32_t grid_k5 = 0, grid_k6 = 0;
   bool timing = false;
@@ -261,11 +266,9 @@ std::string rtc_prologue(const TpcParams& q) {
   return s;
 }
 
-int build_rtc(tpcclus_handle* h) {
+// NVRTC: kernel text -> cubin for sm_100a.
+int compile_cubin(const std::string& src, std::vector<char>* cubin) {
   Rtc& r = rtc();
-  if (!r.ok) return fail(nullptr, TPCCLUS_ERR_NVRTC, "RTC unavailable: " + r.why);
-  auto t0 = std::chrono::steady_clock::now();
-  std::string src = rtc_prologue(h->g.prm) + tpcclus_kernel_source;
   void* prog = nullptr;
   if (r.nvrtcCreateProgram(&prog, src.c_str(), "tpcclus_kernels.cu", 0, nullptr, nullptr) != 0)
     return fail(nullptr, TPCCLUS_ERR_NVRTC, "nvrtcCreateProgram failed");
@@ -286,9 +289,74 @@ int build_rtc(tpcclus_handle* h) {
     return fail(nullptr, TPCCLUS_ERR_NVRTC, "nvrtcCompileProgram failed:\n" + log);
   }
   size_t n = 0; r.nvrtcGetCUBINSize(prog, &n);
-  std::vector<char> cubin(n);
-  r.nvrtcGetCUBIN(prog, cubin.data());
+  cubin->resize(n);
+  r.nvrtcGetCUBIN(prog, cubin->data());
   r.nvrtcDestroyProgram(&prog);
+  return TPCCLUS_OK;
+}
+
+// On-disk cubin cache (PAPER.md 97: several processes per node share one run-time compilation,
+// serialised by a file lock).  Key = hash of the exact text handed to NVRTC (prologue with every
+// baked parameter + kernel source) and of the NVRTC version.  The compile happens under an
+// exclusive flock on <key>.lock; the cubin is written to a temporary name and renamed, so a
+// reader sees a whole file or none.  Any I/O problem just means "compile, do not cache".
+std::string g_cache_dir;   // set by tpcclus_set_rtc_cache_dir or $TPCCLUS_RTC_CACHE
+
+bool read_file(const std::string& path, std::vector<char>* out) {
+  FILE* f = fopen(path.c_str(), "rb");
+  if (!f) return false;
+  fseek(f, 0, SEEK_END);
+  long n = ftell(f);
+  fseek(f, 0, SEEK_SET);
+  bool ok = n > 0;
+  if (ok) { out->resize((size_t)n); ok = fread(out->data(), 1, (size_t)n, f) == (size_t)n; }
+  fclose(f);
+  return ok;
+}
+
+int cubin_for(const std::string& src, std::vector<char>* cubin, bool* hit) {
+  *hit = false;
+  std::string dir = g_cache_dir;
+  if (dir.empty()) { const char* e = getenv("TPCCLUS_RTC_CACHE"); if (e) dir = e; }
+  if (dir.empty()) return compile_cubin(src, cubin);
+  int vmaj = 0, vmin = 0;
+  if (rtc().nvrtcVersion) rtc().nvrtcVersion(&vmaj, &vmin);
+  uint64_t hsh = 1469598103934665603ull;   // FNV-1a
+  auto mix = [&](const char* p, size_t n) { for (size_t i = 0; i < n; ++i) { hsh ^= (unsigned char)p[i]; hsh *= 1099511628211ull; } };
+  mix(src.data(), src.size());
+  char tag[64]; snprintf(tag, sizeof tag, "|nvrtc %d.%d|sm_100a", vmaj, vmin); mix(tag, strlen(tag));
+  char name[64]; snprintf(name, sizeof name, "/tpcclus_%016llx", (unsigned long long)hsh);
+  const std::string base = dir + name, file = base + ".cubin", lock = base + ".lock";
+  if (read_file(file, cubin)) { *hit = true; return TPCCLUS_OK; }
+  int fd = open(lock.c_str(), O_CREAT | O_RDWR, 0644);
+  if (fd >= 0) flock(fd, LOCK_EX);   // whoever comes second waits here, then finds the file
+  int rc = TPCCLUS_OK;
+  if (fd >= 0 && read_file(file, cubin)) {
+    *hit = true;
+  } else {
+    rc = compile_cubin(src, cubin);
+    if (rc == TPCCLUS_OK && fd >= 0) {
+      char tmp[64]; snprintf(tmp, sizeof tmp, ".tmp%d", (int)getpid());
+      FILE* f = fopen((file + tmp).c_str(), "wb");
+      if (f) {
+        bool ok = fwrite(cubin->data(), 1, cubin->size(), f) == cubin->size();
+        ok = fclose(f) == 0 && ok;
+        if (ok) rename((file + tmp).c_str(), file.c_str()); else remove((file + tmp).c_str());
+      }
+    }
+  }
+  if (fd >= 0) { flock(fd, LOCK_UN); close(fd); }
+  return rc;
+}
+
+int build_rtc(tpcclus_handle* h) {
+  Rtc& r = rtc();
+  if (!r.ok) return fail(nullptr, TPCCLUS_ERR_NVRTC, "RTC unavailable: " + r.why);
+  auto t0 = std::chrono::steady_clock::now();
+  std::string src = rtc_prologue(h->g.prm) + tpcclus_kernel_source;
+  std::vector<char> cubin;
+  int rc = cubin_for(src, &cubin, &h->rtc_cache_hit);
+  if (rc != TPCCLUS_OK) return rc;
   if (cudaFree(nullptr) != cudaSuccess) { cudaGetLastError(); return fail(nullptr, TPCCLUS_ERR_CUDA, "no CUDA context"); }
   if ((rc = r.cuModuleLoadData(&h->module, cubin.data())) != 0) {
     const char* s = nullptr; r.cuGetErrorString(rc, &s);
@@ -411,6 +479,13 @@ int tpcclus_last_timing(tpcclus_handle* h, const char** names, float* ms, int ca
 }
 
 double tpcclus_rtc_build_ms(const tpcclus_handle* h) { return h ? h->rtc_ms : 0.0; }
+
+int tpcclus_rtc_cache_hit(const tpcclus_handle* h) { return h && h->rtc_cache_hit ? 1 : 0; }
+
+int tpcclus_set_rtc_cache_dir(const char* dir) {
+  g_cache_dir = dir ? dir : "";
+  return TPCCLUS_OK;
+}
 
 }  // extern "C"
 

@@ -379,3 +379,48 @@ def test_order_and_build_invariance_at_scale(tp, cuda_device):
             ref = out
         else:
             assert out.shape == ref.shape and torch.equal(out, ref), (order, rtc)
+
+
+def _rtc_child(cache_dir, q):
+    import paper_2511_17018_b200 as tp
+    import torch
+    tp.tpcclus_set_rtc_cache_dir(cache_dir)
+    fr = make_frame(1)
+    c = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, fr.n_digits, rtc=True)
+    det = c.run_sync(fr.digits.to("cuda:0"), tp.MODE_DETERMINISTIC)[0].tobytes()
+    q.put((c.rtc_cache_hit, c.rtc_build_ms, det))
+    c.close()
+
+
+def test_rtc_cubin_cache(tp, cuda_device, tmp_path):
+    """PAPER.md 97: processes of one node share a run-time compilation through a file lock.  Two
+    processes started together on an empty cache: exactly one compiles, the other waits and loads;
+    a third handle hits the cache outright; a different parameter set is a different key; results
+    never change."""
+    import multiprocessing as mp
+    fr = make_frame(1)
+    exp, _ = _oracle(fr.digits_numpy(), fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads)
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    ps = [ctx.Process(target=_rtc_child, args=(str(tmp_path), q)) for _ in range(2)]
+    for p in ps:
+        p.start()
+    res = [q.get(timeout=300) for _ in ps]
+    for p in ps:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert sorted(r[0] for r in res) == [False, True]            # one compiled, one loaded
+    assert all(r[2] == exp.tobytes() for r in res)
+    assert len(list(tmp_path.glob("tpcclus_*.cubin"))) == 1
+    tp.tpcclus_set_rtc_cache_dir(str(tmp_path))
+    try:
+        c = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, fr.n_digits, rtc=True)
+        assert c.rtc_cache_hit and c.rtc_build_ms < max(r[1] for r in res)
+        assert c.run_sync(fr.digits.to(cuda_device), tp.MODE_DETERMINISTIC)[0].tobytes() == exp.tobytes()
+        c.close()
+        c = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, fr.n_digits, thr_peak=9, rtc=True)
+        assert not c.rtc_cache_hit                                # thresholds are baked in: another key
+        c.close()
+        assert len(list(tmp_path.glob("tpcclus_*.cubin"))) == 2
+    finally:
+        tp.tpcclus_set_rtc_cache_dir(None)
