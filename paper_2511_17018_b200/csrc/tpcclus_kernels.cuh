@@ -715,7 +715,9 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
 #define TPC_K6_THREADS (TPC_K6_CONSUMERS + 32u)  // + the producer warp
 #define TPC_K6_CAP 4096u                         // records staged per round (16 KB)
 #define TPC_K6_CAPU (TPC_K6_CAP / 4u)            // ... in 16-byte units
+#ifndef TPC_K6_CTAS
 #define TPC_K6_CTAS 3                            // resident CTAs per SM (shared memory and registers)
+#endif
 
 struct K6Args {
   const u32* blob; const u64* idx; const u32* batch_start;
