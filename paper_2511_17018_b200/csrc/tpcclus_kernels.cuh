@@ -1247,16 +1247,20 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       rk = __popc(mword & ((1u << bitpos) - 1u));
       for (u32 k = 0; k < w; ++k) rk += __popc(s.rowmask[tl * 8u + k]);
       const u16* c = s.tile + tl * pitch + pad + TPC_HALO;
+      // exact integer sums (Q12): per-row partial sums first, so the 25 loads and the adds of
+      // different rows are independent (short dependency chains; any order gives the same bits)
       u32 Q = 0u, Spp = 0u, Stt = 0u;
       int Sp = 0, St = 0;
 #pragma unroll
-      for (int dt = -2; dt <= 2; ++dt)
-#pragma unroll
-        for (int dp = -2; dp <= 2; ++dp) {
-          const u32 q = c[dt * (int)pitch + dp];
-          Q += q; Sp += (int)q * dp; St += (int)q * dt;
-          Spp += q * (u32)(dp * dp); Stt += q * (u32)(dt * dt);
-        }
+      for (int dt = -2; dt <= 2; ++dt) {
+        const u16* cr = c + dt * (int)pitch;
+        const u32 a = cr[-2], b = cr[-1], m = cr[0], d = cr[1], e2 = cr[2];
+        const u32 rq = (a + b) + (m + d) + e2;
+        const int rsp = (int)(2u * e2 + d) - (int)(2u * a + b);
+        const u32 rspp = 4u * (a + e2) + (b + d);
+        Q += rq; Sp += rsp; Spp += rspp;
+        St += (int)rq * dt; Stt += rq * (u32)(dt * dt);
+      }
       const int Vp = (int)(Q * Spp) - Sp * Sp, Vt = (int)(Q * Stt) - St * St;
       const u32 qc = c[0];
       const int t = t_base + (int)tl;
