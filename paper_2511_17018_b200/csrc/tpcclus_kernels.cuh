@@ -779,7 +779,8 @@ struct K6Smem {
   u32* rowmask;    // [TT][8]  O2 survivors, bit = pad
   u32* rowpre; u32* misc; u16* peaks;
 };
-// misc: [0] n_peaks  [3] first tile of the stage  [4] tiles in the stage  [8+2m],[9+2m] offset and
+// misc: [0] n_peaks  [3] first tile of the stage  [4] tiles in the stage  [5] row | sector << 8 |
+//       n_pads << 16  [6] time of row 0 of the first tile  [8+2m],[9+2m] offset and
 //       size (16-byte units) of tile m's records in `rec`
 #define TPC_K6_GROUP 4u   // tiles (consecutive slabs of one bin) a ticket covers
 #define TPC_K6_PMW 9u
@@ -897,6 +898,10 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       const u32 nbatch = a.batch_start[b + 1] - bs0;
       const u64 ib0 = (u64)nsl * bs0 + (u64)sl0 * nbatch;
       const u32 tile0 = b * nsl + sl0;
+      const u32 tc = b % PRM(n_tc), sr = b / PRM(n_tc);
+      const u32 row = sr % PRM(n_rows), sector = sr / PRM(n_rows);
+      const u32 geo = row | (sector << 8) | ((u32)PRM_NPADS(row) << 16);
+      const int t0 = (int)(tc * TPC_TC + sl0 * TPC_TS) - (int)TPC_HALO;   // time of row 0 of the first tile
       bool grouped = false;
       u64 e = 0ull;
       u32 units = 0u, inc = 0u;
@@ -918,7 +923,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
         const u32 t_beg = __shfl_sync(0xFFFFFFFFu, off, (int)(lane & ~7u));
         mbar_wait_backoff(&s.bar[1], ph); ph ^= 1u;
         if (kb == 0u && m < TPC_K6_GROUP) { s.misc[8u + 2u * m] = t_beg; s.misc[9u + 2u * m] = m < cnt ? t_end - t_beg : 0u; }
-        if (lane == 0u) { s.misc[3] = tile0; s.misc[4] = cnt; if (tot != 0u) mbar_expect_tx(&s.bar[0], tot * 16u); }
+        if (lane == 0u) { s.misc[3] = tile0; s.misc[4] = cnt; s.misc[5] = geo; s.misc[6] = (u32)t0; if (tot != 0u) mbar_expect_tx(&s.bar[0], tot * 16u); }
         __syncwarp();
         if (units != 0u) bulk_g2s(s.rec + off * 4u, src, units * 16u, &s.bar[0]);
         __syncwarp();
@@ -931,7 +936,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
           if (bytes != 0u)
             asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(a.blob + (e0 & ((1ull << 40) - 1ull))), "r"(bytes) : "memory");
           mbar_wait_backoff(&s.bar[1], ph); ph ^= 1u;
-          if (lane == 0u) { s.misc[3] = tile0 + k; s.misc[4] = 1u; }   // published by the arrive in k6_stage
+          if (lane == 0u) { s.misc[3] = tile0 + k; s.misc[4] = 1u; s.misc[5] = geo; s.misc[6] = (u32)(t0 + (int)(k * TPC_TS)); }   // published by the arrive in k6_stage
           const u32 total = k6_stage(s, a, ib, nbatch, 0u, e0);
           for (u32 round = 1u; round * TPC_K6_CAPU < total; ++round) {
             mbar_wait_backoff(&s.bar[1], ph); ph ^= 1u;
@@ -965,7 +970,6 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
     const u32 tile = tile0 + mt, total = s.misc[9u + 2u * mt];
     const u32* const rec = s.rec + s.misc[8u + 2u * mt] * 4u;
     const bool last = mt + 1u == ntl;   // the staged records are released after the last tile's use of them
-    const u32 b = tile / nsl, sl = tile - b * nsl;
     if (total == 0u) {   // block-uniform: nothing in this tile; the map stays zero
       __syncwarp();
       if (last && lane_id() == 0u) mbar_arrive(&s.bar[1]);
@@ -976,10 +980,10 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       }
       continue;
     }
-    const u32 tc = b % PRM(n_tc), sr = b / PRM(n_tc);
-    const u32 row = sr % PRM(n_rows), sector = sr / PRM(n_rows);
-    const u32 npads = PRM_NPADS(row);
-    const int t_base = (int)(tc * TPC_TC + sl * TPC_TS) - (int)TPC_HALO;   // time of tile row 0
+    // the producer (which has the time for the divisions) decoded the tile: all tiles of a stage share the bin
+    const u32 geo = s.misc[5];
+    const u32 row = geo & 0xFFu, sector = (geo >> 8) & 0xFFu, npads = geo >> 16;
+    const int t_base = (int)s.misc[6] + (int)(mt * TPC_TS);   // time of tile row 0
     csync();   // A: the previous tile is done with the map, and the map is zero
     // ---- O0: scatter the tile's records ------------------------------------------------------
     for (u32 round = 0u;;) {
