@@ -763,6 +763,12 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, u32 bytes, 
 __device__ __forceinline__ u32 vmax2(u32 a, u32 b) { u32 d; asm("max.u16x2 %0, %1, %2;" : "=r"(d) : "r"(a), "r"(b)); return d; }
 // barrier 1 = the consumer threads only (the producer warp never joins it)
 __device__ __forceinline__ void csync() { asm volatile("bar.sync 1, %0;" ::"n"(TPC_K6_CONSUMERS) : "memory"); }
+__device__ __forceinline__ u32 csync_popc(bool v) {   // barrier + number of threads with v set
+  u32 r;
+  asm volatile("{\n.reg .pred p;\nsetp.ne.u32 p, %1, 0;\nbar.red.popc.u32 %0, 1, %2, p;\n}"
+               : "=r"(r) : "r"((u32)v), "n"(TPC_K6_CONSUMERS) : "memory");
+  return r;
+}
 __device__ __forceinline__ u32 csync_or(u32 v) {
   u32 r;
   asm volatile("{\n.reg .pred p, q;\nsetp.ne.u32 p, %1, 0;\nbar.red.or.pred q, 1, %2, p;\nselp.u32 %0, 1, 0, q;\n}"
@@ -1158,6 +1164,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
     const u32 npk = s.misc[0];
 
     // ---- O2: suppression of the owned peaks against the un-updated peak set -----------------
+    bool survived = false;
     for (u32 i = tid; i < npk; i += TPC_K6_CONSUMERS) {
       const u32 e = s.peaks[i];
       const u32 tl = e >> 8, pad = e & 0xFFu;
@@ -1198,9 +1205,12 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
               }
           }
       }
-      if (!dead) atomicOr(&s.rowmask[tl * 8u + (pad >> 5)], 1u << (pad & 31u));
+      if (!dead) { atomicOr(&s.rowmask[tl * 8u + (pad >> 5)], 1u << (pad & 31u)); survived = true; }
     }
-    csync();   // F: survivor set complete
+    // F: survivor set complete.  With at most one peak per thread (the usual case) the barrier
+    // itself counts the survivors, so the tile's base can be requested before the rank scan.
+    const u32 fcount = csync_popc(survived);
+    const bool early = npk <= TPC_K6_CONSUMERS;   // block-uniform
 
     // ---- rank (last warp) || O3 + O4 (everyone else first) ------------------------------------
     // rowpre[tl] = survivors in rows < tl, which ranks every cluster in (time, pad) order inside
@@ -1209,6 +1219,11 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
     // results meet at barrier G.
     if (tid >= TPC_K6_CONSUMERS - 32u) {
       const u32 lane = lane_id();
+      u64 at = 0ull;   // FAST / DET_TEMP: the tile's place, one global atomic (in flight during the scan below)
+      if (early && lane == 31u) {
+        if (MODE == TPC_MODE_FAST) at = atomicAdd(a.n_clusters, (u64)fcount);
+        if (MODE == TPC_MODE_DET_TEMP) at = atomicAdd(a.temp_cursor, (u64)fcount);
+      }
       u32 cnt[5], t = 0u;
 #pragma unroll
       for (int k = 0; k < 5; ++k) {
@@ -1227,10 +1242,10 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
 #pragma unroll
       for (int k = 0; k < 5; ++k) { const u32 tl = lane * 5u + (u32)k; if (tl < TPC_TT) s.rowpre[tl] = ex; ex += cnt[k]; }
       const u32 count = __shfl_sync(0xFFFFFFFFu, inc, 31);
-      if (MODE == TPC_MODE_FAST) { if (lane == 31u) s.base[0] = atomicAdd(a.n_clusters, (u64)count); }
+      if (MODE == TPC_MODE_FAST) { if (lane == 31u) s.base[0] = early ? at : atomicAdd(a.n_clusters, (u64)count); }
       if (MODE == TPC_MODE_DET_TEMP) {
         if (lane == 31u) {
-          const u64 at = atomicAdd(a.temp_cursor, (u64)count);
+          if (!early) at = atomicAdd(a.temp_cursor, (u64)count);
           a.tile_base[tile] = at; a.tile_cnt[tile] = count; s.base[0] = at;
           if (at + count > a.temp_cap) atomicOr(a.det_flag, 1u);
         }
