@@ -289,13 +289,6 @@ def main():
                                    "kernel_ms": avg[nm], "share_of_step": avg[nm] / step_sum}
     dom = max(per_kernel_roof, key=lambda nm: avg[nm]) if per_kernel_roof else None
     roof = dict(per_kernel_roof[dom], peak_source=peak_src) if dom else None
-    # what actually bounds K1/K5: one shared-memory atomic per record, 1 lane per clock and SM
-    # (DESIGN.md section 6): floor = records / (SMs x SM clock)
-    sm_clk = (clk.summary()["sm_mhz"] or 1965.0) * 1e6
-    n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
-    lsu = {nm: {"bound": "lsu-atomics", "floor_ms": n / (n_sm * sm_clk) * 1e3, "kernel_ms": avg[nm],
-                "frac": n / (n_sm * sm_clk) * 1e3 / avg[nm]}
-           for nm in ("k_partition_coarse", "k_partition_fine") if nm in avg}
     b_alg = 8 * n + 32 * n_clusters
     method = {"b_alg_bytes": b_alg, "achieved_gbs": b_alg / (ms_step * 1e-3) / 1e9,
               "frac_of_peak": b_alg / (ms_step * 1e-3) / 1e9 / peak}
@@ -318,7 +311,7 @@ def main():
                    "n_digits": n, "n_clusters": n_clusters, "occupancy": fr.meta["occupancy"],
                    "checksum": "%016x" % fr.meta["checksum"], "l2": "inputs (%.1f GB) larger than L2" % (8 * n / 1e9)},
         "clocks": clk.summary(), "e2e": e2e, "gpu_launches": c.launches_per_run(mode) * args.steps,
-        "roofline": roof, "rooflines": per_kernel_roof, "lsu_rooflines": lsu, "method_roofline": method,
+        "roofline": roof, "rooflines": per_kernel_roof, "method_roofline": method,
         "kernels_ms": avg, "cpu_baseline": cpu,
     }
     print(json.dumps(out))
