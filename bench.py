@@ -39,9 +39,9 @@ def _log(msg):
 
 
 METRIC = "TPC clusterizer digits/s on Pb-Pb-like time frame"
-# ncu --set full, CFG[4] shuffled FAST generic, one launch each (profiles/r01c_ncu_full_summary.txt)
-NCU_TRAFFIC_BYTES = {"k_partition_coarse": 12766551000 + 6479542000, "k_partition_fine": 9145850000 + 7143103000,
-                     "k_cluster_tiles_fast": 7338236000 + 1902622000}
+# ncu --set full, CFG[4] shuffled FAST generic, one launch each (profiles/r01d_ncu_full_summary.txt)
+NCU_TRAFFIC_BYTES = {"k_partition_coarse": 12764779000 + 6478431000, "k_partition_fine": 9146624000 + 7140715000,
+                     "k_cluster_tiles_fast": 7184330000 + 1901887000}
 UNIT = "digits/s"
 
 
@@ -277,7 +277,7 @@ def main():
         "k_cluster_tiles_det_emit": 4 * n + 32 * n_clusters,
     }
     # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full`
-    # capture of this very workload (profiles/r01c_README.md); null for any other workload
+    # capture of this very workload (profiles/r01d_README.md); null for any other workload
     traffic = NCU_TRAFFIC_BYTES if (k == 4 and args.order == "shuffled" and not args.rtc) else {}
     step_sum = sum(avg.values())
     per_kernel_roof = {}
