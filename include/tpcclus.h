@@ -87,7 +87,9 @@ enum {
   TPCCLUS_STATUS_OVERFLOW = 1,  /* more clusters than out->capacity; *n_clusters is still the
                                    true total, the buffer holds `capacity` valid records (FAST:
                                    any subset; DETERMINISTIC: the first `capacity` in order) */
-  TPCCLUS_STATUS_BAD_DIGITS = 2 /* at least one digit was out of range and ignored */
+  TPCCLUS_STATUS_BAD_DIGITS = 2, /* at least one digit was out of range and ignored */
+  TPCCLUS_STATUS_NO_PACKED = 4   /* tpcclus_run_packed only: the frame has more clusters than the run
+                                    buffer holds (max_digits / 8); nothing was written but *n_clusters */
 };
 
 /* return codes */
@@ -97,7 +99,8 @@ enum {
   TPCCLUS_ERR_CUDA = -2,
   TPCCLUS_ERR_NVRTC = -3,
   TPCCLUS_ERR_WORKSPACE_TOO_SMALL = -4,
-  TPCCLUS_ERR_UNSUPPORTED_GEOMETRY = -5 /* n_sectors*n_rows*ceil(n_time/16256) > 5632 coarse bins */
+  TPCCLUS_ERR_UNSUPPORTED_GEOMETRY = -5 /* more than 5503 coarse bins n_sectors*n_rows*ceil(n_time/16256):
+                                           the first partition pass keeps 40 B of shared memory per bin */
 };
 
 typedef struct {
@@ -121,6 +124,33 @@ typedef struct {
   uint64_t* n_clusters;      /* DEVICE, caller-owned: true count, also on overflow           */
   uint32_t* status;          /* DEVICE, TPCCLUS_STATUS_* bits; may be NULL                   */
 } tpcclus_out;
+
+/* Packed native output: 16 bytes per cluster in fixed point, grouped by
+ * pad row, with an index of where each (sector,row) starts -- the form the steps after the
+ * clusterizer consume (PAPER.md 107 names them: coordinate transformation, error estimation).
+ * Sector and row are not stored per cluster: they follow from the index.  The record is a pure
+ * function (O6) of the 32-byte DETERMINISTIC record:
+ *   time_fix  = rn(time_mean  * 256)    24 bit     pad_fix       = min(rn(pad_mean * 256), 65535)
+ *   sigma_*_fix = rn(sigma_* * 16384)   16 bit     rn = float32 -> integer, round to nearest even
+ * (the multiplications by a power of two are exact), so it is bitwise reproducible as well. */
+typedef struct {
+  uint32_t time_fix_pad_peak;  /* time_fix[0:24) | pad_peak[24:32)                            */
+  uint16_t pad_fix;
+  uint16_t time_peak;
+  uint16_t q_tot;              /* <= 25575                                                    */
+  uint16_t q_max_flags;        /* q_max[0:10) | flags[10:13)                                  */
+  uint16_t sigma_pad_fix;
+  uint16_t sigma_time_fix;
+} tpcclus_cluster16;
+
+typedef struct {
+  tpcclus_cluster16* clusters; /* DEVICE, caller-owned, 16-byte aligned                       */
+  uint64_t capacity;           /* in clusters                                                 */
+  uint64_t* n_clusters;        /* DEVICE: true count, also on overflow                        */
+  uint32_t* status;            /* DEVICE, TPCCLUS_STATUS_* bits; may be NULL                  */
+  uint64_t* row_index;         /* DEVICE, n_sectors * n_rows + 1 entries: clusters of (s, r) are
+                                  [row_index[s * n_rows + r], row_index[s * n_rows + r + 1])  */
+} tpcclus_out_packed;
 
 /* Bytes of device workspace a handle with these parameters needs (depends on the geometry
  * and max_digits only).  Returns 0 for invalid or unsupported parameters.  Host call. */
@@ -187,6 +217,14 @@ TPCCLUS_API double tpcclus_rtc_build_ms(const tpcclus_handle* h);
 TPCCLUS_API int tpcclus_set_rtc_cache_dir(const char* dir);
 /* 1 if this RTC handle's cubin came from the cache, else 0. */
 TPCCLUS_API int tpcclus_rtc_cache_hit(const tpcclus_handle* h);
+
+/* Same path as tpcclus_run in DETERMINISTIC mode (order, tie-breaks, arithmetic), output in the
+ * packed form above.  Clusters are in (sector,row,time_peak,pad_peak) order; on OVERFLOW the first
+ * `capacity` are kept and row_index still refers to the full list.  Needs the run buffer
+ * (clusters <= max_digits / 8, true for every frame but adversarial ones): otherwise
+ * TPCCLUS_STATUS_NO_PACKED is set and only *n_clusters is valid.  Enqueues only, like tpcclus_run. */
+TPCCLUS_API int tpcclus_run_packed(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n,
+                                   const tpcclus_out_packed* out, void* cuda_stream);
 
 /* Debug/parity hook for step a1 (the charge map): after a run(), rebuilds the dense
  * [sector][row][time][pad] uint16 map (O0) from the binned digits into d_map (DEVICE,
