@@ -165,7 +165,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--order", default="shuffled", choices=["shuffled", "readout", "cell"])
-    ap.add_argument("--mode", default="fast", choices=["fast", "det"])
+    ap.add_argument("--mode", default="fast", choices=["fast", "det", "packed"])
     ap.add_argument("--rtc", action="store_true")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -199,11 +199,17 @@ def main():
     torch.cuda.synchronize(dev)
     _log("frame generated: %d digits" % n)
     mode = tp.MODE_FAST if args.mode == "fast" else tp.MODE_DETERMINISTIC
+    packed = args.mode == "packed"   # deterministic path, 16-byte records + row index
     c = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, n, rtc=args.rtc, device=local)
     # size the output from a first (untimed) run
     probe_cap = max(n // 3, 1024)
-    clusters = torch.empty((probe_cap, 32), dtype=torch.uint8, device=dev)
-    _, nt, stt = c.run(digits, mode, clusters=clusters)
+    clusters = torch.empty((probe_cap, 16 if packed else 32), dtype=torch.uint8, device=dev)
+
+    def step():
+        if packed:
+            return c.run_packed(digits, clusters=clusters)[2:]
+        return c.run(digits, mode, clusters=clusters)[1:]
+    nt, stt = step()
     torch.cuda.synchronize(dev)
     n_clusters, status = int(nt.item()), int(stt.item())
     assert status == 0 and n_clusters <= probe_cap, (status, n_clusters, probe_cap)
@@ -214,7 +220,7 @@ def main():
         torch.cuda.synchronize(dev)
 
     for _ in range(max(args.warmup, 3)):
-        c.run(digits, mode, clusters=clusters)
+        step()
     c.set_timing(True)
     per_kernel = {}
     barrier()
@@ -222,7 +228,7 @@ def main():
     with ClockSampler(local) as clk:
         e0.record()
         for _ in range(args.steps):
-            c.run(digits, mode, clusters=clusters)
+            step()
             for nm, ms in c.last_timing():      # events recorded on the run's stream, inside the timed region
                 per_kernel.setdefault(nm, []).append(ms)
         e1.record()
@@ -236,7 +242,7 @@ def main():
 
     # ---- e2e: host buffers through tpcclus_run_host, copies inside the timed region -----------
     e2e = None
-    if args.e2e_steps > 0:
+    if args.e2e_steps > 0 and not packed:
         cap = n_clusters + 1024
         c.close()
         del c, clusters
@@ -273,8 +279,9 @@ def main():
         "k_partition_coarse": 8 * n + 4 * n,                    # read every digit once, write one 4-byte record
         "k_partition_fine": 4 * n + 4 * n,                      # read the records, write them tile-sorted
         "k_cluster_tiles_fast": 4 * n + 32 * n_clusters,        # read the tile records, write the clusters
-        "k_cluster_tiles_det_count": 4 * n,
-        "k_cluster_tiles_det_emit": 4 * n + 32 * n_clusters,
+        "k_cluster_tiles_det_temp": 4 * n + 32 * n_clusters,     # ... as runs into the temporary buffer
+        "k_emit_ordered": 64 * n_clusters,                       # DET: ordered copy of the runs
+        "k_emit_packed": 48 * n_clusters,                        # packed: 32 B in, 16 B out
     }
     # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full`
     # capture of this very workload (profiles/r01d_README.md); null for any other workload

@@ -18,7 +18,7 @@ _LIB_PATH = os.path.join(_HERE, "libtpcclus.so")
 
 MODE_FAST, MODE_DETERMINISTIC = 0, 1
 RTC = 1
-STATUS_OVERFLOW, STATUS_BAD_DIGITS = 1, 2
+STATUS_OVERFLOW, STATUS_BAD_DIGITS, STATUS_NO_PACKED = 1, 2, 4
 FLAG_EDGE_PAD, FLAG_EDGE_TIME, FLAG_SATURATED = 1, 2, 4
 
 # include/tpcclus.h: tpcclus_digit (8 B) and tpcclus_cluster (32 B)
@@ -27,7 +27,9 @@ DIGIT_DTYPE = np.dtype([("charge", "<u2"), ("time", "<u2"), ("pad", "u1"), ("row
 CLUSTER_DTYPE = np.dtype([("pad_mean", "<f4"), ("time_mean", "<f4"), ("sigma_pad", "<f4"), ("sigma_time", "<f4"),
                           ("q_tot", "<u4"), ("q_max", "<u2"), ("time_peak", "<u2"), ("pad_peak", "u1"),
                           ("row", "u1"), ("sector", "u1"), ("flags", "u1"), ("reserved", "<u4")])
-assert DIGIT_DTYPE.itemsize == 8 and CLUSTER_DTYPE.itemsize == 32
+CLUSTER16_DTYPE = np.dtype([("time_fix_pad_peak", "<u4"), ("pad_fix", "<u2"), ("time_peak", "<u2"), ("q_tot", "<u2"),
+                            ("q_max_flags", "<u2"), ("sigma_pad_fix", "<u2"), ("sigma_time_fix", "<u2")])
+assert DIGIT_DTYPE.itemsize == 8 and CLUSTER_DTYPE.itemsize == 32 and CLUSTER16_DTYPE.itemsize == 16
 
 
 class tpcclus_params(C.Structure):
@@ -42,6 +44,11 @@ class tpcclus_out(C.Structure):
                 ("status", C.c_void_p)]
 
 
+class tpcclus_out_packed(C.Structure):
+    _fields_ = [("clusters", C.c_void_p), ("capacity", C.c_uint64), ("n_clusters", C.c_void_p),
+                ("status", C.c_void_p), ("row_index", C.c_void_p)]
+
+
 class TpcclusError(RuntimeError):
     def __init__(self, code, what, detail=""):
         super().__init__("%s: %s (%d)%s" % (what, lib().tpcclus_error_string(code).decode(), code,
@@ -54,7 +61,7 @@ _lib = None
 EXPORTS = ("tpcclus_workspace_bytes", "tpcclus_workspace_bytes_host", "tpcclus_create", "tpcclus_run",
            "tpcclus_run_host", "tpcclus_destroy", "tpcclus_error_string", "tpcclus_last_error",
            "tpcclus_launches_per_run", "tpcclus_set_timing", "tpcclus_last_timing", "tpcclus_rtc_build_ms",
-           "tpcclus_debug_dense_map", "tpcclus_debug_det_fallback", "tpcclus_set_rtc_cache_dir", "tpcclus_rtc_cache_hit")
+           "tpcclus_debug_dense_map", "tpcclus_debug_det_fallback", "tpcclus_set_rtc_cache_dir", "tpcclus_rtc_cache_hit", "tpcclus_run_packed")
 
 
 def lib() -> C.CDLL:
@@ -75,6 +82,8 @@ def lib() -> C.CDLL:
     L.tpcclus_create.argtypes = [P(tpcclus_params), P(C.c_void_p)]
     L.tpcclus_run.restype = C.c_int
     L.tpcclus_run.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, P(tpcclus_out), C.c_int, C.c_void_p]
+    L.tpcclus_run_packed.restype = C.c_int
+    L.tpcclus_run_packed.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, P(tpcclus_out_packed), C.c_void_p]
     L.tpcclus_run_host.restype = C.c_int
     L.tpcclus_run_host.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p, C.c_uint64,
                                    P(C.c_uint64), P(C.c_uint32), C.c_int, C.c_void_p]
@@ -198,6 +207,24 @@ class Clusterizer:
         n_true, status = int(n.item()), int(st.item())
         m = min(n_true, cl.shape[0])
         return cl[:m].cpu().numpy().view(CLUSTER_DTYPE).reshape(-1), n_true, status
+
+    def run_packed(self, digits, clusters=None, capacity=None, stream=None):
+        """Deterministic path, packed output: (clusters uint8[cap,16], row_index int64[S*R+1],
+        n_clusters int64[1], status int32[1]); enqueues without synchronising."""
+        torch = self._torch
+        n = digits.numel() if digits.dtype == torch.int64 else digits.numel() // 8
+        assert digits.is_cuda and digits.is_contiguous()
+        if clusters is None:
+            cap = int(capacity if capacity is not None else max(n, 1))
+            clusters = torch.empty((cap, 16), dtype=torch.uint8, device=self.device)
+        ridx = torch.empty(self.n_sectors * self.n_rows + 1, dtype=torch.int64, device=self.device)
+        out = tpcclus_out_packed(clusters.data_ptr(), clusters.shape[0], self._n.data_ptr(), self._status.data_ptr(),
+                                 ridx.data_ptr())
+        st = (stream or torch.cuda.current_stream(self.device)).cuda_stream
+        rc = lib().tpcclus_run_packed(self._h, C.c_void_p(digits.data_ptr()), n, C.byref(out), C.c_void_p(st))
+        if rc != 0:
+            raise TpcclusError(rc, "tpcclus_run_packed", (lib().tpcclus_last_error(self._h) or b"").decode())
+        return clusters, ridx, self._n, self._status
 
     # -- host path (e2e) -----------------------------------------------------------------------
     def run_host(self, digits_host, clusters_host, mode=MODE_FAST, stream=None):

@@ -188,16 +188,16 @@ Rtc& rtc() {
 }
 
 enum KernelId { K_PART_COARSE, K_DIR_COUNT, K_DIR_SCAN, K_DIR_FILL, K_PART_FINE, K_TILES_FAST, K_TILES_DET,
-                K_TILES_DET_TEMP, K_TILES_DUMP, K_SCAN_LOCAL, K_SCAN_SUMS, K_EMIT_ORDERED, K_COUNT_ };
+                K_TILES_DET_TEMP, K_TILES_DUMP, K_SCAN_LOCAL, K_SCAN_SUMS, K_EMIT_ORDERED, K_EMIT_PACKED, K_COUNT_ };
 const char* const kKernelNames[K_COUNT_] = {
     "k_partition_coarse", "k_dir_count", "k_dir_scan", "k_dir_fill", "k_partition_fine", "k_cluster_tiles_fast",
     "k_cluster_tiles_det", "k_cluster_tiles_det_temp", "k_cluster_tiles_dump_map", "k_scan_local", "k_scan_sums",
-    "k_emit_ordered"};
+    "k_emit_ordered", "k_emit_packed"};
 const void* const kKernelPtrs[K_COUNT_] = {
     (const void*)k_partition_coarse, (const void*)k_dir_count, (const void*)k_dir_scan, (const void*)k_dir_fill,
     (const void*)k_partition_fine, (const void*)k_cluster_tiles_fast, (const void*)k_cluster_tiles_det,
     (const void*)k_cluster_tiles_det_temp, (const void*)k_cluster_tiles_dump_map, (const void*)k_scan_local,
-    (const void*)k_scan_sums, (const void*)k_emit_ordered};
+    (const void*)k_scan_sums, (const void*)k_emit_ordered, (const void*)k_emit_packed};
 
 }  // namespace
 
@@ -547,32 +547,37 @@ int enqueue_binning(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n
 
 extern "C" {
 
-int tpcclus_run(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n, const tpcclus_out* out, int mode,
-                void* cuda_stream) {
+// run() and run_packed(): `packed` != nullptr selects the packed output of the deterministic path.
+static int run_impl(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n, const tpcclus_out* out,
+                    const tpcclus_out_packed* packed, int mode, void* cuda_stream) {
   if (!h) return TPCCLUS_ERR_INVALID_ARG;
   h->err.clear();
-  if (!out || !out->n_clusters || (!out->clusters && out->capacity) || (!d_digits && n) || n > h->g.max_digits ||
+  void* o_clusters = packed ? (void*)packed->clusters : out ? (void*)out->clusters : nullptr;
+  const uint64_t o_capacity = packed ? packed->capacity : out ? out->capacity : 0;
+  uint64_t* o_n = packed ? packed->n_clusters : out ? out->n_clusters : nullptr;
+  uint32_t* o_status = packed ? packed->status : out ? out->status : nullptr;
+  if ((!out && !packed) || !o_n || (!o_clusters && o_capacity) || (!d_digits && n) || n > h->g.max_digits ||
       (mode != TPCCLUS_MODE_FAST && mode != TPCCLUS_MODE_DETERMINISTIC) || ((uintptr_t)d_digits & 15u) ||
-      ((uintptr_t)out->clusters & 15u) || ((uintptr_t)out->n_clusters & 7u))
+      ((uintptr_t)o_clusters & 15u) || ((uintptr_t)o_n & 7u) || (packed && (!packed->row_index || ((uintptr_t)packed->row_index & 7u))))
     return fail(h, TPCCLUS_ERR_INVALID_ARG, "tpcclus_run: bad argument");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   CUDA_TRY(h, cudaSetDevice(h->params.device));
   h->n_timed = 0;
   RunPtrs p = ptrs(h);
-  u32* status = out->status ? out->status : p.status;
+  u32* status = o_status ? o_status : p.status;
   int rc = enqueue_binning(h, d_digits, n, status, st);
   if (rc) return rc;
 
   K6Args a;
   a.blob = p.blob; a.idx = p.idx; a.batch_start = p.batch_start;
-  a.out = (uint4*)out->clusters; a.capacity = out->capacity; a.n_clusters = (u64*)out->n_clusters; a.status = status;
+  a.out = (uint4*)o_clusters; a.capacity = o_capacity; a.n_clusters = (u64*)o_n; a.status = status;
   a.ticket = p.ticket; a.tile_state = p.tile_state;
   a.temp = p.pool; a.temp_cap = h->g.n_chunks_max * 8ull; a.temp_cursor = p.temp_cursor;   // the K1 pool is dead after K5
   a.tile_base = p.tile_base; a.tile_cnt = p.tile_cnt; a.det_flag = p.det_flag;
   a.dmap = nullptr; a.row_off = p.row_off;
   void* ka[] = {&a};
   if (mode == TPCCLUS_MODE_FAST) {
-    CUDA_TRY(h, cudaMemsetAsync(out->n_clusters, 0, 8, st));
+    CUDA_TRY(h, cudaMemsetAsync(o_n, 0, 8, st));
     if ((rc = launch(h, K_TILES_FAST, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
   } else {
     // ordered output (PAPER.md 47-50): runs into the temporary buffer, scan of the tile counts,
@@ -583,17 +588,34 @@ int tpcclus_run(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n, co
     u32 nt = g.n_tiles, nblk = g.n_scan_blocks;
     { void* s[] = {&p.tile_cnt, &p.tile_local, &p.block_sum, &nt};
       if ((rc = launch(h, K_SCAN_LOCAL, dim3(nblk), dim3(TPC_SCAN_THREADS), 0, st, s))) return rc; }
-    { u64* total = (u64*)out->n_clusters;
+    { u64* total = (u64*)o_n;
       void* s[] = {&p.block_sum, &p.block_prefix, &nblk, &total};
       if ((rc = launch(h, K_SCAN_SUMS, dim3(1), dim3(TPC_SCAN_THREADS), 0, st, s))) return rc; }
-    { uint4* o = (uint4*)out->clusters; u64 cap = out->capacity;
+    uint4* o = (uint4*)o_clusters; u64 cap = o_capacity;
+    if (packed) {
+      u64* ri = (u64*)packed->row_index;
+      void* s[] = {&a.temp, &p.tile_base, &p.tile_cnt, &p.tile_local, &p.block_prefix, &nt, &o, &cap, &ri, &p.det_flag, &status};
+      if ((rc = launch(h, K_EMIT_PACKED, dim3(g.g1 * 8u), dim3(256), 0, st, s))) return rc;
+    } else {
       void* s[] = {&a.temp, &p.tile_base, &p.tile_cnt, &p.tile_local, &p.block_prefix, &nt, &o, &cap, &p.det_flag, &status};
-      if ((rc = launch(h, K_EMIT_ORDERED, dim3(g.g1 * 8u), dim3(256), 0, st, s))) return rc; }
-    CUDA_TRY(h, cudaMemsetAsync(p.ticket, 0, 4, st));
-    if ((rc = launch(h, K_TILES_DET, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
+      if ((rc = launch(h, K_EMIT_ORDERED, dim3(g.g1 * 8u), dim3(256), 0, st, s))) return rc;
+      CUDA_TRY(h, cudaMemsetAsync(p.ticket, 0, 4, st));
+      if ((rc = launch(h, K_TILES_DET, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
+    }
   }
   h->ran = true;
   return TPCCLUS_OK;
+}
+
+int tpcclus_run(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n, const tpcclus_out* out, int mode,
+                void* cuda_stream) {
+  return run_impl(h, d_digits, n, out, nullptr, mode, cuda_stream);
+}
+
+int tpcclus_run_packed(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n, const tpcclus_out_packed* out,
+                       void* cuda_stream) {
+  if (!out) return TPCCLUS_ERR_INVALID_ARG;
+  return run_impl(h, d_digits, n, nullptr, out, TPCCLUS_MODE_DETERMINISTIC, cuda_stream);
 }
 
 int tpcclus_run_host(tpcclus_handle* h, const tpcclus_digit* h_digits, uint64_t n, tpcclus_cluster* h_clusters,

@@ -524,6 +524,53 @@ k_emit_ordered(const uint4* __restrict__ temp, const u64* __restrict__ tile_base
   if (over) atomicOr(status, TPC_STATUS_OVERFLOW);
 }
 
+// K9p: the packed variant of K9 (O6: 16-byte fixed-point record) plus
+// the per-row index.  One warp per tile, one cluster per lane; the first tile of every pad row
+// also writes where that row starts.  When the run buffer was too small (flag) nothing is
+// written but the NO_PACKED status bit.
+#define TPC_STATUS_NO_PACKED 4u
+extern "C" __global__ void __launch_bounds__(256)
+k_emit_packed(const uint4* __restrict__ temp, const u64* __restrict__ tile_base, const u32* __restrict__ tile_cnt,
+              const u32* __restrict__ tile_local, const u64* __restrict__ block_prefix, u32 n_tiles,
+              uint4* __restrict__ out, u64 capacity, u64* __restrict__ row_index, const u32* __restrict__ flag,
+              u32* __restrict__ status) {
+  if (*flag != 0u) {
+    if (blockIdx.x == 0 && threadIdx.x == 0) atomicOr(status, TPC_STATUS_NO_PACKED);
+    return;
+  }
+  const u32 lane = threadIdx.x & 31u;
+  const u32 tiles_per_row = PRM(n_tc) * PRM(n_sl);   // bins of one (sector,row) are consecutive
+  bool over = false;
+  for (u32 tile = blockIdx.x * 8u + (threadIdx.x >> 5); tile <= n_tiles; tile += gridDim.x * 8u) {
+    const u64 dst0 = tile < n_tiles ? block_prefix[tile / TPC_SCAN_PER_CTA] + tile_local[tile]
+                                    : block_prefix[(n_tiles - 1u) / TPC_SCAN_PER_CTA] + tile_local[n_tiles - 1u] + tile_cnt[n_tiles - 1u];
+    if (lane == 0u && tile % tiles_per_row == 0u) row_index[tile / tiles_per_row] = dst0;   // incl. the end sentinel
+    if (tile == n_tiles) break;
+    const u32 cnt = tile_cnt[tile];
+    if (cnt == 0u) continue;
+    const u64 src = tile_base[tile] * 2ull;
+    u64 keep = capacity > dst0 ? capacity - dst0 : 0ull;   // Q22: the first `capacity` clusters stay, in order
+    if (keep < cnt) over = true; else keep = cnt;
+    for (u32 i = lane; i < (u32)keep; i += 32u) {
+      const uint4 a = temp[src + 2ull * i], b = temp[src + 2ull * i + 1ull];
+      // a = pad_mean, time_mean, sigma_pad, sigma_time (float32 bits); b = q_tot, q_max | time_peak << 16,
+      // pad_peak | row << 8 | sector << 16 | flags << 24, 0
+      const u32 time_fix = __float2uint_rn(__fmul_rn(__uint_as_float(a.y), 256.0f));
+      u32 pad_fix = __float2uint_rn(__fmul_rn(__uint_as_float(a.x), 256.0f));
+      if (pad_fix > 65535u) pad_fix = 65535u;
+      const u32 sp = __float2uint_rn(__fmul_rn(__uint_as_float(a.z), 16384.0f));
+      const u32 st = __float2uint_rn(__fmul_rn(__uint_as_float(a.w), 16384.0f));
+      uint4 o;
+      o.x = time_fix | ((b.z & 0xFFu) << 24);
+      o.y = pad_fix | (b.y & 0xFFFF0000u);                                  // pad_fix | time_peak << 16
+      o.z = (b.x & 0xFFFFu) | (((b.y & 0x3FFu) | ((b.z >> 24) << 10)) << 16);   // q_tot | (q_max | flags << 10) << 16
+      o.w = sp | (st << 16);
+      out[dst0 + i] = o;
+    }
+  }
+  if (over) atomicOr(status, TPC_STATUS_OVERFLOW);
+}
+
 // ==========================================================================================
 // K5  partition_fine  (NS (1), second half: route every record to the tile(s) whose shared-
 //     memory charge map needs it; a record within 3 time bins of a slab border is copied

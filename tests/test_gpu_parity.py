@@ -424,3 +424,41 @@ def test_rtc_cubin_cache(tp, cuda_device, tmp_path):
         assert len(list(tmp_path.glob("tpcclus_*.cubin"))) == 2
     finally:
         tp.tpcclus_set_rtc_cache_dir(None)
+
+
+def test_packed_output_and_row_index(tp, cuda_device):
+    """the packed 16-byte records and the per-row index, byte for byte
+    against the oracle's encoding of its own deterministic records."""
+    import torch
+    from oracle.pack16 import pack16, row_index
+    for fr in (make_frame(1), make_frame(0), make_frame(4, device=cuda_device, sectors=[0, 7, 35], n_time=300)):
+        exp, _ = _oracle(fr.digits_numpy(), fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads)
+        c = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, fr.n_digits)
+        cl, ridx, nt, st = c.run_packed(fr.digits.to(cuda_device))
+        torch.cuda.synchronize()
+        n = int(nt.item())
+        assert n == len(exp) and int(st.item()) == 0
+        assert cl[:n].cpu().numpy().tobytes() == pack16(exp).tobytes()
+        assert ridx.cpu().numpy().astype(np.uint64).tolist() == row_index(exp, fr.n_sectors, fr.n_rows).tolist()
+        # overflow: the first `capacity` stay in order, the index still describes the whole list
+        cap = n // 2
+        cl2, ridx2, nt, st = c.run_packed(fr.digits.to(cuda_device), capacity=cap)
+        torch.cuda.synchronize()
+        assert int(nt.item()) == n and int(st.item()) == tp.STATUS_OVERFLOW
+        assert cl2.cpu().numpy().tobytes() == pack16(exp[:cap]).tobytes() and torch.equal(ridx2, ridx)
+        # the 32-byte path of the same handle is unaffected
+        assert c.run_sync(fr.digits.to(cuda_device), tp.MODE_DETERMINISTIC)[0].tobytes() == exp.tobytes()
+        c.close()
+    # more clusters than the run buffer holds: said loudly, nothing written
+    T, P, R = 3000, 138, 4
+    rows = np.zeros((R, T // 2, P // 2), dtype=t1.DIGIT)
+    rows["time"] = (2 * np.arange(T // 2, dtype=np.uint16))[None, :, None]
+    rows["pad"] = (2 * np.arange(P // 2, dtype=np.uint8))[None, None, :]
+    rows["row"] = np.arange(R, dtype=np.uint8)[:, None, None]
+    rows["charge"] = 50
+    d = rows.reshape(-1)
+    c = tp.Clusterizer(1, R, T, [P] * R, len(d))
+    _, _, nt, st = c.run_packed(_digits_tensor(d, cuda_device))
+    torch.cuda.synchronize()
+    assert int(nt.item()) == len(d) and int(st.item()) == tp.STATUS_NO_PACKED
+    c.close()
