@@ -160,7 +160,10 @@ TPCCLUS_API uint64_t tpcclus_workspace_bytes(const tpcclus_params* params);
  * parameter block goes to __constant__ memory at the head of every run(), stream-ordered,
  * so several handles with different geometry can share a process: PAPER.md 85).  With
  * TPCCLUS_RTC the kernels are compiled here for sm_100a by NVRTC and loaded as a module
- * (PAPER.md 64, 91).  Host call, synchronous.  *out is NULL on failure. */
+ * (PAPER.md 64, 91).  Host call, synchronous.  *out is NULL on failure.
+ * Generic (non-RTC) handles of one process share ONE __constant__ block: runs of handles with
+ * DIFFERENT parameters must not overlap in time on different streams (same stream, or equal
+ * parameters, or RTC handles -- which carry their constants in their own module -- are fine). */
 TPCCLUS_API int tpcclus_create(const tpcclus_params* params, tpcclus_handle** out);
 
 /* Clusterizes one time frame: enqueues every step of the path (NS (1)..(5)) on
