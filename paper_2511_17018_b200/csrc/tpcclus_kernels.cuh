@@ -572,22 +572,30 @@ k_emit_packed(const uint4* __restrict__ temp, const u64* __restrict__ tile_base,
 }
 
 // ==========================================================================================
-// K5  partition_fine  (NS (1), second half: route every record to the tile(s) whose shared-
-//     memory charge map needs it; a record within 3 time bins of a slab border is copied
-//     into the neighbouring tile as halo)
+// K5  partition_fine  (NS (1), second half: group every record with the tile(s) whose shared-
+//     memory charge map needs it)
 //
 // A batch = up to TPC_CPB chunks (<= 8192 records) of ONE coarse bin.  The CTA counting-sorts
-// the batch by slab in shared memory and writes the sorted batch as one contiguous blob
-// (runs padded to 32 B), plus one index entry per (tile, batch):  pos[0:40) | count[40:64).
+// the batch in shared memory and writes it as one contiguous blob.  Sort key = 2 * slab + (m >= 6)
+// with u = slab * TS + m: each slab is split into its first 6 rows (A) and the rest (B), so the
+// layout is  A0 B0 A1 B1 A2 ...  and tile `sl`, which needs u in [sl*TS, sl*TS + TS + 6), reads
+// the CONTIGUOUS range A_sl B_sl A_sl+1.  The border rows A are shared by two tiles instead of
+// being copied: no halo duplicates, one shared atomic per record.  Every A starts on a 4-record
+// (16-byte, the bulk-copy alignment) boundary, zero records filling the gap after the B before,
+// so a tile's range starts aligned; rounding its end up to 16 bytes can only reach into B_sl+1,
+// whose records (other slab parity, m >= 6) K6 recognises as foreign.  One index entry per
+// (tile, batch): pos[0:40) | count[40:64).  The batch end is padded with zero records to 32 B.
 // index layout: idx[n_sl * batch_start[b] + sl * nbatch_b + kb], so a tile finds the runs
 // of all batches of its bin in one contiguous read.
 //
-// tile record (4 B):  pad[0:8) | tl[8:16) | q[16:26)   tl = row of the tile, 0..TPC_TT-1
-// tile sl of a bin holds u in [sl*TS, sl*TS + TS + 6);  it OWNS tl in [3, TS+3).
+// tile record (4 B):  pad[0:8) | f[8:16) | q[16:26)   f = m | (slab & 1) << 7      (0 = padding)
+// For tile sl, tl = f ^ ((sl & 1) << 7) is the row in its map: own slab -> m, next slab -> TS + m;
+// tl >= TPC_TT means "not mine".  Tile sl OWNS rows tl in [3, TS+3).
 // ==========================================================================================
 #define TPC_NSLMAX 128u   // >= slabs per bin: TPC_TC / TPC_TS = 127
-#define TPC_K5_BUF (2u * TPC_CPB * TPC_CHUNK + 8u * TPC_NSLMAX)   // u32 words: records + halo copies + run padding
-__host__ __device__ inline u32 tpc_k5_smem_bytes() { return (TPC_K5_BUF + 4u * TPC_NSLMAX + 8u) * 4u; }
+#define TPC_NKEY (2u * TPC_NSLMAX + 32u)   // sort keys: 2 per slab + A of the slab after the last; multiple of 32
+#define TPC_K5_BUF (TPC_CPB * TPC_CHUNK + 4u * TPC_NSLMAX + 8u)   // u32 words: the records of a batch + alignment gaps + end padding
+__host__ __device__ inline u32 tpc_k5_smem_bytes() { return (TPC_K5_BUF + 2u * TPC_NKEY + 8u) * 4u; }
 
 extern "C" __global__ void __launch_bounds__(TPC_K5_THREADS, 2)
 k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, const u32* __restrict__ chunk_list,
@@ -596,10 +604,8 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
                  u64* __restrict__ idx, u32* __restrict__ status) {
   extern __shared__ __align__(128) u32 smem_u32[];
   u32* buf = smem_u32;                       // [TPC_K5_BUF]
-  u32* s_cnt = buf + TPC_K5_BUF;             // [NSLMAX] primaries per slab
-  u32* s_dcnt = s_cnt + TPC_NSLMAX;          // [NSLMAX] halo copies per slab
-  u32* s_off = s_dcnt + TPC_NSLMAX;          // [NSLMAX + 1] run start (multiple of 8)
-  u32* s_dcur = s_off + TPC_NSLMAX + 4u;     // [NSLMAX]
+  u32* s_cnt = buf + TPC_K5_BUF;             // [NKEY] records per key
+  u32* s_off = s_cnt + TPC_NKEY;             // [NKEY + 1] start of every key's run
   __shared__ u64 s_gbase;
   const u32 nb = PRM(n_bins), nsl = PRM(n_sl);
   const u32 n_batches = batch_start[nb];
@@ -648,10 +654,10 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
   for (u32 batch = blockIdx.x; batch < n_batches; batch += gridDim.x) {
     const u32 b = cur_b.b, kb = cur_b.kb, nbatch_b = cur_b.nbatch_b;
     const u32 npads = PRM_NPADS((b / PRM(n_tc)) % PRM(n_rows));   // one bin = one pad row
-    if (threadIdx.x < TPC_NSLMAX) { s_cnt[threadIdx.x] = 0u; s_dcnt[threadIdx.x] = 0u; s_dcur[threadIdx.x] = 0u; }
+    if (threadIdx.x < TPC_NKEY) s_cnt[threadIdx.x] = 0u;
     __syncthreads();
 
-    // ---- <= 16 records per thread: count per slab, remember the rank -------------------------
+    // ---- <= 16 records per thread: count per key, remember the rank -------------------------
     u32 rec[16];
     u32 rank[8];
 #pragma unroll
@@ -667,10 +673,9 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
         if ((r & 0xFFu) >= npads && r != 0u) { r = 0u; bad = true; }   // O0 / Q4: pad out of range -> ignored + flagged
         u32 rk = 0u;
         if (r != 0u) {
-          u32 u = (r >> 8) & 0x3FFFu;
-          u32 sl1 = u / TPC_TS, m = u - sl1 * TPC_TS;
-          if (sl1 < nsl) rk = atomicAdd(&s_cnt[sl1], 1u);
-          if (sl1 >= 1u && m < 2u * TPC_HALO) atomicAdd(&s_dcnt[sl1 - 1u], 1u);
+          const u32 u = (r >> 8) & 0x3FFFu;
+          const u32 key = 2u * (u / TPC_TS) + ((u % TPC_TS) >= 2u * TPC_HALO ? 1u : 0u);   // <= 2 * nsl (u < TC + 6)
+          rk = atomicAdd(&s_cnt[key], 1u);
         }
         rec[i * 4 + j] = r;
         if (j & 1) rank[i * 2 + (j >> 1)] |= rk << 16; else rank[i * 2 + (j >> 1)] = rk;
@@ -678,61 +683,61 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
     }
     ids(nxt_b, cidn);   // chunk ids of the next batch: in flight during the scan and the placing
     __syncthreads();
-    // ---- exclusive scan of padded run lengths (one warp, NSLMAX/32 slabs per lane) ---------
+    // ---- exclusive scan of the run lengths (one warp, NKEY/32 keys = NKEY/64 slabs per lane);
+    //      every slab's A run starts on a multiple of 4 records ----------------------------------
     if (threadIdx.x < 32) {
-      u32 len[TPC_NSLMAX / 32u], t = 0u;
+      u32 la[TPC_NKEY / 64u], lb[TPC_NKEY / 64u], t = 0u;
 #pragma unroll
-      for (int k = 0; k < (int)(TPC_NSLMAX / 32u); ++k) {
-        u32 sl = threadIdx.x * (TPC_NSLMAX / 32u) + (u32)k;
-        len[k] = sl < nsl ? ((s_cnt[sl] + s_dcnt[sl] + 7u) & ~7u) : 0u;
-        t += len[k];
+      for (int k = 0; k < (int)(TPC_NKEY / 64u); ++k) {
+        const u32 key = 2u * (threadIdx.x * (TPC_NKEY / 64u) + (u32)k);
+        la[k] = s_cnt[key]; lb[k] = s_cnt[key + 1u];
+        t += (la[k] + lb[k] + 3u) & ~3u;
       }
       u32 inc = t;
 #pragma unroll
       for (int d = 1; d < 32; d <<= 1) { u32 o = __shfl_up_sync(0xFFFFFFFFu, inc, d); if ((int)threadIdx.x >= d) inc += o; }
       u32 e = inc - t;
 #pragma unroll
-      for (int k = 0; k < (int)(TPC_NSLMAX / 32u); ++k) { s_off[threadIdx.x * (TPC_NSLMAX / 32u) + (u32)k] = e; e += len[k]; }
+      for (int k = 0; k < (int)(TPC_NKEY / 64u); ++k) {
+        const u32 key = 2u * (threadIdx.x * (TPC_NKEY / 64u) + (u32)k);
+        s_off[key] = e; s_off[key + 1u] = e + la[k];
+        const u32 end = e + la[k] + lb[k];
+        e += (la[k] + lb[k] + 3u) & ~3u;
+        for (u32 g = end; g < e; ++g) buf[g] = 0u;   // the gap before the next A (nobody else writes there)
+      }
       if (threadIdx.x == 31) {
-        s_off[TPC_NSLMAX] = inc;
-        s_gbase = atomicAdd(blob_cursor, (u64)inc);
+        s_off[TPC_NKEY] = inc;
+        s_gbase = atomicAdd(blob_cursor, (u64)((inc + 7u) & ~7u));   // batches start 32-byte aligned
       }
     }
     __syncthreads();
     // ---- place ------------------------------------------------------------------------------
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
-      u32 r = rec[k];
+      const u32 r = rec[k];
       if (r != 0u) {
-        u32 u = (r >> 8) & 0x3FFFu;
-        u32 sl1 = u / TPC_TS, m = u - sl1 * TPC_TS;
-        u32 base = (r & 0xFFu) | ((r >> 22) << 16);
-        u32 rk = (rank[k >> 1] >> ((k & 1) * 16)) & 0xFFFFu;
-        if (sl1 < nsl) buf[s_off[sl1] + rk] = base | (m << 8);
-        if (sl1 >= 1u && m < 2u * TPC_HALO) {
-          u32 d = atomicAdd(&s_dcur[sl1 - 1u], 1u);
-          buf[s_off[sl1 - 1u] + s_cnt[sl1 - 1u] + d] = base | ((m + TPC_TS) << 8);
-        }
+        const u32 u = (r >> 8) & 0x3FFFu;
+        const u32 sl1 = u / TPC_TS, m = u % TPC_TS;
+        const u32 key = 2u * sl1 + (m >= 2u * TPC_HALO ? 1u : 0u);
+        const u32 rk = (rank[k >> 1] >> ((k & 1) * 16)) & 0xFFFFu;
+        buf[s_off[key] + rk] = (r & 0xFFu) | ((m | ((sl1 & 1u) << 7)) << 8) | ((r >> 22) << 16);
       }
     }
     pieces(cidn, vn, nrecn);   // records of the next batch: in flight during the dump
     cur_b = nxt_b;
     look(batch + 2u * gridDim.x, nxt_b);
-    if (threadIdx.x >= TPC_NSLMAX && threadIdx.x < TPC_NSLMAX + nsl) {   // zero the padding of every run (K6 skips record 0)
-      const u32 sl = threadIdx.x - TPC_NSLMAX;
-      for (u32 k = s_off[sl] + s_cnt[sl] + s_dcnt[sl]; k < s_off[sl + 1u]; ++k) buf[k] = 0u;
-    }
+    const u32 total = s_off[TPC_NKEY];
+    if (threadIdx.x < 8u && total + threadIdx.x < ((total + 7u) & ~7u)) buf[total + threadIdx.x] = 0u;   // end padding
     __syncthreads();
     // ---- dump the sorted batch + its index entries -----------------------------------------
     const u64 gbase = s_gbase;
-    const u32 total = s_off[TPC_NSLMAX];
     uint4* dst = (uint4*)(blob + gbase);       // gbase is a multiple of 8 records (32 B)
     const uint4* src = (const uint4*)buf;
-    for (u32 i = threadIdx.x; i < (total >> 2); i += TPC_K5_THREADS) dst[i] = src[i];
-    if (threadIdx.x < nsl) {
-      u32 sl = threadIdx.x;
-      idx[(u64)nsl * batch_start[b] + (u64)sl * nbatch_b + kb] =
-          (gbase + s_off[sl]) | ((u64)(s_cnt[sl] + s_dcnt[sl]) << 40);
+    for (u32 i = threadIdx.x; i < ((total + 7u) >> 3) * 2u; i += TPC_K5_THREADS) dst[i] = src[i];
+    if (threadIdx.x < nsl) {   // tile sl reads A_sl B_sl A_sl+1
+      const u32 sl = threadIdx.x;
+      const u32 beg = s_off[2u * sl], end = s_off[2u * sl + 3u];   // beg is a multiple of 4
+      idx[(u64)nsl * batch_start[b] + (u64)sl * nbatch_b + kb] = (gbase + beg) | ((u64)(end - beg) << 40);
     }
     __syncthreads();
   }
@@ -833,7 +838,7 @@ struct K6Smem {
   u32* rowpre; u32* misc; u16* peaks;
 };
 // misc: [0] n_peaks  [3] first tile of the stage  [4] tiles in the stage  [5] row | sector << 8 |
-//       n_pads << 16  [6] time of row 0 of the first tile  [8+2m],[9+2m] offset and
+//       n_pads << 16  [6] time of row 0 of the first tile  [7] its slab  [8+2m],[9+2m] offset and
 //       size (16-byte units) of tile m's records in `rec`
 #define TPC_K6_GROUP 4u   // tiles (consecutive slabs of one bin) a ticket covers
 #define TPC_K6_PMW 9u
@@ -883,9 +888,13 @@ __device__ __forceinline__ u64 k6_chain(u64* state, u32 tile, u32 count) {
   return excl;
 }
 
+// Tile row of a K5 record for the tile of slab `sl`: own slab -> m, next slab -> TS + m (its first
+// 6 rows close this tile); anything >= TPC_TT is a foreign record (up to 3 of them follow a run).
+__device__ __forceinline__ u32 k6_row(u32 r, u32 sl) { return ((r >> 8) & 0xFFu) ^ ((sl & 1u) << 7); }
+
 // Producer warp: stages round `round` of a tile -- the 16-byte units [round*CAPU, (round+1)*CAPU)
-// of the concatenation of the tile's runs (one run per K5 batch of the bin, 32-byte aligned and
-// zero-padded by K5) -- and arrives on the full barrier.  Returns the tile's total units.
+// of the concatenation of the tile's runs (one run per K5 batch of the bin, 16-byte aligned,
+// possibly followed by up to 3 foreign records: k6_row) -- and arrives on the full barrier.  Returns the tile's total units.
 __device__ __forceinline__ u32 k6_stage(const K6Smem& s, const K6Args& a, u64 ib, u32 nbatch, u32 round, u64 e0) {
   const u32 lane = lane_id();
   const u32 lo = round * TPC_K6_CAPU, hi = lo + TPC_K6_CAPU;
@@ -976,7 +985,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
         const u32 t_beg = __shfl_sync(0xFFFFFFFFu, off, (int)(lane & ~7u));
         mbar_wait_backoff(&s.bar[1], ph); ph ^= 1u;
         if (kb == 0u && m < TPC_K6_GROUP) { s.misc[8u + 2u * m] = t_beg; s.misc[9u + 2u * m] = m < cnt ? t_end - t_beg : 0u; }
-        if (lane == 0u) { s.misc[3] = tile0; s.misc[4] = cnt; s.misc[5] = geo; s.misc[6] = (u32)t0; if (tot != 0u) mbar_expect_tx(&s.bar[0], tot * 16u); }
+        if (lane == 0u) { s.misc[3] = tile0; s.misc[4] = cnt; s.misc[5] = geo; s.misc[6] = (u32)t0; s.misc[7] = sl0; if (tot != 0u) mbar_expect_tx(&s.bar[0], tot * 16u); }
         __syncwarp();
         if (units != 0u) bulk_g2s(s.rec + off * 4u, src, units * 16u, &s.bar[0]);
         __syncwarp();
@@ -989,7 +998,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
           if (bytes != 0u)
             asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(a.blob + (e0 & ((1ull << 40) - 1ull))), "r"(bytes) : "memory");
           mbar_wait_backoff(&s.bar[1], ph); ph ^= 1u;
-          if (lane == 0u) { s.misc[3] = tile0 + k; s.misc[4] = 1u; s.misc[5] = geo; s.misc[6] = (u32)(t0 + (int)(k * TPC_TS)); }   // published by the arrive in k6_stage
+          if (lane == 0u) { s.misc[3] = tile0 + k; s.misc[4] = 1u; s.misc[5] = geo; s.misc[6] = (u32)(t0 + (int)(k * TPC_TS)); s.misc[7] = sl0 + k; }   // published by the arrive in k6_stage
           const u32 total = k6_stage(s, a, ib, nbatch, 0u, e0);
           for (u32 round = 1u; round * TPC_K6_CAPU < total; ++round) {
             mbar_wait_backoff(&s.bar[1], ph); ph ^= 1u;
@@ -1037,6 +1046,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
     const u32 geo = s.misc[5];
     const u32 row = geo & 0xFFu, sector = (geo >> 8) & 0xFFu, npads = geo >> 16;
     const int t_base = (int)s.misc[6] + (int)(mt * TPC_TS);   // time of tile row 0
+    const u32 sl = s.misc[7] + mt;                            // slab of this tile inside its bin
     csync();   // A: the previous tile is done with the map, and the map is zero
     // ---- O0: scatter the tile's records ------------------------------------------------------
     for (u32 round = 0u;;) {
@@ -1048,8 +1058,10 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
         const u32 rr[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
         for (int k = 0; k < 4; ++k)
-          if (rr[k] != 0u)   // 0 = run padding (every real record has q >= 1)
-            s.tile[((rr[k] >> 8) & 0xFFu) * pitch + (rr[k] & 0xFFu) + TPC_HALO] = (u16)((rr[k] >> 16) & 0x3FFu);
+          if (rr[k] != 0u) {   // 0 = batch padding (every real record has q >= 1)
+            const u32 tl = k6_row(rr[k], sl);
+            if (tl < TPC_TT) s.tile[tl * pitch + (rr[k] & 0xFFu) + TPC_HALO] = (u16)((rr[k] >> 16) & 0x3FFu);
+          }
       }
       if (MODE != TPC_MODE_FAST) {
         // Q5, deterministic: two digits on one cell -> the maximum, whatever the order.  Re-check
@@ -1061,12 +1073,14 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
             const uint4 v = r4[u];
             const u32 rr[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
-            for (int k = 0; k < 4; ++k)
-              if (rr[k] != 0u) {
-                const u32 cell = ((rr[k] >> 8) & 0xFFu) * pitch + (rr[k] & 0xFFu) + TPC_HALO;
+            for (int k = 0; k < 4; ++k) {
+              const u32 tl = k6_row(rr[k], sl);
+              if (rr[k] != 0u && tl < TPC_TT) {
+                const u32 cell = tl * pitch + (rr[k] & 0xFFu) + TPC_HALO;
                 const u16 q = (u16)((rr[k] >> 16) & 0x3FFu);
                 if (s.tile[cell] < q) { s.tile[cell] = q; any = 1u; }
               }
+            }
           }
           if (!csync_or(any)) break;
         }
@@ -1113,7 +1127,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
         bool cand[4];
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
-          const u32 q = (rr[k] >> 16) & 0x3FFu, tl = (rr[k] >> 8) & 0xFFu, pad = rr[k] & 0xFFu;
+          const u32 q = (rr[k] >> 16) & 0x3FFu, tl = k6_row(rr[k], sl), pad = rr[k] & 0xFFu;
           cand[k] = q >= thr && tl - 1u < TPC_TT - 2u;   // (q = 0 for run padding)
           const u32 x = pad + TPC_HALO, h = x & 1u, sh = 16u - 16u * h;
           const u32* w = s.tile32 + (cand[k] ? (tl - 1u) * nW + (x >> 1) - 1u + h : 0u);
@@ -1125,7 +1139,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
         }
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
-          const u32 q = (rr[k] >> 16) & 0x3FFu, tl = (rr[k] >> 8) & 0xFFu, pad = rr[k] & 0xFFu;
+          const u32 q = (rr[k] >> 16) & 0x3FFu, tl = k6_row(rr[k], sl), pad = rr[k] & 0xFFu;
           const u32 e = max(max(pu[k] & 0xFFFFu, pu[k] >> 16), max(nu[k], pm[k] & 0xFFFFu));
           const u32 l = max(max(pd[k] & 0xFFFFu, pd[k] >> 16), max(nd[k], nm[k]));
           if (cand[k] && (pm[k] >> 16) == q && q > e && q >= l) {   // (!= q: a smaller duplicate of this cell)
