@@ -40,8 +40,8 @@ def _log(msg):
 
 METRIC = "TPC clusterizer digits/s on Pb-Pb-like time frame"
 # ncu --set full, CFG[4] shuffled FAST generic, one launch each (profiles/r01d_ncu_full_summary.txt)
-NCU_TRAFFIC_BYTES = {"k_partition_coarse": 12764779000 + 6478431000, "k_partition_fine": 9146624000 + 7140715000,
-                     "k_cluster_tiles_fast": 7184330000 + 1901887000}
+NCU_TRAFFIC_BYTES = {"k_partition_coarse": 12766098000 + 6478920000, "k_partition_fine": 9156652000 + 6744179000,
+                     "k_cluster_tiles_fast": 6711538000 + 1900586000}
 UNIT = "digits/s"
 
 
