@@ -78,8 +78,9 @@ def survivors_of(m, pk, rank, noise_eps):
     return out
 
 
-def cluster_of(m, T, P, c, s, r):
-    """O3 + O4 (flags as in O4)."""
+def cluster_of(m, T, P, c, s, r, cog_gated=False):
+    """O3 + O4 (flags as in O4).  cog_gated = reading Q10' (R7): an outer-ring cell of the
+    window counts only if the inner cell between it and the peak holds charge."""
     t_c, p_c = c
     Q = Sp = St = Spp = Stt = 0
     for dt, dp in product(range(-2, 3), repeat=2):
@@ -87,6 +88,10 @@ def cluster_of(m, T, P, c, s, r):
         if not (0 <= x[0] < T and 0 <= x[1] < P):
             continue
         q = m.get(x, 0)
+        if cog_gated and max(abs(dt), abs(dp)) == 2:
+            inner = (t_c + max(-1, min(1, dt)), p_c + max(-1, min(1, dp)))
+            if m.get(inner, 0) == 0:     # the inner cell is in range whenever the outer one is
+                continue
         Q += q
         Sp += q * dp
         St += q * dt
@@ -113,7 +118,7 @@ def cluster_of(m, T, P, c, s, r):
     )
 
 
-def clusterize(digits, n_sectors, n_rows, n_time, n_pads, thr_peak=6, noise_eps=4):
+def clusterize(digits, n_sectors, n_rows, n_time, n_pads, thr_peak=6, noise_eps=4, cog_gated=False):
     """O0..O5.  Returns (list of cluster dicts in (sector,row,time,pad) order, bad_flag)."""
     maps, bad = build_maps(digits, n_sectors, n_rows, n_time, n_pads)
     out = []
@@ -123,7 +128,7 @@ def clusterize(digits, n_sectors, n_rows, n_time, n_pads, thr_peak=6, noise_eps=
         pk, rank = peaks_of(m, T, P, thr_peak)
         sv = survivors_of(m, pk, rank, noise_eps)
         for c in sorted(sv):  # (time, pad) ascending == O5 within a row
-            out.append(cluster_of(m, T, P, c, s, r))
+            out.append(cluster_of(m, T, P, c, s, r, cog_gated))
     return out, bad
 
 

@@ -62,6 +62,8 @@ def lib():
             ctypes.c_uint32, ctypes.c_uint32, ctypes.c_void_p, ctypes.c_uint64,
             ctypes.c_void_p, ctypes.c_uint64, ctypes.c_void_p, ctypes.c_void_p,
         ]
+        _lib.oracle_clusterize_ex.restype = ctypes.c_int64
+        _lib.oracle_clusterize_ex.argtypes = _lib.oracle_clusterize.argtypes + [ctypes.c_int]
         _lib.oracle_finalize.restype = None
         _lib.oracle_finalize.argtypes = [
             ctypes.c_uint32, ctypes.c_int32, ctypes.c_int32, ctypes.c_uint32, ctypes.c_uint32,
@@ -77,7 +79,7 @@ def lib():
 
 
 def clusterize(digits, n_sectors, n_rows, n_time, n_pads, thr_peak=6, noise_eps=4,
-               capacity=None, return_map=False, timing=None):
+               capacity=None, return_map=False, timing=None, cog_gated=False):
     """Run O0..O5.  ``digits``: array of dtype DIGIT (or uint64 / (n,8) uint8 view).
 
     Returns ``(clusters[DIGIT->CLUSTER array], status)`` (+ the O0 map if
@@ -98,10 +100,10 @@ def clusterize(digits, n_sectors, n_rows, n_time, n_pads, thr_peak=6, noise_eps=
     if return_map:
         dbg = np.zeros(int(n_sectors) * int(n_time) * int(pads.astype(np.int64).sum()), dtype=np.uint16)
     t0 = time.perf_counter()
-    cnt = lib().oracle_clusterize(
+    cnt = lib().oracle_clusterize_ex(
         n_sectors, n_rows, n_time, pads.ctypes.data, thr_peak, noise_eps,
         d.ctypes.data, n, out.ctypes.data, capacity, ctypes.byref(status),
-        dbg.ctypes.data if dbg is not None else None,
+        dbg.ctypes.data if dbg is not None else None, 1 if cog_gated else 0,
     )
     if timing is not None:
         timing["seconds"] = time.perf_counter() - t0

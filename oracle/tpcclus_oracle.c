@@ -140,14 +140,20 @@ void oracle_finalize(uint32_t Q, int32_t Sp, int32_t St, uint32_t Spp, uint32_t 
   out4[3] = st;
 }
 
-/* O3 + O4 for one surviving peak. */
+/* O3 + O4 for one surviving peak.  `gated` selects reading Q10' (DESIGN.md
+ * R7): a cell of the outer ring of the 5x5 window, max(|dp|,|dt|) = 2, counts only if the inner
+ * cell between it and the peak -- (clamp(dt,-1,1), clamp(dp,-1,1)) -- is non-empty. */
 static void make_cluster(const row_map* m, uint32_t s, uint32_t r, int64_t t, int64_t p,
-                         orc_cluster* c) {
+                         orc_cluster* c, int gated) {
   uint32_t Q = 0, Spp = 0, Stt = 0;
   int32_t Sp = 0, St = 0;
   for (int dt = -2; dt <= 2; ++dt)
     for (int dp = -2; dp <= 2; ++dp) {
       uint32_t q = cell(m, t + dt, p + dp); /* Q8/Q10: clipped window, weight 1 */
+      if (gated && (iabs(dt) == 2 || iabs(dp) == 2)) {
+        int it = dt < -1 ? -1 : (dt > 1 ? 1 : dt), ip = dp < -1 ? -1 : (dp > 1 ? 1 : dp);
+        if (cell(m, t + it, p + ip) == 0) q = 0; /* Q10': weight 0 */
+      }
       Q += q;
       Sp += (int32_t)q * dp;
       St += (int32_t)q * dt;
@@ -182,10 +188,23 @@ static void make_cluster(const row_map* m, uint32_t s, uint32_t r, int64_t t, in
  * If dbg_map != NULL it must hold n_sectors * sum_r(T*n_pads[r]) uint16 and
  * receives the O0 map in [sector][row][time][pad] order (for map-level pins).
  */
+int64_t oracle_clusterize_ex(uint32_t n_sectors, uint32_t n_rows, uint32_t n_time,
+                             const uint16_t* n_pads, uint32_t thr_peak, uint32_t noise_eps,
+                             const orc_digit* digits, uint64_t n_digits, orc_cluster* out,
+                             uint64_t capacity, uint32_t* status, uint16_t* dbg_map, int cog_gated);
+
 int64_t oracle_clusterize(uint32_t n_sectors, uint32_t n_rows, uint32_t n_time,
                           const uint16_t* n_pads, uint32_t thr_peak, uint32_t noise_eps,
                           const orc_digit* digits, uint64_t n_digits, orc_cluster* out,
                           uint64_t capacity, uint32_t* status, uint16_t* dbg_map) {
+  return oracle_clusterize_ex(n_sectors, n_rows, n_time, n_pads, thr_peak, noise_eps, digits, n_digits, out,
+                              capacity, status, dbg_map, 0);
+}
+
+int64_t oracle_clusterize_ex(uint32_t n_sectors, uint32_t n_rows, uint32_t n_time,
+                             const uint16_t* n_pads, uint32_t thr_peak, uint32_t noise_eps,
+                             const orc_digit* digits, uint64_t n_digits, orc_cluster* out,
+                             uint64_t capacity, uint32_t* status, uint16_t* dbg_map, int cog_gated) {
   uint32_t st = 0;
   uint64_t n_out = 0;
 
@@ -247,7 +266,7 @@ int64_t oracle_clusterize(uint32_t n_sectors, uint32_t n_rows, uint32_t n_time,
         for (uint32_t p = 0; p < m.P; ++p) {
           if (!pkr[(size_t)t * m.P + p]) continue;
           if (is_suppressed(&m, pkr, t, p, noise_eps)) continue;
-          if (n_out < capacity) make_cluster(&m, s, r, t, p, &out[n_out]);
+          if (n_out < capacity) make_cluster(&m, s, r, t, p, &out[n_out], cog_gated);
           else st |= ORC_STATUS_OVERFLOW;
           ++n_out;
         }
