@@ -88,6 +88,7 @@ int make_geometry(const tpcclus_params* p, Geometry* g) {
   q.max_pads = maxp;
   q.pitch = (maxp + 2 * TPC_HALO + 7) / 8 * 8;
   q.thr_peak = p->thr_peak; q.noise_eps = p->noise_eps;
+  q.cog_gated = (p->flags & TPCCLUS_COG_GATED) ? 1u : 0u;
   q.max_peaks = ((TPC_TT - 2 + 1) / 2) * ((maxp + 1) / 2);   // no two peaks are 8-neighbours; rows 1..TT-2 are scanned
 
   g->max_digits = p->max_digits;
@@ -188,16 +189,20 @@ Rtc& rtc() {
 }
 
 enum KernelId { K_PART_COARSE, K_DIR_COUNT, K_DIR_SCAN, K_DIR_FILL, K_PART_FINE, K_TILES_FAST, K_TILES_DET,
-                K_TILES_DET_TEMP, K_TILES_DUMP, K_SCAN_LOCAL, K_SCAN_SUMS, K_EMIT_ORDERED, K_EMIT_PACKED, K_COUNT_ };
+                K_TILES_DET_TEMP, K_TILES_DUMP, K_SCAN_LOCAL, K_SCAN_SUMS, K_EMIT_ORDERED, K_EMIT_PACKED,
+                K_TILES_FAST_G, K_TILES_DET_G, K_TILES_DET_TEMP_G, K_COUNT_ };
 const char* const kKernelNames[K_COUNT_] = {
     "k_partition_coarse", "k_dir_count", "k_dir_scan", "k_dir_fill", "k_partition_fine", "k_cluster_tiles_fast",
     "k_cluster_tiles_det", "k_cluster_tiles_det_temp", "k_cluster_tiles_dump_map", "k_scan_local", "k_scan_sums",
-    "k_emit_ordered", "k_emit_packed"};
+    "k_emit_ordered", "k_emit_packed", "k_cluster_tiles_fast_gated", "k_cluster_tiles_det_gated",
+    "k_cluster_tiles_det_temp_gated"};
 const void* const kKernelPtrs[K_COUNT_] = {
     (const void*)k_partition_coarse, (const void*)k_dir_count, (const void*)k_dir_scan, (const void*)k_dir_fill,
     (const void*)k_partition_fine, (const void*)k_cluster_tiles_fast, (const void*)k_cluster_tiles_det,
     (const void*)k_cluster_tiles_det_temp, (const void*)k_cluster_tiles_dump_map, (const void*)k_scan_local,
-    (const void*)k_scan_sums, (const void*)k_emit_ordered, (const void*)k_emit_packed};
+    (const void*)k_scan_sums, (const void*)k_emit_ordered, (const void*)k_emit_packed,
+    (const void*)k_cluster_tiles_fast_gated, (const void*)k_cluster_tiles_det_gated,
+    (const void*)k_cluster_tiles_det_temp_gated};
 
 }  // namespace
 
@@ -258,7 +263,7 @@ std::string rtc_prologue(const TpcParams& q) {
   std::string s = "#define TPC_RTC 1\n";
 #define DEF(f) do { snprintf(buf, sizeof buf, "#define TPC_" #f " %uu\n", q.f); s += buf; } while (0)
   DEF(n_sectors); DEF(n_rows); DEF(n_time); DEF(n_tc); DEF(n_bins); DEF(n_sl); DEF(pitch); DEF(max_pads);
-  DEF(thr_peak); DEF(noise_eps); DEF(max_peaks);
+  DEF(thr_peak); DEF(noise_eps); DEF(max_peaks); DEF(cog_gated);
 #undef DEF
   s += "__device__ const unsigned short TPC_NPADS_TABLE[256] = {";
   for (int r = 0; r < 256; ++r) { snprintf(buf, sizeof buf, "%u,", (unsigned)q.n_pads[r]); s += buf; }
@@ -367,7 +372,8 @@ int build_rtc(tpcclus_handle* h) {
       return fail(nullptr, TPCCLUS_ERR_NVRTC, std::string("cuModuleGetFunction: ") + kKernelNames[k]);
   const int CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES = 8;
   struct { int k; uint32_t b; } sm[] = {{K_PART_COARSE, h->smem_k1}, {K_PART_FINE, h->smem_k5}, {K_TILES_FAST, h->smem_k6},
-                                        {K_TILES_DET, h->smem_k6}, {K_TILES_DET_TEMP, h->smem_k6}, {K_TILES_DUMP, h->smem_k6}};
+                                        {K_TILES_DET, h->smem_k6}, {K_TILES_DET_TEMP, h->smem_k6}, {K_TILES_DUMP, h->smem_k6},
+                                        {K_TILES_FAST_G, h->smem_k6}, {K_TILES_DET_G, h->smem_k6}, {K_TILES_DET_TEMP_G, h->smem_k6}};
   for (auto& e : sm)
     if (r.cuFuncSetAttribute(h->fn[e.k], CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES, (int)e.b) != 0)
       return fail(nullptr, TPCCLUS_ERR_CUDA, std::string("cuFuncSetAttribute: ") + kKernelNames[e.k]);
@@ -421,7 +427,8 @@ int tpcclus_create(const tpcclus_params* p, tpcclus_handle** out) {
     if (rc != TPCCLUS_OK) return bail(rc);
   } else {
     struct { int k; uint32_t b; } sm[] = {{K_PART_COARSE, h->smem_k1}, {K_PART_FINE, h->smem_k5}, {K_TILES_FAST, h->smem_k6},
-                                          {K_TILES_DET, h->smem_k6}, {K_TILES_DET_TEMP, h->smem_k6}, {K_TILES_DUMP, h->smem_k6}};
+                                          {K_TILES_DET, h->smem_k6}, {K_TILES_DET_TEMP, h->smem_k6}, {K_TILES_DUMP, h->smem_k6},
+                                        {K_TILES_FAST_G, h->smem_k6}, {K_TILES_DET_G, h->smem_k6}, {K_TILES_DET_TEMP_G, h->smem_k6}};
     for (auto& s : sm) {
       e = cudaFuncSetAttribute(kKernelPtrs[s.k], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s.b);
       if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("cudaFuncSetAttribute(") + kKernelNames[s.k] + "): " + cudaGetErrorString(e); return bail(TPCCLUS_ERR_CUDA); }
@@ -576,15 +583,16 @@ static int run_impl(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n
   a.tile_base = p.tile_base; a.tile_cnt = p.tile_cnt; a.det_flag = p.det_flag;
   a.dmap = nullptr; a.row_off = p.row_off;
   void* ka[] = {&a};
+  const bool gated = h->g.prm.cog_gated != 0u;   // reading Q10': its own kernel variants
   if (mode == TPCCLUS_MODE_FAST) {
     CUDA_TRY(h, cudaMemsetAsync(o_n, 0, 8, st));
-    if ((rc = launch(h, K_TILES_FAST, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
+    if ((rc = launch(h, gated ? K_TILES_FAST_G : K_TILES_FAST, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
   } else {
     // ordered output (PAPER.md 47-50): runs into the temporary buffer, scan of the tile counts,
     // ordered copy.  Should the buffer be too small (more than max_digits/8 clusters) the flag is
     // set, K9 does nothing and the chained-scan K6 redoes the frame; otherwise that launch exits at once.
     const Geometry& g = h->g;
-    if ((rc = launch(h, K_TILES_DET_TEMP, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
+    if ((rc = launch(h, gated ? K_TILES_DET_TEMP_G : K_TILES_DET_TEMP, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
     u32 nt = g.n_tiles, nblk = g.n_scan_blocks;
     { void* s[] = {&p.tile_cnt, &p.tile_local, &p.block_sum, &nt};
       if ((rc = launch(h, K_SCAN_LOCAL, dim3(nblk), dim3(TPC_SCAN_THREADS), 0, st, s))) return rc; }
@@ -600,7 +608,7 @@ static int run_impl(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n
       void* s[] = {&a.temp, &p.tile_base, &p.tile_cnt, &p.tile_local, &p.block_prefix, &nt, &o, &cap, &p.det_flag, &status};
       if ((rc = launch(h, K_EMIT_ORDERED, dim3(g.g1 * 8u), dim3(256), 0, st, s))) return rc;
       CUDA_TRY(h, cudaMemsetAsync(p.ticket, 0, 4, st));
-      if ((rc = launch(h, K_TILES_DET, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
+      if ((rc = launch(h, gated ? K_TILES_DET_G : K_TILES_DET, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
     }
   }
   h->ran = true;

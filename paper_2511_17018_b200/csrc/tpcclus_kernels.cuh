@@ -47,7 +47,7 @@ struct TpcParams {
   u32 max_pads;
   u32 thr_peak, noise_eps;
   u32 max_peaks;   // capacity of the per-tile peak list
-  u32 pad_[1];
+  u32 cog_gated;   // Q10' (host side only: selects the *_gated kernel variants)
   u16 n_pads[256];
 };
 
@@ -922,7 +922,7 @@ __device__ __forceinline__ u32 k6_stage(const K6Smem& s, const K6Args& a, u64 ib
   return pos;
 }
 
-template <int MODE>
+template <int MODE, bool GATED>
 __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
   const K6Smem s = k6_smem(smem);
   const u32 nb = PRM(n_bins), nsl = PRM(n_sl), pitch = PRM(pitch);
@@ -1331,15 +1331,40 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       // different rows are independent (short dependency chains; any order gives the same bits)
       u32 Q = 0u, Spp = 0u, Stt = 0u;
       int Sp = 0, St = 0;
+      if (!GATED) {   // Q10: every in-range cell, weight 1 (the reading is a kernel variant: no run-time test)
 #pragma unroll
-      for (int dt = -2; dt <= 2; ++dt) {
-        const u16* cr = c + dt * (int)pitch;
-        const u32 a = cr[-2], b = cr[-1], m = cr[0], d = cr[1], e2 = cr[2];
-        const u32 rq = (a + b) + (m + d) + e2;
-        const int rsp = (int)(2u * e2 + d) - (int)(2u * a + b);
-        const u32 rspp = 4u * (a + e2) + (b + d);
-        Q += rq; Sp += rsp; Spp += rspp;
-        St += (int)rq * dt; Stt += rq * (u32)(dt * dt);
+        for (int dt = -2; dt <= 2; ++dt) {
+          const u16* cr = c + dt * (int)pitch;
+          const u32 a = cr[-2], b = cr[-1], m = cr[0], d = cr[1], e2 = cr[2];
+          const u32 rq = (a + b) + (m + d) + e2;
+          const int rsp = (int)(2u * e2 + d) - (int)(2u * a + b);
+          const u32 rspp = 4u * (a + e2) + (b + d);
+          Q += rq; Sp += rsp; Spp += rspp;
+          St += (int)rq * dt; Stt += rq * (u32)(dt * dt);
+        }
+      } else {                 // Q10': an outer-ring cell counts only if the inner cell towards the peak holds charge
+        u32 w5[5][5];
+#pragma unroll
+        for (int dt = -2; dt <= 2; ++dt)
+#pragma unroll
+          for (int dp = -2; dp <= 2; ++dp) w5[dt + 2][dp + 2] = c[dt * (int)pitch + dp];
+#pragma unroll
+        for (int dt = -2; dt <= 2; ++dt)
+#pragma unroll
+          for (int dp = -2; dp <= 2; ++dp)
+            if (dt == -2 || dt == 2 || dp == -2 || dp == 2) {
+              const int it = dt < -1 ? -1 : (dt > 1 ? 1 : dt), ip = dp < -1 ? -1 : (dp > 1 ? 1 : dp);
+              if (w5[it + 2][ip + 2] == 0u) w5[dt + 2][dp + 2] = 0u;
+            }
+#pragma unroll
+        for (int dt = -2; dt <= 2; ++dt) {
+          const u32 a = w5[dt + 2][0], b = w5[dt + 2][1], m = w5[dt + 2][2], d = w5[dt + 2][3], e2 = w5[dt + 2][4];
+          const u32 rq = (a + b) + (m + d) + e2;
+          const int rsp = (int)(2u * e2 + d) - (int)(2u * a + b);
+          const u32 rspp = 4u * (a + e2) + (b + d);
+          Q += rq; Sp += rsp; Spp += rspp;
+          St += (int)rq * dt; Stt += rq * (u32)(dt * dt);
+        }
       }
       const int Vp = (int)(Q * Spp) - Sp * Sp, Vt = (int)(Q * Stt) - St * St;
       const u32 qc = c[0];
@@ -1387,20 +1412,19 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
   }
 }
 
-extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, TPC_K6_CTAS) k_cluster_tiles_fast(K6Args a) {
-  extern __shared__ __align__(128) u32 smem_u32[];
-  k6_body<TPC_MODE_FAST>(a, smem_u32);
-}
-extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, TPC_K6_CTAS) k_cluster_tiles_det(K6Args a) {
-  extern __shared__ __align__(128) u32 smem_u32[];
-  if (*a.det_flag == 0u) return;   // K7-K9 already delivered the ordered output
-  k6_body<TPC_MODE_DET>(a, smem_u32);
-}
-extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, TPC_K6_CTAS) k_cluster_tiles_det_temp(K6Args a) {
-  extern __shared__ __align__(128) u32 smem_u32[];
-  k6_body<TPC_MODE_DET_TEMP>(a, smem_u32);
-}
-extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, TPC_K6_CTAS) k_cluster_tiles_dump_map(K6Args a) {
-  extern __shared__ __align__(128) u32 smem_u32[];
-  k6_body<TPC_MODE_DUMP_MAP>(a, smem_u32);
-}
+#define TPC_K6_ENTRY(name, MODE, GATED, GUARD)                                                          \
+  extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, TPC_K6_CTAS) name(K6Args a) {             \
+    extern __shared__ __align__(128) u32 smem_u32[];                                                    \
+    GUARD                                                                                               \
+    k6_body<MODE, GATED>(a, smem_u32);                                                                  \
+  }
+// the chained-scan variants only run when K7-K9 could not deliver the ordered output (flag set)
+#define TPC_K6_IF_FLAG if (*a.det_flag == 0u) return;
+TPC_K6_ENTRY(k_cluster_tiles_fast, TPC_MODE_FAST, false, )
+TPC_K6_ENTRY(k_cluster_tiles_det, TPC_MODE_DET, false, TPC_K6_IF_FLAG)
+TPC_K6_ENTRY(k_cluster_tiles_det_temp, TPC_MODE_DET_TEMP, false, )
+TPC_K6_ENTRY(k_cluster_tiles_dump_map, TPC_MODE_DUMP_MAP, false, )
+// reading Q10' (TPCCLUS_COG_GATED)
+TPC_K6_ENTRY(k_cluster_tiles_fast_gated, TPC_MODE_FAST, true, )
+TPC_K6_ENTRY(k_cluster_tiles_det_gated, TPC_MODE_DET, true, TPC_K6_IF_FLAG)
+TPC_K6_ENTRY(k_cluster_tiles_det_temp_gated, TPC_MODE_DET_TEMP, true, )

@@ -462,3 +462,21 @@ def test_packed_output_and_row_index(tp, cuda_device):
     torch.cuda.synchronize()
     assert int(nt.item()) == len(d) and int(st.item()) == tp.STATUS_NO_PACKED
     c.close()
+
+
+def test_cog_gated_reading(tp, cuda_device):
+    """Reading Q10' (TPCCLUS_COG_GATED): outer-ring gating of the CoG window,
+    byte for byte against the oracle in the same reading -- deterministic, fast, generic and RTC."""
+    frames = [make_frame(1), make_frame(0), make_frame(4, device=cuda_device, sectors=[3, 20], n_time=300)]
+    for fr in frames:
+        d_np = fr.digits_numpy()
+        exp, st, n = t1.clusterize(d_np.view(t1.DIGIT), fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, cog_gated=True)
+        plain, _ = _oracle(d_np, fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads)
+        assert exp.tobytes() != plain.tobytes() and len(exp) == len(plain)      # the reading matters on these frames
+        for rtc in (False, True):
+            c = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, fr.n_digits, rtc=rtc, cog_gated=True)
+            det = c.run_sync(fr.digits.to(cuda_device), tp.MODE_DETERMINISTIC)[0]
+            fast = c.run_sync(fr.digits.to(cuda_device), tp.MODE_FAST)[0]
+            c.close()
+            assert det.tobytes() == exp.tobytes(), (fr.meta["name"], rtc)
+            _check_fast(fast, exp)
