@@ -1053,21 +1053,25 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       u32 nu = total - round * TPC_K6_CAPU;
       if (nu > TPC_K6_CAPU) nu = TPC_K6_CAPU;
       const uint4* r4 = (const uint4*)rec;
-      for (u32 u = tid; u < nu; u += TPC_K6_CONSUMERS) {
-        const uint4 v = r4[u];
-        const u32 rr[4] = {v.x, v.y, v.z, v.w};
+      if (MODE == TPC_MODE_FAST || round == 0u) {   // plain stores: FAST may keep either of two digits on one
+                                                    // cell (Q5); DET: the map is still empty in round 0, the loop below settles it
+        for (u32 u = tid; u < nu; u += TPC_K6_CONSUMERS) {
+          const uint4 v = r4[u];
+          const u32 rr[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
-        for (int k = 0; k < 4; ++k)
-          if (rr[k] != 0u) {   // 0 = batch padding (every real record has q >= 1)
-            const u32 tl = k6_row(rr[k], sl);
-            if (tl < TPC_TT) s.tile[tl * pitch + (rr[k] & 0xFFu) + TPC_HALO] = (u16)((rr[k] >> 16) & 0x3FFu);
-          }
+          for (int k = 0; k < 4; ++k)
+            if (rr[k] != 0u) {   // 0 = batch padding (every real record has q >= 1)
+              const u32 tl = k6_row(rr[k], sl);
+              if (tl < TPC_TT) s.tile[tl * pitch + (rr[k] & 0xFFu) + TPC_HALO] = (u16)((rr[k] >> 16) & 0x3FFu);
+            }
+        }
       }
       if (MODE != TPC_MODE_FAST) {
-        // Q5, deterministic: two digits on one cell -> the maximum, whatever the order.  Re-check
-        // until stable; with duplicate-free input this is one read per record and one barrier.
-        for (;;) {
-          csync();
+        // Q5, deterministic: two digits on one cell -> the maximum, whatever the order and however
+        // many staging rounds the tile takes: from here on a cell is only ever raised, and the pass
+        // repeats until no record is larger than its cell.  Duplicate-free input: one confirming pass.
+        if (round == 0u) csync();
+        for (;;) {   // passes are separated by the barrier inside csync_or
           u32 any = 0u;
           for (u32 u = tid; u < nu; u += TPC_K6_CONSUMERS) {
             const uint4 v = r4[u];

@@ -480,3 +480,45 @@ def test_cog_gated_reading(tp, cuda_device):
             c.close()
             assert det.tobytes() == exp.tobytes(), (fr.meta["name"], rtc)
             _check_fast(fast, exp)
+
+
+def test_random_geometries_fuzz(tp, cuda_device):
+    """Seeded fuzz over the parameter space the five configs do not span: odd sector/row counts,
+    pad rows from 1 to 256 pads, time lengths around the tile and time-chunk borders, thresholds,
+    duplicates and out-of-range digits.  Deterministic = byte-identical, fast = same set; status equal."""
+    rng = np.random.default_rng(77)
+    cases = [(1, 1, 1, [1]), (2, 3, 127, [1, 2, 256]), (3, 2, 128, [255, 7]), (1, 4, 129, [33, 64, 65, 250]),
+             (2, 2, 262, [138, 66]), (1, 2, 16255, [20, 9]), (1, 1, 16257, [12]), (1, 1, 16262, [40])]
+    for (S, R, T, pads) in cases:
+        for thr, eps, dens in ((6, 4, 0.25), (1, 0, 0.6), (40, 1023, 0.08)):
+            cells = int(sum(pads)) * T * S
+            n = max(1, min(int(cells * dens), 60000))
+            d = np.zeros(n, dtype=t1.DIGIT)
+            d["sector"] = rng.integers(0, S, n)
+            d["row"] = rng.integers(0, R, n)
+            d["pad"] = rng.integers(0, 256, n) % np.asarray(pads)[d["row"]]
+            # cluster the digits in time so that peaks, ridges and ties actually occur
+            d["time"] = (rng.integers(0, max(T // 8, 1), n) * 8 + rng.integers(0, 8, n)) % T
+            d["charge"] = np.where(rng.random(n) < 0.3, rng.integers(1, 12, n), rng.integers(1, 1100, n))
+            k = max(1, n // 50)                       # a few bad ones: pad, time, row, sector out of range; zero charge
+            bad = rng.integers(0, n, k)
+            d["pad"][bad[: k // 4]] = 255 if max(pads) < 256 else d["pad"][bad[: k // 4]]
+            d["charge"][bad[k // 4: k // 2]] = 0
+            if T < 65535:
+                d["time"][bad[k // 2: 3 * k // 4]] = T
+            d["row"][bad[3 * k // 4:]] = R
+            exp, st_exp = _oracle(d, S, R, T, pads, thr, eps)
+            det, _, st = _run_both(tp, _digits_tensor(d, cuda_device), S, R, T, pads, thr, eps)
+            assert st == st_exp, (S, R, T, pads, thr, eps, st, st_exp)
+            assert det.tobytes() == exp.tobytes(), (S, R, T, pads, thr, eps)    # duplicates: the maximum wins (Q5)
+            # FAST promises the same set for duplicate-free input only (Q5): one digit per cell, the largest
+            order = np.lexsort((-d["charge"].astype(np.int64), d["pad"], d["time"], d["row"], d["sector"]))
+            ds = d[order]
+            first = np.ones(len(ds), dtype=bool)
+            first[1:] = (ds["pad"][1:] != ds["pad"][:-1]) | (ds["time"][1:] != ds["time"][:-1]) | \
+                (ds["row"][1:] != ds["row"][:-1]) | (ds["sector"][1:] != ds["sector"][:-1])
+            du = ds[first][rng.permutation(int(first.sum()))]
+            exp_u, _ = _oracle(du, S, R, T, pads, thr, eps)
+            assert exp_u.tobytes() == exp.tobytes()                               # the oracle agrees: max per cell
+            _, fast, _ = _run_both(tp, _digits_tensor(du, cuda_device), S, R, T, pads, thr, eps)
+            _check_fast(fast, exp)
