@@ -488,7 +488,8 @@ def test_random_geometries_fuzz(tp, cuda_device):
     duplicates and out-of-range digits.  Deterministic = byte-identical, fast = same set; status equal."""
     rng = np.random.default_rng(77)
     cases = [(1, 1, 1, [1]), (2, 3, 127, [1, 2, 256]), (3, 2, 128, [255, 7]), (1, 4, 129, [33, 64, 65, 250]),
-             (2, 2, 262, [138, 66]), (1, 2, 16255, [20, 9]), (1, 1, 16257, [12]), (1, 1, 16262, [40])]
+             (2, 2, 262, [138, 66]), (1, 2, 16255, [20, 9]), (1, 1, 16257, [12]), (1, 1, 16262, [40]),
+             (1, 1, 65536, [5]), (2, 1, 40000, [256]), (7, 5, 300, [17, 30, 1, 99, 140])]
     for (S, R, T, pads) in cases:
         for thr, eps, dens in ((6, 4, 0.25), (1, 0, 0.6), (40, 1023, 0.08)):
             cells = int(sum(pads)) * T * S
@@ -505,7 +506,7 @@ def test_random_geometries_fuzz(tp, cuda_device):
             d["pad"][bad[: k // 4]] = 255 if max(pads) < 256 else d["pad"][bad[: k // 4]]
             d["charge"][bad[k // 4: k // 2]] = 0
             if T < 65535:
-                d["time"][bad[k // 2: 3 * k // 4]] = T
+                d["time"][bad[k // 2: 3 * k // 4]] = T   # (T = 65536 cannot be exceeded in 16 bits)
             d["row"][bad[3 * k // 4:]] = R
             exp, st_exp = _oracle(d, S, R, T, pads, thr, eps)
             det, _, st = _run_both(tp, _digits_tensor(d, cuda_device), S, R, T, pads, thr, eps)
