@@ -1066,7 +1066,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
             }
         }
       }
-      if (MODE != TPC_MODE_FAST) {
+      if (MODE != TPC_MODE_FAST && total > TPC_K6_CAPU) {   // (a single-round tile checks in its peak pass instead)
         // Q5, deterministic: two digits on one cell -> the maximum, whatever the order and however
         // many staging rounds the tile takes: from here on a cell is only ever raised, and the pass
         // repeats until no record is larger than its cell.  Duplicate-free input: one confirming pass.
@@ -1120,40 +1120,78 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
     // the occupancy, not the tile area; a tile that needed several staging rounds takes the
     // dense scan below instead.  A peak sets its bit in pmask (which also removes duplicates of
     // one cell); the peaks of owned rows go into the list the later phases walk.
+    bool d_done = false;   // block-uniform: barrier D already passed
     if (sparse) {
       const u32 nW = pitch >> 1;
       const uint4* r4 = (const uint4*)rec;
-      for (u32 u = tid; u < total; u += TPC_K6_CONSUMERS) {
-        const uint4 v = r4[u];
-        const u32 rr[4] = {v.x, v.y, v.z, v.w};
-        // the four records of a piece are independent: all their loads are issued before any test
-        u32 pu[4], nu[4], pm[4], nm[4], pd[4], nd[4];
-        bool cand[4];
+      // `check` (DET): also verify that no cell holds less than one of its records -- the plain
+      // stores of the scatter may have left a smaller duplicate on top (Q5)
+      auto peak_pass = [&](const bool check) -> u32 {
+        u32 viol = 0u;
+        for (u32 u = tid; u < total; u += TPC_K6_CONSUMERS) {
+          const uint4 v = r4[u];
+          const u32 rr[4] = {v.x, v.y, v.z, v.w};
+          // the four records of a piece are independent: all their loads are issued before any test
+          u32 pu[4], nu[4], pm[4], nm[4], pd[4], nd[4];
+          bool cand[4];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          const u32 q = (rr[k] >> 16) & 0x3FFu, tl = k6_row(rr[k], sl), pad = rr[k] & 0xFFu;
-          cand[k] = q >= thr && tl - 1u < TPC_TT - 2u;   // (q = 0 for run padding)
-          const u32 x = pad + TPC_HALO, h = x & 1u, sh = 16u - 16u * h;
-          const u32* w = s.tile32 + (cand[k] ? (tl - 1u) * nW + (x >> 1) - 1u + h : 0u);
-          pu[k] = __funnelshift_r(w[0], w[1], sh); nu[k] = (w[1] >> sh) & 0xFFFFu;
-          w += nW;
-          pm[k] = __funnelshift_r(w[0], w[1], sh); nm[k] = (w[1] >> sh) & 0xFFFFu;
-          w += nW;
-          pd[k] = __funnelshift_r(w[0], w[1], sh); nd[k] = (w[1] >> sh) & 0xFFFFu;
-        }
+          for (int k = 0; k < 4; ++k) {
+            const u32 q = (rr[k] >> 16) & 0x3FFu, tl = k6_row(rr[k], sl), pad = rr[k] & 0xFFu;
+            cand[k] = q >= thr && tl - 1u < TPC_TT - 2u;   // (q = 0 for run padding)
+            if (check && !cand[k] && rr[k] != 0u && tl < TPC_TT && s.tile[tl * pitch + pad + TPC_HALO] < q) viol = 1u;
+            const u32 x = pad + TPC_HALO, h = x & 1u, sh = 16u - 16u * h;
+            const u32* w = s.tile32 + (cand[k] ? (tl - 1u) * nW + (x >> 1) - 1u + h : 0u);
+            pu[k] = __funnelshift_r(w[0], w[1], sh); nu[k] = (w[1] >> sh) & 0xFFFFu;
+            w += nW;
+            pm[k] = __funnelshift_r(w[0], w[1], sh); nm[k] = (w[1] >> sh) & 0xFFFFu;
+            w += nW;
+            pd[k] = __funnelshift_r(w[0], w[1], sh); nd[k] = (w[1] >> sh) & 0xFFFFu;
+          }
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          const u32 q = (rr[k] >> 16) & 0x3FFu, tl = k6_row(rr[k], sl), pad = rr[k] & 0xFFu;
-          const u32 e = max(max(pu[k] & 0xFFFFu, pu[k] >> 16), max(nu[k], pm[k] & 0xFFFFu));
-          const u32 l = max(max(pd[k] & 0xFFFFu, pd[k] >> 16), max(nd[k], nm[k]));
-          if (cand[k] && (pm[k] >> 16) == q && q > e && q >= l) {   // (!= q: a smaller duplicate of this cell)
-            const u32 bit = 1u << ((pad + 2u) & 31u);
-            const u32 old = atomicOr(&s.pmask[tl * TPC_K6_PMW + ((pad + 2u) >> 5)], bit);
-            if (!(old & bit) && tl >= TPC_HALO && tl < TPC_TS + TPC_HALO) {   // a halo-row peak is emitted by its own tile
-              const u32 i = atomicAdd(&s.misc[0], 1u);
-              s.peaks[i] = (u16)((tl << 8) | pad);
+          for (int k = 0; k < 4; ++k) {
+            const u32 q = (rr[k] >> 16) & 0x3FFu, tl = k6_row(rr[k], sl), pad = rr[k] & 0xFFu;
+            const u32 e = max(max(pu[k] & 0xFFFFu, pu[k] >> 16), max(nu[k], pm[k] & 0xFFFFu));
+            const u32 l = max(max(pd[k] & 0xFFFFu, pd[k] >> 16), max(nd[k], nm[k]));
+            if (check && cand[k] && (pm[k] >> 16) < q) viol = 1u;   // the cell holds a smaller duplicate of this record (Q5)
+            if (cand[k] && (pm[k] >> 16) == q && q > e && q >= l) {   // (!= q: a smaller duplicate of this cell)
+              const u32 bit = 1u << ((pad + 2u) & 31u);
+              const u32 old = atomicOr(&s.pmask[tl * TPC_K6_PMW + ((pad + 2u) >> 5)], bit);
+              if (!(old & bit) && tl >= TPC_HALO && tl < TPC_TS + TPC_HALO) {   // a halo-row peak is emitted by its own tile
+                const u32 i = atomicAdd(&s.misc[0], 1u);
+                s.peaks[i] = (u16)((tl << 8) | pad);
+              }
             }
           }
+        }
+        return viol;
+      };
+      if (MODE == TPC_MODE_FAST) {
+        peak_pass(false);
+      } else {
+        d_done = true;
+        if (csync_or(peak_pass(true))) {   // rare: duplicates in this tile.  Settle the maxima, forget the peaks, test again.
+          for (;;) {
+            u32 any = 0u;
+            for (u32 u = tid; u < total; u += TPC_K6_CONSUMERS) {
+              const uint4 v = r4[u];
+              const u32 rr[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+              for (int k = 0; k < 4; ++k) {
+                const u32 tl = k6_row(rr[k], sl);
+                if (rr[k] != 0u && tl < TPC_TT) {
+                  const u32 cell = tl * pitch + (rr[k] & 0xFFu) + TPC_HALO;
+                  const u16 q = (u16)((rr[k] >> 16) & 0x3FFu);
+                  if (s.tile[cell] < q) { s.tile[cell] = q; any = 1u; }
+                }
+              }
+            }
+            if (!csync_or(any)) break;
+          }
+          for (u32 i = tid; i < TPC_TT * TPC_K6_PMW; i += TPC_K6_CONSUMERS) s.pmask[i] = 0u;
+          if (tid == 0) s.misc[0] = 0u;
+          csync();
+          peak_pass(false);
+          csync();
         }
       }
       __syncwarp();
@@ -1225,7 +1263,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
         }
       }
     }
-    csync();   // D: peak set complete
+    if (!d_done) csync();   // D: peak set complete
     const u32 npk = s.misc[0];
 
     // ---- O2: suppression of the owned peaks against the un-updated peak set -----------------
