@@ -1131,7 +1131,10 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
         for (u32 u = tid; u < total; u += TPC_K6_CONSUMERS) {
           const uint4 v = r4[u];
           const u32 rr[4] = {v.x, v.y, v.z, v.w};
-          // the four records of a piece are independent: all their loads are issued before any test
+          // the four records of a piece are independent: their loads are issued together, in two
+          // stages -- the own row first (two thirds of the candidates already lose against a pad
+          // neighbour there), then the rows above and below for those still in the race; the others
+          // read word 0, a broadcast that costs no bank conflict
           u32 pu[4], nu[4], pm[4], nm[4], pd[4], nd[4];
           bool cand[4];
 #pragma unroll
@@ -1140,20 +1143,26 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
             cand[k] = q >= thr && tl - 1u < TPC_TT - 2u;   // (q = 0 for run padding)
             if (check && !cand[k] && rr[k] != 0u && tl < TPC_TT && s.tile[tl * pitch + pad + TPC_HALO] < q) viol = 1u;
             const u32 x = pad + TPC_HALO, h = x & 1u, sh = 16u - 16u * h;
+            const u32* w = s.tile32 + (cand[k] ? tl * nW + (x >> 1) - 1u + h : 0u);
+            pm[k] = __funnelshift_r(w[0], w[1], sh); nm[k] = (w[1] >> sh) & 0xFFFFu;
+          }
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            const u32 q = (rr[k] >> 16) & 0x3FFu, tl = k6_row(rr[k], sl), pad = rr[k] & 0xFFu;
+            if (check && cand[k] && (pm[k] >> 16) < q) viol = 1u;   // the cell holds a smaller duplicate of this record (Q5)
+            cand[k] = cand[k] && (pm[k] >> 16) == q && q > (pm[k] & 0xFFFFu) && q >= nm[k];   // (!= q: a smaller duplicate of this cell)
+            const u32 x = pad + TPC_HALO, h = x & 1u, sh = 16u - 16u * h;
             const u32* w = s.tile32 + (cand[k] ? (tl - 1u) * nW + (x >> 1) - 1u + h : 0u);
             pu[k] = __funnelshift_r(w[0], w[1], sh); nu[k] = (w[1] >> sh) & 0xFFFFu;
-            w += nW;
-            pm[k] = __funnelshift_r(w[0], w[1], sh); nm[k] = (w[1] >> sh) & 0xFFFFu;
-            w += nW;
+            w += 2u * nW;
             pd[k] = __funnelshift_r(w[0], w[1], sh); nd[k] = (w[1] >> sh) & 0xFFFFu;
           }
 #pragma unroll
           for (int k = 0; k < 4; ++k) {
             const u32 q = (rr[k] >> 16) & 0x3FFu, tl = k6_row(rr[k], sl), pad = rr[k] & 0xFFu;
-            const u32 e = max(max(pu[k] & 0xFFFFu, pu[k] >> 16), max(nu[k], pm[k] & 0xFFFFu));
-            const u32 l = max(max(pd[k] & 0xFFFFu, pd[k] >> 16), max(nd[k], nm[k]));
-            if (check && cand[k] && (pm[k] >> 16) < q) viol = 1u;   // the cell holds a smaller duplicate of this record (Q5)
-            if (cand[k] && (pm[k] >> 16) == q && q > e && q >= l) {   // (!= q: a smaller duplicate of this cell)
+            const u32 e = max(max(pu[k] & 0xFFFFu, pu[k] >> 16), nu[k]);
+            const u32 l = max(max(pd[k] & 0xFFFFu, pd[k] >> 16), nd[k]);
+            if (cand[k] && q > e && q >= l) {
               const u32 bit = 1u << ((pad + 2u) & 31u);
               const u32 old = atomicOr(&s.pmask[tl * TPC_K6_PMW + ((pad + 2u) >> 5)], bit);
               if (!(old & bit) && tl >= TPC_HALO && tl < TPC_TS + TPC_HALO) {   // a halo-row peak is emitted by its own tile
