@@ -523,3 +523,43 @@ def test_random_geometries_fuzz(tp, cuda_device):
             assert exp_u.tobytes() == exp.tobytes()                               # the oracle agrees: max per cell
             _, fast, _ = _run_both(tp, _digits_tensor(du, cuda_device), S, R, T, pads, thr, eps)
             _check_fast(fast, exp)
+
+
+def test_handle_reuse_sizes_and_geometries(tp, cuda_device):
+    """One handle fed frames of very different sizes (large, small, empty, large again), capacity 1,
+    and two generic handles of different geometry alternating on one stream (R6: one __constant__
+    block, re-uploaded per run): every run equals the oracle, nothing leaks from run to run."""
+    import torch
+    big, small = make_frame(0), make_frame(0, seed=5, n_time=64)
+    c = tp.Clusterizer(big.n_sectors, big.n_rows, big.n_time, big.n_pads, big.n_digits)
+    sub = big.digits_numpy().view(t1.DIGIT)
+    sub = sub[(sub["time"] < 40) & (sub["row"] < 3)]
+    empty = torch.zeros(0, dtype=torch.int64, device=cuda_device)
+    for d_np in (big.digits_numpy(), sub, None, big.digits_numpy()):
+        if d_np is None:
+            for mode in (tp.MODE_DETERMINISTIC, tp.MODE_FAST):
+                cl, n, st = c.run_sync(empty, mode)
+                assert n == 0 and st == 0 and len(cl) == 0
+            continue
+        exp, _ = _oracle(d_np, big.n_sectors, big.n_rows, big.n_time, big.n_pads)
+        dt = _digits_tensor(np.ascontiguousarray(d_np).view(np.uint64), cuda_device)
+        assert c.run_sync(dt, tp.MODE_DETERMINISTIC)[0].tobytes() == exp.tobytes()
+        _check_fast(c.run_sync(dt, tp.MODE_FAST)[0], exp)
+        # capacity 1: the count is still the true one, the overflow is flagged
+        for mode in (tp.MODE_DETERMINISTIC, tp.MODE_FAST):
+            cl, n, st = c.run_sync(dt, mode, capacity=1)
+            assert n == len(exp) and (st == tp.STATUS_OVERFLOW) == (len(exp) > 1)
+            if mode == tp.MODE_DETERMINISTIC:
+                assert cl.tobytes() == exp[:1].tobytes()
+    # a second handle with another geometry, alternating with the first on the same stream
+    c2 = tp.Clusterizer(small.n_sectors, small.n_rows, small.n_time, small.n_pads, small.n_digits, thr_peak=9)
+    exp_b, _ = _oracle(big.digits_numpy(), big.n_sectors, big.n_rows, big.n_time, big.n_pads)
+    exp_s, _ = _oracle(small.digits_numpy(), small.n_sectors, small.n_rows, small.n_time, small.n_pads, 9, 4)
+    db, ds = big.digits.to(cuda_device), small.digits.to(cuda_device)
+    for _ in range(3):
+        rb = c.run(db, tp.MODE_DETERMINISTIC)
+        rs = c2.run(ds, tp.MODE_DETERMINISTIC)      # enqueued right behind, no sync in between
+        torch.cuda.synchronize()
+        assert rb[0][:int(rb[1].item())].cpu().numpy().tobytes() == exp_b.tobytes()
+        assert rs[0][:int(rs[1].item())].cpu().numpy().tobytes() == exp_s.tobytes()
+    c.close(); c2.close()
