@@ -660,6 +660,10 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
     // ---- <= 16 records per thread: count per key, remember the rank -------------------------
     u32 rec[16];
     u32 rank[8];
+    // Does this warp's share of the batch look time-ordered (its first 32 records in one slab)?
+    // Only then is it worth testing every warp step for a common key (see below).
+    int agg;
+    __match_all_sync(0xFFFFFFFFu, ((vn[0].x >> 8) & 0x3FFFu) / TPC_TS, &agg);
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
       const u32 sub = (threadIdx.x + (u32)i * TPC_K5_THREADS) & 15u;
@@ -672,10 +676,22 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
         u32 r = r4[j];   // q >= 1 in every valid record, so 0 = none
         if ((r & 0xFFu) >= npads && r != 0u) { r = 0u; bad = true; }   // O0 / Q4: pad out of range -> ignored + flagged
         u32 rk = 0u;
-        if (r != 0u) {
+        {
           const u32 u = (r >> 8) & 0x3FFFu;
-          const u32 key = 2u * (u / TPC_TS) + ((u % TPC_TS) >= 2u * TPC_HALO ? 1u : 0u);   // <= 2 * nsl (u < TC + 6)
-          rk = atomicAdd(&s_cnt[key], 1u);
+          const u32 key = r != 0u ? 2u * (u / TPC_TS) + ((u % TPC_TS) >= 2u * TPC_HALO ? 1u : 0u) : 0xFFFFFFFFu;   // <= 2 * nsl (u < TC + 6)
+          // time-ordered input (readout order) puts the 32 records of a warp step into ONE run: then a
+          // single atomic serves the warp; otherwise (shuffled input: ~28 different keys) one per record
+          int same = 0;
+          if (agg) __match_all_sync(0xFFFFFFFFu, key, &same);
+          if (same) {
+            if (key != 0xFFFFFFFFu) {
+              u32 base = 0u;
+              if (lane_id() == 0u) base = atomicAdd(&s_cnt[key], 32u);
+              rk = __shfl_sync(0xFFFFFFFFu, base, 0) + lane_id();
+            }
+          } else if (r != 0u) {
+            rk = atomicAdd(&s_cnt[key], 1u);
+          }
         }
         rec[i * 4 + j] = r;
         if (j & 1) rank[i * 2 + (j >> 1)] |= rk << 16; else rank[i * 2 + (j >> 1)] = rk;
