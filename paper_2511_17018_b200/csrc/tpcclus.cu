@@ -413,7 +413,7 @@ int tpcclus_create(const tpcclus_params* p, tpcclus_handle** out) {
   h->smem_k1 = tpc_k1_smem_bytes(g.prm.n_bins);
   h->smem_k5 = tpc_k5_smem_bytes();
   h->smem_k6 = tpc_k6_smem_bytes(g.prm.pitch, g.prm.max_peaks);
-  h->grid_k5 = g.g1 * 2u;
+  h->grid_k5 = g.g1;
   h->grid_k6 = g.g1 * TPC_K6_CTAS < g.n_tiles ? g.g1 * TPC_K6_CTAS : g.n_tiles;
   auto bail = [&](int code) { std::string e = h->err.empty() ? g_create_error : h->err; delete h; g_create_error = e; return code; };
   // static table for the debug map hook

@@ -28,10 +28,10 @@ typedef unsigned char u8;
 #define TPC_TC 16256u          // time bins per coarse time-chunk: 127*128, +6 halo < 2^14
 #define TPC_STAGE 8u           // records (32 B) staged per coarse bin in K1
 #define TPC_CHUNK 64u          // records per pool chunk (256 B)
-#define TPC_CPB 128u           // chunks per K5 batch (<= 8192 records)
+#define TPC_CPB 256u           // chunks per K5 batch (<= 16384 records)
 #define TPC_K1_THREADS 1024
 #define TPC_K1_DPT 4           // digits per thread per round
-#define TPC_K5_THREADS 512
+#define TPC_K5_THREADS 1024
 #define TPC_SCAN_THREADS 1024
 #define TPC_SCAN_PER_CTA 4096u
 
@@ -575,7 +575,7 @@ k_emit_packed(const uint4* __restrict__ temp, const u64* __restrict__ tile_base,
 // K5  partition_fine  (NS (1), second half: group every record with the tile(s) whose shared-
 //     memory charge map needs it)
 //
-// A batch = up to TPC_CPB chunks (<= 8192 records) of ONE coarse bin.  The CTA counting-sorts
+// A batch = up to TPC_CPB chunks (<= 16384 records) of ONE coarse bin.  The CTA counting-sorts
 // the batch in shared memory and writes it as one contiguous blob.  Sort key = 2 * slab + (m >= 6)
 // with u = slab * TS + m: each slab is split into its first 6 rows (A) and the rest (B), so the
 // layout is  A0 B0 A1 B1 A2 ...  and tile `sl`, which needs u in [sl*TS, sl*TS + TS + 6), reads
@@ -597,7 +597,7 @@ k_emit_packed(const uint4* __restrict__ temp, const u64* __restrict__ tile_base,
 #define TPC_K5_BUF (TPC_CPB * TPC_CHUNK + 4u * TPC_NSLMAX + 8u)   // u32 words: the records of a batch + alignment gaps + end padding
 __host__ __device__ inline u32 tpc_k5_smem_bytes() { return (TPC_K5_BUF + 2u * TPC_NKEY + 8u) * 4u; }
 
-extern "C" __global__ void __launch_bounds__(TPC_K5_THREADS, 2)
+extern "C" __global__ void __launch_bounds__(TPC_K5_THREADS, 1)
 k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, const u32* __restrict__ chunk_list,
                  const u32* __restrict__ bin_chunk_start, const u32* __restrict__ batch_start,
                  const u32* __restrict__ batch_bin, u32* __restrict__ blob, u64* __restrict__ blob_cursor,
