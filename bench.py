@@ -40,8 +40,8 @@ def _log(msg):
 
 METRIC = "TPC clusterizer digits/s on Pb-Pb-like time frame"
 # ncu --set full, CFG[4] shuffled FAST generic, one launch each (profiles/r01d_ncu_full_summary.txt)
-NCU_TRAFFIC_BYTES = {"k_partition_coarse": 12766098000 + 6478920000, "k_partition_fine": 9156652000 + 6744179000,
-                     "k_cluster_tiles_fast": 6711538000 + 1900586000}
+NCU_TRAFFIC_BYTES = {"k_partition_coarse": 12764361000 + 6479759000, "k_partition_fine": 9074966000 + 6495987000,
+                     "k_cluster_tiles_fast": 6544173000 + 1900446000}
 UNIT = "digits/s"
 
 
