@@ -277,15 +277,15 @@ int compile_cubin(const std::string& src, std::vector<char>* cubin) {
   void* prog = nullptr;
   if (r.nvrtcCreateProgram(&prog, src.c_str(), "tpcclus_kernels.cu", 0, nullptr, nullptr) != 0)
     return fail(nullptr, TPCCLUS_ERR_NVRTC, "nvrtcCreateProgram failed");
-  const char* opts[] = {"--gpu-architecture=sm_100a", "-std=c++17", "-lineinfo", "--fmad=false", "--prec-div=true",
+  const char* opts[] = {"--gpu-architecture=sm_100a", "-std=c++17", "-default-device", "-lineinfo", "--fmad=false", "--prec-div=true",
                         "--prec-sqrt=true", "--ftz=false", "-DTPC_NO_ST256=1"};
-  int rc = r.nvrtcCompileProgram(prog, 7, opts);
+  int rc = r.nvrtcCompileProgram(prog, 8, opts);
   if (rc != 0) {   // older NVRTC: retry without the 256-bit store
     r.nvrtcDestroyProgram(&prog);
     prog = nullptr;
     if (r.nvrtcCreateProgram(&prog, src.c_str(), "tpcclus_kernels.cu", 0, nullptr, nullptr) != 0)
       return fail(nullptr, TPCCLUS_ERR_NVRTC, "nvrtcCreateProgram failed");
-    rc = r.nvrtcCompileProgram(prog, 8, opts);
+    rc = r.nvrtcCompileProgram(prog, 9, opts);
   }
   if (rc != 0) {
     size_t n = 0; r.nvrtcGetProgramLogSize(prog, &n);

@@ -938,6 +938,7 @@ __device__ __forceinline__ u32 k6_stage(const K6Smem& s, const K6Args& a, u64 ib
   return pos;
 }
 
+template <int V> struct TpcInt { static constexpr int v = V; };
 template <int MODE, bool GATED>
 __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
   const K6Smem s = k6_smem(smem);
@@ -1071,6 +1072,11 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       const uint4* r4 = (const uint4*)rec;
       if (MODE == TPC_MODE_FAST || round == 0u) {   // plain stores: FAST may keep either of two digits on one
                                                     // cell (Q5); DET: the map is still empty in round 0, the loop below settles it
+        if (nu * 4u <= TPC_K6_CONSUMERS) {   // a sparse tile: one record per thread, spread over all warps
+          const u32 r = tid < nu * 4u ? rec[tid] : 0u;
+          const u32 tl = k6_row(r, sl);
+          if (r != 0u && tl < TPC_TT) s.tile[tl * pitch + (r & 0xFFu) + TPC_HALO] = (u16)((r >> 16) & 0x3FFu);
+        } else
         for (u32 u = tid; u < nu; u += TPC_K6_CONSUMERS) {
           const uint4 v = r4[u];
           const u32 rr[4] = {v.x, v.y, v.z, v.w};
@@ -1142,19 +1148,21 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       const uint4* r4 = (const uint4*)rec;
       // `check` (DET): also verify that no cell holds less than one of its records -- the plain
       // stores of the scatter may have left a smaller duplicate on top (Q5)
-      auto peak_pass = [&](const bool check) -> u32 {
+      const u32 nrec = total * 4u;
+      // K records of one thread: K = 4 (a 16-byte piece, the loads of the four in flight together)
+      // or K = 1 (a sparse tile: one record per thread, spread over all warps)
+      auto peak_recs = [&](auto kt, const u32* rr, const bool check) -> u32 {
+        constexpr int K = decltype(kt)::v;
         u32 viol = 0u;
-        for (u32 u = tid; u < total; u += TPC_K6_CONSUMERS) {
-          const uint4 v = r4[u];
-          const u32 rr[4] = {v.x, v.y, v.z, v.w};
+        {
           // the four records of a piece are independent: their loads are issued together, in two
           // stages -- the own row first (two thirds of the candidates already lose against a pad
           // neighbour there), then the rows above and below for those still in the race; the others
           // read word 0, a broadcast that costs no bank conflict
-          u32 pu[4], nu[4], pm[4], nm[4], pd[4], nd[4];
-          bool cand[4];
+          u32 pu[K], nu[K], pm[K], nm[K], pd[K], nd[K];
+          bool cand[K];
 #pragma unroll
-          for (int k = 0; k < 4; ++k) {
+          for (int k = 0; k < K; ++k) {
             const u32 q = (rr[k] >> 16) & 0x3FFu, tl = k6_row(rr[k], sl), pad = rr[k] & 0xFFu;
             cand[k] = q >= thr && tl - 1u < TPC_TT - 2u;   // (q = 0 for run padding)
             if (check && !cand[k] && rr[k] != 0u && tl < TPC_TT && s.tile[tl * pitch + pad + TPC_HALO] < q) viol = 1u;
@@ -1163,7 +1171,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
             pm[k] = __funnelshift_r(w[0], w[1], sh); nm[k] = (w[1] >> sh) & 0xFFFFu;
           }
 #pragma unroll
-          for (int k = 0; k < 4; ++k) {
+          for (int k = 0; k < K; ++k) {
             const u32 q = (rr[k] >> 16) & 0x3FFu, tl = k6_row(rr[k], sl), pad = rr[k] & 0xFFu;
             if (check && cand[k] && (pm[k] >> 16) < q) viol = 1u;   // the cell holds a smaller duplicate of this record (Q5)
             cand[k] = cand[k] && (pm[k] >> 16) == q && q > (pm[k] & 0xFFFFu) && q >= nm[k];   // (!= q: a smaller duplicate of this cell)
@@ -1174,7 +1182,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
             pd[k] = __funnelshift_r(w[0], w[1], sh); nd[k] = (w[1] >> sh) & 0xFFFFu;
           }
 #pragma unroll
-          for (int k = 0; k < 4; ++k) {
+          for (int k = 0; k < K; ++k) {
             const u32 q = (rr[k] >> 16) & 0x3FFu, tl = k6_row(rr[k], sl), pad = rr[k] & 0xFFu;
             const u32 e = max(max(pu[k] & 0xFFFFu, pu[k] >> 16), nu[k]);
             const u32 l = max(max(pd[k] & 0xFFFFu, pd[k] >> 16), nd[k]);
@@ -1188,6 +1196,19 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
             }
           }
         }
+        return viol;
+      };
+      auto peak_pass = [&](const bool check) -> u32 {
+        u32 viol = 0u;
+        if (nrec <= TPC_K6_CONSUMERS) {
+          const u32 r1[1] = {tid < nrec ? rec[tid] : 0u};
+          viol = peak_recs(TpcInt<1>(), r1, check);
+        } else
+          for (u32 u = tid; u < total; u += TPC_K6_CONSUMERS) {
+            const uint4 v = r4[u];
+            const u32 rr[4] = {v.x, v.y, v.z, v.w};
+            viol |= peak_recs(TpcInt<4>(), rr, check);
+          }
         return viol;
       };
       if (MODE == TPC_MODE_FAST) {
@@ -1352,16 +1373,22 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
         if (MODE == TPC_MODE_FAST) at = atomicAdd(a.n_clusters, (u64)fcount);
         if (MODE == TPC_MODE_DET_TEMP) at = atomicAdd(a.temp_cursor, (u64)fcount);
       }
+      __syncwarp();   // keeps the atomic ahead of the loads below (ptxas sinks it otherwise)
       u32 cnt[5], t = 0u;
+      {   // a lane counts 5 consecutive rows: ten 128-bit loads issued together, no branches
+        const uint4* rm = (const uint4*)s.rowmask;
+        uint4 v[10];
 #pragma unroll
-      for (int k = 0; k < 5; ++k) {
-        const u32 tl = lane * 5u + (u32)k;
-        u32 n = 0u;
-        if (tl < TPC_TT) {
-#pragma unroll
-          for (int w = 0; w < 8; ++w) n += __popc(s.rowmask[tl * 8u + w]);
+        for (int k = 0; k < 5; ++k) {
+          const u32 tl = lane * 5u + (u32)k, tc = tl < TPC_TT ? tl : TPC_TT - 1u;
+          v[2 * k] = rm[tc * 2u]; v[2 * k + 1] = rm[tc * 2u + 1u];
         }
-        cnt[k] = n; t += n;
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+          const uint4 x = v[2 * k], y = v[2 * k + 1];
+          const u32 n = (__popc(x.x) + __popc(x.y)) + (__popc(x.z) + __popc(x.w)) + ((__popc(y.x) + __popc(y.y)) + (__popc(y.z) + __popc(y.w)));
+          cnt[k] = lane * 5u + (u32)k < TPC_TT ? n : 0u; t += cnt[k];
+        }
       }
       u32 inc = t;
 #pragma unroll
