@@ -1065,6 +1065,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
     const int t_base = (int)s.misc[6] + (int)(mt * TPC_TS);   // time of tile row 0
     const u32 sl = s.misc[7] + mt;                            // slab of this tile inside its bin
     csync();   // A: the previous tile is done with the map, and the map is zero
+    u32 my_r = 0u;   // sparse tile: this thread's record, if it lies in the tile
     // ---- O0: scatter the tile's records ------------------------------------------------------
     for (u32 round = 0u;;) {
       u32 nu = total - round * TPC_K6_CAPU;
@@ -1075,7 +1076,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
         if (nu * 4u <= TPC_K6_CONSUMERS) {   // a sparse tile: one record per thread, spread over all warps
           const u32 r = tid < nu * 4u ? rec[tid] : 0u;
           const u32 tl = k6_row(r, sl);
-          if (r != 0u && tl < TPC_TT) s.tile[tl * pitch + (r & 0xFFu) + TPC_HALO] = (u16)((r >> 16) & 0x3FFu);
+          if (r != 0u && tl < TPC_TT) { s.tile[tl * pitch + (r & 0xFFu) + TPC_HALO] = (u16)((r >> 16) & 0x3FFu); my_r = r; }
         } else
         for (u32 u = tid; u < nu; u += TPC_K6_CONSUMERS) {
           const uint4 v = r4[u];
@@ -1501,7 +1502,19 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       }
       if (npk > TPC_K6_CONSUMERS) csync();   // block-uniform: the extra clusters still read the map
     }
-    zero_tile();   // for the next tile (barrier A orders it before the scatter)
+    // for the next tile (barrier A orders it before the scatter).  A sparse tile undoes its own
+    // writes instead of sweeping 50 KB: every cell, peak bit and survivor bit sits at a record,
+    // and the thread that owns the record clears the three words.
+    if (total * 4u <= TPC_K6_CONSUMERS) {   // block-uniform (the condition of the sparse scatter)
+      if (my_r != 0u) {
+        const u32 tl = k6_row(my_r, sl), pad = my_r & 0xFFu;
+        s.tile[tl * pitch + pad + TPC_HALO] = 0;
+        s.pmask[tl * TPC_K6_PMW + ((pad + 2u) >> 5)] = 0u;
+        s.rowmask[tl * 8u + (pad >> 5)] = 0u;
+      }
+      if (tid == 0) s.misc[0] = 0u;
+    } else
+      zero_tile();
    }
   }
 }
