@@ -563,3 +563,52 @@ def test_handle_reuse_sizes_and_geometries(tp, cuda_device):
         assert rb[0][:int(rb[1].item())].cpu().numpy().tobytes() == exp_b.tobytes()
         assert rs[0][:int(rs[1].item())].cpu().numpy().tobytes() == exp_s.tobytes()
     c.close(); c2.close()
+
+
+def test_sparse_dense_tile_alternation(tp, cuda_device):
+    """K6 takes a tile with <= 256 staged records through the one-record-per-thread path, which
+    undoes its own map writes instead of sweeping the map; larger tiles take the 16-byte-piece
+    path, tiles above the staging capacity several rounds.  One CTA handles consecutive slabs of
+    a bin, so every kind of tile here is followed by every other kind: record counts 0, 1 and
+    every value around the 256 boundary, a few thousand, and > 4096 (multi-round), with
+    duplicates on one cell (Q5), pads out of range (Q4) and records on the slab border rows that
+    two tiles share.  A cell left behind by an undo or a missed sweep shows up as a phantom
+    cluster or a wrong sum in the next tile."""
+    rng = np.random.default_rng(83)
+    P, n_slabs = 64, 330
+    T = 128 * n_slabs            # 42240 bins = 3 coarse time-chunks
+    counts = [0, 1, 2, 31, 32, 33, 64, 65, 128, 300, 1000, 3000, 4090, 4100, 5000] + list(range(236, 280))
+    rows = []
+    for r in (0, 1):
+        order = rng.permutation(n_slabs)
+        for i, sl in enumerate(order):
+            n = counts[(i + 7 * r) % len(counts)]
+            lo = 0 if i % 3 == 0 else 6          # every third slab also uses the border rows
+            hi = 128 if i % 3 == 0 else 122
+            cells = rng.choice((hi - lo) * P, size=n, replace=False)
+            t = sl * 128 + lo + cells // P
+            p = cells % P
+            q = rng.integers(1, 400, n)
+            rows += [(0, r, int(p[k]), int(t[k]), int(q[k])) for k in range(n)]
+            if n and i % 4 == 0:   # duplicates of one cell with other charges, an out-of-range pad
+                for k in range(min(n, 5)):
+                    rows.append((0, r, int(p[k]), int(t[k]), int(rng.integers(1, 1023))))
+                rows.append((0, r, P + 3, int(t[0]), 77))
+    d = t1.make_digits(rows)
+    exp, st_exp = _oracle(d, 1, 2, T, [P, P])
+    assert st_exp != 0                       # the out-of-range pads are flagged
+    # FAST promises the same set for duplicate-free input only (Q5): one digit per cell, the largest
+    ds = d[np.lexsort((-d["charge"].astype(np.int64), d["pad"], d["time"], d["row"]))]
+    first = np.ones(len(ds), dtype=bool)
+    first[1:] = (ds["pad"][1:] != ds["pad"][:-1]) | (ds["time"][1:] != ds["time"][:-1]) | (ds["row"][1:] != ds["row"][:-1])
+    du = ds[first]
+    exp_u, _ = _oracle(du, 1, 2, T, [P, P])
+    assert exp_u.tobytes() == exp.tobytes()
+    for _ in range(2):
+        dd = d[rng.permutation(len(d))]
+        det, _, st = _run_both(tp, _digits_tensor(dd, cuda_device), 1, 2, T, [P, P])
+        assert st == st_exp and det.tobytes() == exp.tobytes()
+        dd = du[rng.permutation(len(du))]
+        det, fast, st = _run_both(tp, _digits_tensor(dd, cuda_device), 1, 2, T, [P, P])
+        assert st == st_exp and det.tobytes() == exp.tobytes()
+        _check_fast(fast, exp)
