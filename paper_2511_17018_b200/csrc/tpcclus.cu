@@ -117,10 +117,10 @@ int make_geometry(const tpcclus_params* p, Geometry* g) {
   L.temp_cursor = take(8);
   L.det_flag = take(4);
   L.tile_state = take(8ull * g->n_tiles);   // DET chained scan: must start at 0 every run
+  L.bin_chunk_start = take(4ull * (nb + 1));   // K2 accumulates the per-bin chunk totals here, K3 scans them in place
   L.counters_bytes = o - L.counters;
-  L.slice_cnt = take(4ull * nb * g->g1);
+  L.slice_cnt = take(4ull * align_up(nb, 4) * g->g1);   // row pitch: a multiple of 4 entries
   L.used = take(4ull * g->g1);
-  L.bin_chunk_start = take(4ull * (nb + 1));
   L.batch_start = take(4ull * (nb + 1));
   L.batch_bin = take(4ull * g->n_batches_max);
   L.dir = take(4ull * g->n_chunks_max);
@@ -538,12 +538,12 @@ int enqueue_binning(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n
   int rc;
   { void* a[] = {&dig, &n64, &per_cta, &p.pool, &p.dir, &p.used, &slice_cap, &status};
     if ((rc = launch(h, K_PART_COARSE, dim3(g.g1), dim3(TPC_K1_THREADS), h->smem_k1, st, a))) return rc; }
-  u32 n_slices = g.g1, smem_nb = 4u * g.prm.n_bins;
-  { void* a[] = {&p.dir, &p.used, &slice_cap, &p.slice_cnt};
+  u32 smem_nb = 4u * g.prm.n_bins;
+  { void* a[] = {&p.dir, &p.used, &slice_cap, &p.slice_cnt, &p.bin_chunk_start};
     if ((rc = launch(h, K_DIR_COUNT, dim3(g.g1), dim3(TPC_SCAN_THREADS), smem_nb, st, a))) return rc; }
-  { void* a[] = {&p.slice_cnt, &n_slices, &p.bin_chunk_start, &p.batch_start, &p.batch_bin};
+  { void* a[] = {&p.bin_chunk_start, &p.batch_start, &p.batch_bin};
     if ((rc = launch(h, K_DIR_SCAN, dim3(1), dim3(TPC_SCAN_THREADS), smem_nb, st, a))) return rc; }
-  { void* a[] = {&p.dir, &p.used, &slice_cap, &p.slice_cnt, &p.chunk_list};
+  { void* a[] = {&p.dir, &p.used, &slice_cap, &p.slice_cnt, &p.bin_chunk_start, &p.chunk_list};
     if ((rc = launch(h, K_DIR_FILL, dim3(g.g1), dim3(TPC_SCAN_THREADS), smem_nb, st, a))) return rc; }
   { void* a[] = {&p.pool, &p.dir, &p.chunk_list, &p.bin_chunk_start, &p.batch_start, &p.batch_bin, &p.blob, &p.blob_cursor, &p.idx, &status};
     if ((rc = launch(h, K_PART_FINE, dim3(h->grid_k5), dim3(TPC_K5_THREADS), h->smem_k5, st, a))) return rc; }

@@ -369,13 +369,16 @@ k_partition_coarse(const uint2* __restrict__ digits, u64 n, u64 per_cta, uint4* 
 // ==========================================================================================
 // K2..K4  chunk directory -> per-bin chunk lists (bookkeeping of the scatter; ~2.6e7 chunks
 // at CFG[4], 4 bytes each).  One CTA per K1 slice with a shared-memory histogram, so there
-// are no global atomics: K2 counts chunks per (slice, bin), K3 turns the matrix into offsets
-// (slices of one bin follow each other), K4 places the chunk ids.  The order of chunks inside
+// are no global atomics on hot addresses: K2 counts chunks per (slice, bin) and adds its row
+// to the per-bin totals (one spread reduction per non-empty entry), K3 -- a single CTA -- scans
+// the NB totals into bin and batch offsets, K4 derives its slice's cursors from the count
+// matrix (slices of one bin follow each other) and places the chunk ids.  The order of chunks inside
 // a (slice, bin) group is whatever the shared atomics give: nothing downstream depends on
 // it (the map build is a max, O0/Q5).
 // ==========================================================================================
 extern "C" __global__ void __launch_bounds__(TPC_SCAN_THREADS)
-k_dir_count(const u32* __restrict__ dir, const u32* __restrict__ used, u32 slice_cap, u32* __restrict__ slice_cnt) {
+k_dir_count(const u32* __restrict__ dir, const u32* __restrict__ used, u32 slice_cap, u32* __restrict__ slice_cnt,
+            u32* __restrict__ bin_total) {   // bin_total = bin_chunk_start, zeroed at the head of the run
   extern __shared__ __align__(128) u32 smem_u32[];
   const u32 nb = PRM(n_bins);
   for (u32 i = threadIdx.x; i < nb; i += TPC_SCAN_THREADS) smem_u32[i] = 0u;
@@ -384,25 +387,24 @@ k_dir_count(const u32* __restrict__ dir, const u32* __restrict__ used, u32 slice
   const u32* d = dir + (u64)blockIdx.x * slice_cap;
   for (u32 c = threadIdx.x; c < n; c += TPC_SCAN_THREADS) atomicAdd(&smem_u32[d[c] >> 8], 1u);
   __syncthreads();
-  for (u32 i = threadIdx.x; i < nb; i += TPC_SCAN_THREADS) slice_cnt[(u64)blockIdx.x * nb + i] = smem_u32[i];
+  for (u32 i = threadIdx.x; i < nb; i += TPC_SCAN_THREADS) {
+    const u32 c = smem_u32[i];
+    slice_cnt[(u64)blockIdx.x * ((nb + 3u) & ~3u) + i] = c;   // row pitch: a multiple of 4 entries (K4 reads 16 bytes)
+    if (c != 0u) atomicAdd(&bin_total[i], c);   // integer sum: the order does not matter
+  }
 }
 
 // single CTA: exclusive scans over the bins.
 //   bin_chunk_start[b] = sum_{b'<b} nchunks[b']          (NB+1 entries)
 //   batch_start[b]     = sum_{b'<b} ceil(nchunks[b']/CPB) (NB+1 entries; [NB] = total batches)
 //   batch_bin[k]       = the bin batch k belongs to
-//   slice_cnt[s][b]   := bin_chunk_start[b] + sum_{s'<s} slice_cnt[s'][b]   (in place: K4's cursors)
+// On entry bin_chunk_start[b] holds nchunks[b] (summed over the slices by K2).
 extern "C" __global__ void __launch_bounds__(TPC_SCAN_THREADS)
-k_dir_scan(u32* __restrict__ slice_cnt, u32 n_slices, u32* __restrict__ bin_chunk_start, u32* __restrict__ batch_start,
-           u32* __restrict__ batch_bin) {
+k_dir_scan(u32* __restrict__ bin_chunk_start, u32* __restrict__ batch_start, u32* __restrict__ batch_bin) {
   extern __shared__ __align__(128) u32 smem_u32[];   // [nb] chunks per bin
   __shared__ u32 s_a[TPC_SCAN_THREADS], s_b[TPC_SCAN_THREADS];
   const u32 nb = PRM(n_bins);
-  for (u32 b = threadIdx.x; b < nb; b += TPC_SCAN_THREADS) {   // coalesced over bins
-    u32 t = 0u;
-    for (u32 sl = 0u; sl < n_slices; ++sl) t += slice_cnt[(u64)sl * nb + b];
-    smem_u32[b] = t;
-  }
+  for (u32 b = threadIdx.x; b < nb; b += TPC_SCAN_THREADS) smem_u32[b] = bin_chunk_start[b];
   __syncthreads();
   const u32 per = (nb + TPC_SCAN_THREADS - 1u) / TPC_SCAN_THREADS;
   const u32 lo = threadIdx.x * per;
@@ -428,19 +430,33 @@ k_dir_scan(u32* __restrict__ slice_cnt, u32 n_slices, u32* __restrict__ bin_chun
     ea += c; eb += nbt;
   }
   if (threadIdx.x == TPC_SCAN_THREADS - 1u) { bin_chunk_start[nb] = s_a[threadIdx.x]; batch_start[nb] = s_b[threadIdx.x]; }
-  __syncthreads();   // bin_chunk_start[] of this CTA's own writes is read below (same CTA: visible after the barrier)
-  for (u32 b = threadIdx.x; b < nb; b += TPC_SCAN_THREADS) {
-    u32 run = bin_chunk_start[b];
-    for (u32 sl = 0u; sl < n_slices; ++sl) { const u32 t = slice_cnt[(u64)sl * nb + b]; slice_cnt[(u64)sl * nb + b] = run; run += t; }
-  }
 }
 
 extern "C" __global__ void __launch_bounds__(TPC_SCAN_THREADS)
 k_dir_fill(const u32* __restrict__ dir, const u32* __restrict__ used, u32 slice_cap,
-           const u32* __restrict__ slice_cnt, u32* __restrict__ chunk_list) {
+           const u32* __restrict__ slice_cnt, const u32* __restrict__ bin_chunk_start, u32* __restrict__ chunk_list) {
   extern __shared__ __align__(128) u32 smem_u32[];   // [nb] cursors of this slice
   const u32 nb = PRM(n_bins);
-  for (u32 i = threadIdx.x; i < nb; i += TPC_SCAN_THREADS) smem_u32[i] = slice_cnt[(u64)blockIdx.x * nb + i];
+  // cursor of slice s in bin i = bin start + the counts of the slices before it = bin end - the
+  // counts of the slices from s on: whichever is the shorter column walk (the matrix sits in L2)
+  const u32 s = blockIdx.x, ns = gridDim.x, nq = (nb + 3u) >> 2;   // 16-byte words per matrix row
+  const bool fwd = 2u * s <= ns;
+  const u32 k0 = fwd ? 0u : s, k1 = fwd ? s : ns;
+  const uint4* m4 = (const uint4*)slice_cnt;
+  for (u32 j = threadIdx.x; j < nq; j += TPC_SCAN_THREADS) {   // four bins per thread and load
+    uint4 acc = make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll 8
+    for (u32 k = k0; k < k1; ++k) {
+      const uint4 v = m4[(u64)k * nq + j];
+      acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
+    }
+    const u32 a[4] = {acc.x, acc.y, acc.z, acc.w};
+#pragma unroll
+    for (u32 e = 0u; e < 4u; ++e) {
+      const u32 i = 4u * j + e;   // entries past nb are row padding
+      if (i < nb) smem_u32[i] = fwd ? bin_chunk_start[i] + a[e] : bin_chunk_start[i + 1u] - a[e];
+    }
+  }
   __syncthreads();
   const u32 n = used[blockIdx.x];
   const u32 id0 = blockIdx.x * slice_cap;
