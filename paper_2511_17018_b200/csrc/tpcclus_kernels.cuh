@@ -666,12 +666,16 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
   ids(cur_b, cidn);
   pieces(cidn, vn, nrecn);
   look(blockIdx.x + gridDim.x, nxt_b);
+  if (threadIdx.x < TPC_NKEY) s_cnt[threadIdx.x] = 0u;
+  __syncthreads();
 
+  // Three block barriers per batch: count | scan | place | dump.  The counters are cleared in the
+  // place phase (the scan was their last reader) and the dump of a batch needs no barrier after
+  // it: the next writers of buf / s_off / s_gbase (the scan warp) sit behind the barrier that
+  // follows the next count, which every thread reaches only after its dump.
   for (u32 batch = blockIdx.x; batch < n_batches; batch += gridDim.x) {
     const u32 b = cur_b.b, kb = cur_b.kb, nbatch_b = cur_b.nbatch_b;
     const u32 npads = PRM_NPADS((b / PRM(n_tc)) % PRM(n_rows));   // one bin = one pad row
-    if (threadIdx.x < TPC_NKEY) s_cnt[threadIdx.x] = 0u;
-    __syncthreads();
 
     // ---- <= 16 records per thread: count per key, remember the rank -------------------------
     u32 rec[16];
@@ -717,6 +721,8 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
     __syncthreads();
     // ---- exclusive scan of the run lengths (one warp, NKEY/32 keys = NKEY/64 slabs per lane);
     //      every slab's A run starts on a multiple of 4 records ----------------------------------
+    u64 gb = 0ull;   // lane 31: the batch's place in the blob; stored after the place phase, so that
+                     // the round trip of the atomic hides behind it instead of holding up the barrier
     if (threadIdx.x < 32) {
       u32 la[TPC_NKEY / 64u], lb[TPC_NKEY / 64u], t = 0u;
 #pragma unroll
@@ -739,7 +745,7 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
       }
       if (threadIdx.x == 31) {
         s_off[TPC_NKEY] = inc;
-        s_gbase = atomicAdd(blob_cursor, (u64)((inc + 7u) & ~7u));   // batches start 32-byte aligned
+        gb = atomicAdd(blob_cursor, (u64)((inc + 7u) & ~7u));   // batches start 32-byte aligned
       }
     }
     __syncthreads();
@@ -755,11 +761,13 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
         buf[s_off[key] + rk] = (r & 0xFFu) | ((m | ((sl1 & 1u) << 7)) << 8) | ((r >> 22) << 16);
       }
     }
+    if (threadIdx.x >= TPC_K5_THREADS - TPC_NKEY) s_cnt[threadIdx.x - (TPC_K5_THREADS - TPC_NKEY)] = 0u;   // for the next batch
     pieces(cidn, vn, nrecn);   // records of the next batch: in flight during the dump
     cur_b = nxt_b;
     look(batch + 2u * gridDim.x, nxt_b);
     const u32 total = s_off[TPC_NKEY];
     if (threadIdx.x < 8u && total + threadIdx.x < ((total + 7u) & ~7u)) buf[total + threadIdx.x] = 0u;   // end padding
+    if (threadIdx.x == 31u) s_gbase = gb;
     __syncthreads();
     // ---- dump the sorted batch + its index entries -----------------------------------------
     const u64 gbase = s_gbase;
@@ -771,7 +779,6 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
       const u32 beg = s_off[2u * sl], end = s_off[2u * sl + 3u];   // beg is a multiple of 4
       idx[(u64)nsl * batch_start[b] + (u64)sl * nbatch_b + kb] = (gbase + beg) | ((u64)(end - beg) << 40);
     }
-    __syncthreads();
   }
   if (bad) atomicOr(status, TPC_STATUS_BAD_DIGITS);
 }
