@@ -174,11 +174,15 @@ __device__ __forceinline__ void k1_flush_single(const K1Smem& s, u32 bin, u32 sl
 // set are still to be placed; FIRST = they have no reserved slot yet.  The flush queue and
 // the spill list are private to the warp and filled with ballots, so the only shared-memory
 // atomics are the slot reservations.  `nsp` = entries this warp parked in the previous pass.
-// Returns (block-uniform) whether any thread still has a pending entry.
-template <int K, bool FIRST>
+// Returns (block-uniform) whether any thread still has a pending entry.  `between` runs after
+// this warp's share of the flush and before the closing barrier: register-only work of the
+// next round (its decode) goes there, where it fills the issue slots the flush -- a few warps
+// on dependent shared-memory chains -- leaves idle.
+struct K1Nothing { __device__ __forceinline__ void operator()() const {} };
+template <int K, bool FIRST, class F = K1Nothing>
 __device__ __forceinline__ bool k1_pass(const K1Smem& s, u32& cur, u32& nsp, const u32 (&bin)[K], const u32 (&rec)[K],
                                         u32 (&slot)[K], u32& pend, u32 slice_base, u32 slice_cap,
-                                        uint4* pool, u32* dir) {
+                                        uint4* pool, u32* dir, F between = F()) {
   const u32 lane = lane_id(), warp = threadIdx.x >> 5, lt = (1u << lane) - 1u;
   u16* fq = s.fq + warp * TPC_K1_WFQ;
   u32* sp_in = s.spill + ((cur * (TPC_K1_THREADS / 32) + warp) * TPC_K1_WSP) * 2u;
@@ -239,6 +243,7 @@ __device__ __forceinline__ bool k1_pass(const K1Smem& s, u32& cur, u32& nsp, con
     if (lf & (1u << K)) k1_flush_single(s, drain_bin, slice_base, slice_cap, pool, dir);
   }
   cur ^= 1u;
+  between();
   return __syncthreads_or((int)pend) != 0;
 }
 
@@ -272,15 +277,10 @@ __device__ __forceinline__ void k1_rounds(const K1Smem& s, const uint2* __restri
       else d[h] = make_uint4(0u, 0u, 0u, 0u);
     }
   };
-  uint4 nxt[TPC_K1_DPT / 2];
-  fetch(0u, nxt);
-  for (u32 j = 0u; j < n_rounds; ++j) {
-    uint4 curd[TPC_K1_DPT / 2];
-#pragma unroll
-    for (int h = 0; h < TPC_K1_DPT / 2; ++h) curd[h] = nxt[h];
-    fetch(j + 1u, nxt);   // prefetch the next round while this one is binned
-    u32 bin[TPC_K1_DPT], rec[TPC_K1_DPT], slot[TPC_K1_DPT], dbin[TPC_K1_DPT], drec[TPC_K1_DPT];
-    u32 pend = 0u, dpend = 0u;
+  // O0's validity / clamp / zero rules and the routing of one round's digits
+  auto decode = [&](const uint4 (&curd)[TPC_K1_DPT / 2], u32 (&bin)[TPC_K1_DPT], u32 (&rec)[TPC_K1_DPT], u32& pend,
+                    u32 (&dbin)[TPC_K1_DPT], u32 (&drec)[TPC_K1_DPT], u32& dpend) {
+    pend = 0u; dpend = 0u;
 #pragma unroll
     for (int k = 0; k < TPC_K1_DPT; ++k) {
       const u32 w0 = (k & 1) ? curd[k >> 1].z : curd[k >> 1].x, w1 = (k & 1) ? curd[k >> 1].w : curd[k >> 1].y;
@@ -306,13 +306,42 @@ __device__ __forceinline__ void k1_rounds(const K1Smem& s, const uint2* __restri
         }
       }
     }
+  };
+  uint4 nxt[TPC_K1_DPT / 2];
+  fetch(0u, nxt);
+  if (!MULTI_TC) {
+    // Software pipeline: the digits of round j+1 are decoded inside round j's flush phase and the
+    // loads of round j+2 issued behind them, so a round is insert | barrier | flush + decode | barrier.
+    u32 bin[TPC_K1_DPT], rec[TPC_K1_DPT], slot[TPC_K1_DPT], nbin[TPC_K1_DPT], nrec[TPC_K1_DPT], unused[TPC_K1_DPT];
+    u32 pend, npend = 0u, dp;
+    decode(nxt, bin, rec, pend, unused, unused, dp);
+    fetch(1u, nxt);
+    for (u32 j = 0u; j < n_rounds; ++j) {
+      auto next_round = [&]() {
+        decode(nxt, nbin, nrec, npend, unused, unused, dp);   // past the end: all zero, nothing pending
+        fetch(j + 2u, nxt);
+      };
+      if (k1_pass<TPC_K1_DPT, true>(s, cur, nsp, bin, rec, slot, pend, slice_base, slice_cap, pool, dir, next_round))
+        while (k1_pass<TPC_K1_DPT, false>(s, cur, nsp, bin, rec, slot, pend, slice_base, slice_cap, pool, dir)) {}
+#pragma unroll
+      for (int k = 0; k < TPC_K1_DPT; ++k) { bin[k] = nbin[k]; rec[k] = nrec[k]; }
+      pend = npend;
+    }
+    return;
+  }
+  for (u32 j = 0u; j < n_rounds; ++j) {
+    uint4 curd[TPC_K1_DPT / 2];
+#pragma unroll
+    for (int h = 0; h < TPC_K1_DPT / 2; ++h) curd[h] = nxt[h];
+    fetch(j + 1u, nxt);   // prefetch the next round while this one is binned
+    u32 bin[TPC_K1_DPT], rec[TPC_K1_DPT], slot[TPC_K1_DPT], dbin[TPC_K1_DPT], drec[TPC_K1_DPT];
+    u32 pend = 0u, dpend = 0u;
+    decode(curd, bin, rec, pend, dbin, drec, dpend);
     if (k1_pass<TPC_K1_DPT, true>(s, cur, nsp, bin, rec, slot, pend, slice_base, slice_cap, pool, dir))
       while (k1_pass<TPC_K1_DPT, false>(s, cur, nsp, bin, rec, slot, pend, slice_base, slice_cap, pool, dir)) {}
-    if (MULTI_TC) {
-      if (__syncthreads_or((int)dpend)) {
-        if (k1_pass<TPC_K1_DPT, true>(s, cur, nsp, dbin, drec, slot, dpend, slice_base, slice_cap, pool, dir))
-          while (k1_pass<TPC_K1_DPT, false>(s, cur, nsp, dbin, drec, slot, dpend, slice_base, slice_cap, pool, dir)) {}
-      }
+    if (__syncthreads_or((int)dpend)) {
+      if (k1_pass<TPC_K1_DPT, true>(s, cur, nsp, dbin, drec, slot, dpend, slice_base, slice_cap, pool, dir))
+        while (k1_pass<TPC_K1_DPT, false>(s, cur, nsp, dbin, drec, slot, dpend, slice_base, slice_cap, pool, dir)) {}
     }
   }
 }
