@@ -39,9 +39,9 @@ def _log(msg):
 
 
 METRIC = "TPC clusterizer digits/s on Pb-Pb-like time frame"
-# ncu --set full, CFG[4] shuffled FAST generic, one launch each (profiles/r01e_ncu_full_summary.txt)
-NCU_TRAFFIC_BYTES = {"k_partition_coarse": 12765752000 + 6478698000, "k_partition_fine": 9077308000 + 6497106000,
-                     "k_cluster_tiles_fast": 6546597000 + 1900535000}
+# ncu --set full, CFG[4] shuffled FAST generic, one launch each (profiles/r01f_ncu_full_summary.txt)
+NCU_TRAFFIC_BYTES = {"k_partition_coarse": 12764491000 + 6479841000, "k_partition_fine": 9064465000 + 6487736000,
+                     "k_cluster_tiles_fast": 6542284000 + 1900004000}
 UNIT = "digits/s"
 
 

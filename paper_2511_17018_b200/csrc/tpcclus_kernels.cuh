@@ -327,8 +327,7 @@ __device__ __forceinline__ void k1_rounds(const K1Smem& s, const uint2* __restri
       for (int k = 0; k < TPC_K1_DPT; ++k) { bin[k] = nbin[k]; rec[k] = nrec[k]; }
       pend = npend;
     }
-    return;
-  }
+  } else
   for (u32 j = 0u; j < n_rounds; ++j) {
     uint4 curd[TPC_K1_DPT / 2];
 #pragma unroll
@@ -489,6 +488,7 @@ k_dir_fill(const u32* __restrict__ dir, const u32* __restrict__ used, u32 slice_
   __syncthreads();
   const u32 n = used[blockIdx.x];
   const u32 id0 = blockIdx.x * slice_cap;
+  // (bound by the scattered 4-byte stores: eight directory loads in flight per thread changed nothing)
   for (u32 c = threadIdx.x; c < n; c += TPC_SCAN_THREADS)
     chunk_list[atomicAdd(&smem_u32[dir[id0 + c] >> 8], 1u)] = id0 + c;
 }
