@@ -747,6 +747,8 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
       }
     }
     ids(nxt_b, cidn);   // chunk ids of the next batch: in flight during the scan and the placing
+    // the bulk stores of the batch before must have read buf before the scan warp writes it again
+    if (threadIdx.x >= TPC_K5_THREADS - 32u) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
     __syncthreads();
     // ---- exclusive scan of the run lengths (one warp, NKEY/32 keys = NKEY/64 slabs per lane);
     //      every slab's A run starts on a multiple of 4 records ----------------------------------
@@ -797,18 +799,29 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
     const u32 total = s_off[TPC_NKEY];
     if (threadIdx.x < 8u && total + threadIdx.x < ((total + 7u) & ~7u)) buf[total + threadIdx.x] = 0u;   // end padding
     if (threadIdx.x == 31u) s_gbase = gb;
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // this thread's writes to buf -> visible to the bulk copy
     __syncthreads();
     // ---- dump the sorted batch + its index entries -----------------------------------------
-    const u64 gbase = s_gbase;
-    uint4* dst = (uint4*)(blob + gbase);       // gbase is a multiple of 8 records (32 B)
-    const uint4* src = (const uint4*)buf;
-    for (u32 i = threadIdx.x; i < ((total + 7u) >> 3) * 2u; i += TPC_K5_THREADS) dst[i] = src[i];
+    // The copy shared -> global is handed to the bulk-copy engine (the last warp issues it, 4 KB per
+    // lane): it costs no LSU wavefronts -- the resource the count and place phases are bound by --
+    // and runs while the CTA already counts the next batch.
+    const u64 gbase = s_gbase;                 // a multiple of 8 records (32 B)
+    if (threadIdx.x >= TPC_K5_THREADS - 32u) {
+      const u32 bytes = ((total + 7u) >> 3) * 32u, off = (threadIdx.x & 31u) * 4096u;
+      if (off < bytes) {
+        const u32 nby = bytes - off < 4096u ? bytes - off : 4096u;
+        asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"((const char*)(blob + gbase) + off),
+                     "r"((u32)__cvta_generic_to_shared(buf) + off), "r"(nby) : "memory");
+      }
+      asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    }
     if (threadIdx.x < nsl) {   // tile sl reads A_sl B_sl A_sl+1
       const u32 sl = threadIdx.x;
       const u32 beg = s_off[2u * sl], end = s_off[2u * sl + 3u];   // beg is a multiple of 4
       idx[(u64)nsl * batch_start[b] + (u64)sl * nbatch_b + kb] = (gbase + beg) | ((u64)(end - beg) << 40);
     }
   }
+  if (threadIdx.x >= TPC_K5_THREADS - 32u) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
   if (bad) atomicOr(status, TPC_STATUS_BAD_DIGITS);
 }
 
