@@ -39,9 +39,9 @@ def _log(msg):
 
 
 METRIC = "TPC clusterizer digits/s on Pb-Pb-like time frame"
-# ncu --set full, CFG[4] shuffled FAST generic, one launch each (profiles/r01f_ncu_full_summary.txt)
-NCU_TRAFFIC_BYTES = {"k_partition_coarse": 12764491000 + 6479841000, "k_partition_fine": 9064465000 + 6487736000,
-                     "k_cluster_tiles_fast": 6542284000 + 1900004000}
+# ncu --set full, CFG[4] shuffled FAST generic, one launch each (profiles/r01g_ncu_full_summary.txt)
+NCU_TRAFFIC_BYTES = {"k_partition_coarse": 12766072000 + 6480317000, "k_partition_fine": 9069988000 + 6489780000,
+                     "k_cluster_tiles_fast": 6544338000 + 1902176000}
 UNIT = "digits/s"
 
 
