@@ -39,12 +39,11 @@ def test_t1_matches_appendix_a(case):
 
 @pytest.mark.parametrize("case", G["cases"], ids=[c["name"] for c in G["cases"]])
 def test_t0_matches_appendix_a(case):
-    # T0 on a small window around the digits (same relative geometry is not needed: the
-    # vectors sit away from edges except the corner case, which is at the origin).
-    small = all(t < 64 and p < 32 for p, t, _ in case["digits"])
-    if not small:
-        pytest.skip("T0 ranks every cell; only the small-coordinate vectors are run through it")
-    cl, bad = t0.clusterize([(0, 0, p, t, q) for p, t, q in case["digits"]], 1, 1, 64, [32],
+    # T0 ranks every cell of the map, so it gets a map just large enough for the vector: the full pad
+    # width and the time range up to the last digit + 8 (no cluster of these vectors sits on the far
+    # time edge, so the EDGE_TIME flag and the clipped windows are those of the full 14256-bin map).
+    T0 = min(T, max(64, max(t for _, t, _ in case["digits"]) + 8))
+    cl, bad = t0.clusterize([(0, 0, p, t, q) for p, t, q in case["digits"]], 1, 1, T0, [P],
                             G["thr_peak"], G["noise_eps"])
     assert not bad and len(cl) == len(case["clusters"])
     for got, exp in zip(cl, case["clusters"]):
