@@ -137,3 +137,51 @@ def make_digits(rows):
     for i, (s, r, p, t, q) in enumerate(rows):
         d[i] = (q, t, p, r, s, 0)
     return d
+
+
+def clusterize_by_sector(digits_of, sectors, n_rows, n_time, n_pads, thr_peak=6, noise_eps=4, threads=None,
+                         timing=None, cog_gated=False):
+    """T1 run sector-parallel ("the same T1 code run sector-parallel ... on all host
+    cores"): sectors never interact (O0, invariant I8 -- pinned in tests/test_oracle_multisector.py),
+    so each sector is clusterized alone by the unchanged single-threaded C routine as a 1-sector
+    geometry and gets its sector number put back.  ctypes releases the GIL, so plain threads do.
+
+    ``digits_of(s)`` returns the DIGIT (or uint64) array of sector ``s`` (any order; the sector
+    field is overwritten on a copy).  Returns ``{s: clusters}``; ``timing`` receives ``seconds``
+    (wall time of the clusterize calls only), ``cores`` (threads used) and ``digits``."""
+    import os
+    from concurrent.futures import ThreadPoolExecutor
+
+    sectors = list(sectors)
+    if threads is None:
+        threads = len(os.sched_getaffinity(0))
+    threads = max(1, min(int(threads), len(sectors)))
+    lib()   # build / load once, outside the threads
+    inputs = {}
+    for s in sectors:
+        d = np.array(digits_of(s), copy=True)
+        if d.dtype != DIGIT:
+            d = d.view(np.uint8).reshape(-1).view(DIGIT)
+        d["sector"] = 0
+        inputs[s] = d
+
+    def one(s):
+        d = inputs[s]
+        cl, st, cnt = clusterize(d, 1, n_rows, n_time, n_pads, thr_peak, noise_eps,
+                                 capacity=max(len(d) // 4, 1024), cog_gated=cog_gated)
+        if cnt != len(cl) or st != 0:
+            raise RuntimeError("oracle: sector %d: status %d, %d clusters for capacity %d" % (s, st, cnt, len(cl)))
+        cl["sector"] = s
+        return s, cl
+
+    t0 = time.perf_counter()
+    if threads == 1:
+        res = dict(one(s) for s in sectors)
+    else:
+        with ThreadPoolExecutor(max_workers=threads) as ex:
+            res = dict(ex.map(one, sectors))
+    if timing is not None:
+        timing["seconds"] = time.perf_counter() - t0
+        timing["cores"] = threads
+        timing["digits"] = int(sum(len(d) for d in inputs.values()))
+    return res

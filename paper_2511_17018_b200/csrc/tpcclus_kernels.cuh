@@ -16,6 +16,25 @@
 //                        ordered emission (O5)
 #pragma once
 
+// ---- compilation units (PAPER.md 64, section 3: "one source file per kernel", compiled straight to a
+// GPU binary and loaded with cuModuleLoad).  TPC_UNITS is a bit mask of the kernel families this
+// translation unit emits; the build compiles the text once per unit (csrc/tpcclus_unit.cu), every
+// unit gets the register allocation that suits it and its own copy of the constant block, which
+// the host's registry finds and fills (PAPER.md 81-85).  0 = declarations only (the host side).
+#define TPC_U_PART_COARSE 0x001u   // k_partition_coarse
+#define TPC_U_DIR 0x002u           // k_dir_count, k_dir_scan, k_dir_fill
+#define TPC_U_PART_FINE 0x004u     // k_partition_fine
+#define TPC_U_TILES_FAST 0x008u    // k_cluster_tiles_fast
+#define TPC_U_TILES_DET 0x010u     // k_cluster_tiles_det_temp, k_cluster_tiles_det
+#define TPC_U_ORDER 0x020u         // k_scan_local, k_scan_sums, k_emit_ordered, k_emit_packed
+#define TPC_U_TILES_DUMP 0x040u    // k_cluster_tiles_dump_map (debug hook of step a1)
+#define TPC_U_TILES_FAST_G 0x080u  // reading Q10' variants
+#define TPC_U_TILES_DET_G 0x100u
+#ifndef TPC_UNITS
+#define TPC_UNITS 0xFFFFFFFFu
+#endif
+#define TPC_U_ANY_TILES (TPC_U_TILES_FAST | TPC_U_TILES_DET | TPC_U_TILES_DUMP | TPC_U_TILES_FAST_G | TPC_U_TILES_DET_G)
+
 typedef unsigned int u32;
 typedef unsigned long long u64;
 typedef unsigned short u16;
@@ -51,14 +70,59 @@ struct TpcParams {
   u16 n_pads[256];
 };
 
+// ---- declarations the host side shares (sizes of the dynamic shared memory, kernel arguments) ----
+#define TPC_STATUS_NO_PACKED 4u
+#define TPC_K1_FQ 2048u      // flush-queue entries (u16 bin ids)
+#define TPC_K1_SPILL 512u    // spill entries per buffer (2 x u32)
+__host__ __device__ inline u32 tpc_k1_smem_bytes(u32 nb) {
+  return (nb * (TPC_STAGE + 2u) + 4u * TPC_K1_SPILL + 8u) * 4u + TPC_K1_FQ * 2u;
+}
+#define TPC_NSLMAX 128u   // >= slabs per bin: TPC_TC / TPC_TS = 127
+#define TPC_NKEY (2u * TPC_NSLMAX + 32u)   // sort keys: 2 per slab + A of the slab after the last; multiple of 32
+#define TPC_K5_BUF (TPC_CPB * TPC_CHUNK + 4u * TPC_NSLMAX + 8u)   // u32 words: the records of a batch + alignment gaps + end padding
+__host__ __device__ inline u32 tpc_k5_smem_bytes() { return (TPC_K5_BUF + 2u * TPC_NKEY + 8u) * 4u; }
+#define TPC_MODE_FAST 0
+#define TPC_MODE_DET 1        // chained scan inside K6 (fallback: any number of clusters)
+#define TPC_MODE_DET_TEMP 2   // runs into the temporary buffer, K7-K9 order them (the usual path)
+#define TPC_MODE_DUMP_MAP 3
+#define TPC_K6_CONSUMERS 256u                   // threads that compute
+#define TPC_K6_THREADS (TPC_K6_CONSUMERS + 32u)  // + the producer warp
+#define TPC_K6_CAP 4096u                         // records staged per round (16 KB)
+#define TPC_K6_CAPU (TPC_K6_CAP / 4u)            // ... in 16-byte units
+#ifndef TPC_K6_CTAS
+#define TPC_K6_CTAS 3                            // resident CTAs per SM (shared memory and registers)
+#endif
+
+struct K6Args {
+  const u32* blob; const u64* idx; const u32* batch_start;
+  uint4* out; u64 capacity; u64* n_clusters; u32* status;
+  u32* ticket;        // next tile to hand out (zeroed per run)
+  u64* tile_state;    // DET: chained scan of the tile counts, [n_tiles], zeroed per run
+  uint4* temp; u64 temp_cap; u64* temp_cursor;   // DET_TEMP: run buffer (the dead K1 pool), in clusters
+  u64* tile_base; u32* tile_cnt; u32* det_flag;  // DET_TEMP: per-tile (place, count); flag = buffer too small
+  u16* dmap; const u64* row_off;   // DUMP_MAP only: row_off[r] = cells of rows < r in one sector; [n_rows] = per sector
+};
+
+#define TPC_K6_GROUP 4u   // tiles (consecutive slabs of one bin) a ticket covers
+#define TPC_K6_PMW 9u
+__host__ __device__ inline u32 tpc_k6_smem_bytes(u32 pitch, u32 max_peaks) {
+  return (TPC_K6_CAP + TPC_TT * pitch / 2u + 4u + 2u + TPC_TT * (8u + TPC_K6_PMW) + TPC_TT + 2u + 16u + (max_peaks + 1u) / 2u) * 4u + 128u;
+}
+
 #ifdef TPC_RTC
 #define PRM(x) (TPC_##x)
 #define PRM_NPADS(r) (TPC_NPADS_TABLE[r])   // emitted by the host in front of this text
 #else
-__constant__ TpcParams c_prm;
+#if TPC_UNITS != 0u
+// One constant block per compilation unit (a non-RDC unit cannot see another unit's symbol:
+// PAPER.md 81).  extern "C": the host's registry looks the symbol up by this name in every module
+// it loads and keeps all copies up to date (PAPER.md 83-85).
+extern "C" { __constant__ TpcParams c_prm; }
+#endif
 #define PRM(x) (c_prm.x)
 #define PRM_NPADS(r) (c_prm.n_pads[r])
 #endif
+#if TPC_UNITS != 0u   // ---- device code ------------------------------------------------------------
 
 // ---- shared-memory sizes (bytes); the host launches with exactly these --------------------
 
@@ -104,8 +168,6 @@ __device__ __forceinline__ u32 lane_id() { return threadIdx.x & 31u; }
 //
 // record (4 B):  pad[0:8) | u[8:22) | q[22:32)   with u = time - tc*TPC_TC + 3  (14 bit)
 // ==========================================================================================
-#define TPC_K1_FQ 2048u      // flush-queue entries (u16 bin ids)
-#define TPC_K1_SPILL 512u    // spill entries per buffer (2 x u32)
 
 struct K1Smem {   // layout computed identically on the host (tpc_k1_smem_bytes)
   u32* stage;     // [NB][8]
@@ -115,9 +177,6 @@ struct K1Smem {   // layout computed identically on the host (tpc_k1_smem_bytes)
   u32* misc;      // [0] next chunk
   u16* fq;        // [warps][TPC_K1_WFQ]
 };
-__host__ __device__ inline u32 tpc_k1_smem_bytes(u32 nb) {
-  return (nb * (TPC_STAGE + 2u) + 4u * TPC_K1_SPILL + 8u) * 4u + TPC_K1_FQ * 2u;
-}
 __device__ __forceinline__ K1Smem k1_smem(u32* base, u32 nb) {   // fixed-size arrays first: constant offsets
   K1Smem s;
   s.misc = base;
@@ -345,6 +404,7 @@ __device__ __forceinline__ void k1_rounds(const K1Smem& s, const uint2* __restri
   }
 }
 
+#if TPC_UNITS & TPC_U_PART_COARSE
 extern "C" __global__ void __launch_bounds__(TPC_K1_THREADS, 1)
 k_partition_coarse(const uint2* __restrict__ digits, u64 n, u64 per_cta, uint4* __restrict__ pool,
                    u32* __restrict__ dir, u32* __restrict__ used, u32 slice_cap, u32* __restrict__ status) {
@@ -393,6 +453,7 @@ k_partition_coarse(const uint2* __restrict__ digits, u64 n, u64 per_cta, uint4* 
     used[blockIdx.x] = u;
   }
 }
+#endif
 
 // ==========================================================================================
 // K2..K4  chunk directory -> per-bin chunk lists (bookkeeping of the scatter; ~2.6e7 chunks
@@ -404,6 +465,7 @@ k_partition_coarse(const uint2* __restrict__ digits, u64 n, u64 per_cta, uint4* 
 // a (slice, bin) group is whatever the shared atomics give: nothing downstream depends on
 // it (the map build is a max, O0/Q5).
 // ==========================================================================================
+#if TPC_UNITS & TPC_U_DIR
 extern "C" __global__ void __launch_bounds__(TPC_SCAN_THREADS)
 k_dir_count(const u32* __restrict__ dir, const u32* __restrict__ used, u32 slice_cap, u32* __restrict__ slice_cnt,
             u32* __restrict__ bin_total) {   // bin_total = bin_chunk_start, zeroed at the head of the run
@@ -421,12 +483,14 @@ k_dir_count(const u32* __restrict__ dir, const u32* __restrict__ used, u32 slice
     if (c != 0u) atomicAdd(&bin_total[i], c);   // integer sum: the order does not matter
   }
 }
+#endif
 
 // single CTA: exclusive scans over the bins.
 //   bin_chunk_start[b] = sum_{b'<b} nchunks[b']          (NB+1 entries)
 //   batch_start[b]     = sum_{b'<b} ceil(nchunks[b']/CPB) (NB+1 entries; [NB] = total batches)
 //   batch_bin[k]       = the bin batch k belongs to
 // On entry bin_chunk_start[b] holds nchunks[b] (summed over the slices by K2).
+#if TPC_UNITS & TPC_U_DIR
 extern "C" __global__ void __launch_bounds__(TPC_SCAN_THREADS)
 k_dir_scan(u32* __restrict__ bin_chunk_start, u32* __restrict__ batch_start, u32* __restrict__ batch_bin) {
   extern __shared__ __align__(128) u32 smem_u32[];   // [nb] chunks per bin
@@ -459,7 +523,9 @@ k_dir_scan(u32* __restrict__ bin_chunk_start, u32* __restrict__ batch_start, u32
   }
   if (threadIdx.x == TPC_SCAN_THREADS - 1u) { bin_chunk_start[nb] = s_a[threadIdx.x]; batch_start[nb] = s_b[threadIdx.x]; }
 }
+#endif
 
+#if TPC_UNITS & TPC_U_DIR
 extern "C" __global__ void __launch_bounds__(TPC_SCAN_THREADS)
 k_dir_fill(const u32* __restrict__ dir, const u32* __restrict__ used, u32 slice_cap,
            const u32* __restrict__ slice_cnt, const u32* __restrict__ bin_chunk_start, u32* __restrict__ chunk_list) {
@@ -492,6 +558,7 @@ k_dir_fill(const u32* __restrict__ dir, const u32* __restrict__ used, u32 slice_
   for (u32 c = threadIdx.x; c < n; c += TPC_SCAN_THREADS)
     chunk_list[atomicAdd(&smem_u32[dir[id0 + c] >> 8], 1u)] = id0 + c;
 }
+#endif
 
 // ==========================================================================================
 // K7/K8/K9  deterministic mode, ordered output (O5 / PAPER.md 47-50: an ordered scan and an
@@ -500,6 +567,7 @@ k_dir_fill(const u32* __restrict__ dir, const u32* __restrict__ used, u32 slice_
 // a temporary buffer and records (place, count) per tile; K7/K8 scan the counts; K9 copies the
 // runs to their final places in tile order.
 // ==========================================================================================
+#if TPC_UNITS & TPC_U_ORDER
 extern "C" __global__ void __launch_bounds__(TPC_SCAN_THREADS)
 k_scan_local(const u32* __restrict__ in, u32* __restrict__ out_local, u32* __restrict__ block_sum, u32 n) {
   __shared__ u32 s[TPC_SCAN_THREADS];
@@ -520,8 +588,10 @@ k_scan_local(const u32* __restrict__ in, u32* __restrict__ out_local, u32* __res
   for (int k = 0; k < 4; ++k) { if (base + k < n) out_local[base + k] = e; e += v[k]; }
   if (threadIdx.x == TPC_SCAN_THREADS - 1u) block_sum[blockIdx.x] = s[threadIdx.x];
 }
+#endif
 
 // single CTA: block_prefix[i] = sum_{j<i} block_sum[j] (64 bit); *total = grand total.
+#if TPC_UNITS & TPC_U_ORDER
 extern "C" __global__ void __launch_bounds__(TPC_SCAN_THREADS)
 k_scan_sums(const u32* __restrict__ block_sum, u64* __restrict__ block_prefix, u32 nblocks, u64* __restrict__ total) {
   __shared__ u64 s[TPC_SCAN_THREADS];
@@ -546,10 +616,12 @@ k_scan_sums(const u32* __restrict__ block_sum, u64* __restrict__ block_prefix, u
   }
   if (threadIdx.x == 0) *total = carry;
 }
+#endif
 
 
 // K9: one warp per tile, 16 bytes per lane.  Skipped as a whole (flag set) when the temporary
 // buffer was too small: the chained-scan variant of K6 then redoes the frame (k6_chain).
+#if TPC_UNITS & TPC_U_ORDER
 extern "C" __global__ void __launch_bounds__(256)
 k_emit_ordered(const uint4* __restrict__ temp, const u64* __restrict__ tile_base, const u32* __restrict__ tile_cnt,
                const u32* __restrict__ tile_local, const u64* __restrict__ block_prefix, u32 n_tiles,
@@ -568,12 +640,13 @@ k_emit_ordered(const uint4* __restrict__ temp, const u64* __restrict__ tile_base
   }
   if (over) atomicOr(status, TPC_STATUS_OVERFLOW);
 }
+#endif
 
 // K9p: the packed variant of K9 (O6: 16-byte fixed-point record) plus
 // the per-row index.  One warp per tile, one cluster per lane; the first tile of every pad row
 // also writes where that row starts.  When the run buffer was too small (flag) nothing is
 // written but the NO_PACKED status bit.
-#define TPC_STATUS_NO_PACKED 4u
+#if TPC_UNITS & TPC_U_ORDER
 extern "C" __global__ void __launch_bounds__(256)
 k_emit_packed(const uint4* __restrict__ temp, const u64* __restrict__ tile_base, const u32* __restrict__ tile_cnt,
               const u32* __restrict__ tile_local, const u64* __restrict__ block_prefix, u32 n_tiles,
@@ -615,6 +688,7 @@ k_emit_packed(const uint4* __restrict__ temp, const u64* __restrict__ tile_base,
   }
   if (over) atomicOr(status, TPC_STATUS_OVERFLOW);
 }
+#endif
 
 // ==========================================================================================
 // K5  partition_fine  (NS (1), second half: group every record with the tile(s) whose shared-
@@ -637,11 +711,8 @@ k_emit_packed(const uint4* __restrict__ temp, const u64* __restrict__ tile_base,
 // For tile sl, tl = f ^ ((sl & 1) << 7) is the row in its map: own slab -> m, next slab -> TS + m;
 // tl >= TPC_TT means "not mine".  Tile sl OWNS rows tl in [3, TS+3).
 // ==========================================================================================
-#define TPC_NSLMAX 128u   // >= slabs per bin: TPC_TC / TPC_TS = 127
-#define TPC_NKEY (2u * TPC_NSLMAX + 32u)   // sort keys: 2 per slab + A of the slab after the last; multiple of 32
-#define TPC_K5_BUF (TPC_CPB * TPC_CHUNK + 4u * TPC_NSLMAX + 8u)   // u32 words: the records of a batch + alignment gaps + end padding
-__host__ __device__ inline u32 tpc_k5_smem_bytes() { return (TPC_K5_BUF + 2u * TPC_NKEY + 8u) * 4u; }
 
+#if TPC_UNITS & TPC_U_PART_FINE
 extern "C" __global__ void __launch_bounds__(TPC_K5_THREADS, 1)
 k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, const u32* __restrict__ chunk_list,
                  const u32* __restrict__ bin_chunk_start, const u32* __restrict__ batch_start,
@@ -824,6 +895,7 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
   if (threadIdx.x >= TPC_K5_THREADS - 32u) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
   if (bad) atomicOr(status, TPC_STATUS_BAD_DIGITS);
 }
+#endif
 
 // ==========================================================================================
 // K6  cluster_tiles  (NS (1) last step + (2) + (3) + (4); rules O0..O5 of SURVEY.md 8(c))
@@ -840,28 +912,6 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
 // from one atomic (FAST) or from a single-pass chained scan of the tile counts (DETERMINISTIC,
 // k6_chain below).  Tiles are handed out by ticket, in increasing order.
 // ==========================================================================================
-#define TPC_MODE_FAST 0
-#define TPC_MODE_DET 1        // chained scan inside K6 (fallback: any number of clusters)
-#define TPC_MODE_DET_TEMP 2   // runs into the temporary buffer, K7-K9 order them (the usual path)
-#define TPC_MODE_DUMP_MAP 3
-#define TPC_K6_CONSUMERS 256u                   // threads that compute
-#define TPC_K6_THREADS (TPC_K6_CONSUMERS + 32u)  // + the producer warp
-#define TPC_K6_CAP 4096u                         // records staged per round (16 KB)
-#define TPC_K6_CAPU (TPC_K6_CAP / 4u)            // ... in 16-byte units
-#ifndef TPC_K6_CTAS
-#define TPC_K6_CTAS 3                            // resident CTAs per SM (shared memory and registers)
-#endif
-
-struct K6Args {
-  const u32* blob; const u64* idx; const u32* batch_start;
-  uint4* out; u64 capacity; u64* n_clusters; u32* status;
-  u32* ticket;        // next tile to hand out (zeroed per run)
-  u64* tile_state;    // DET: chained scan of the tile counts, [n_tiles], zeroed per run
-  uint4* temp; u64 temp_cap; u64* temp_cursor;   // DET_TEMP: run buffer (the dead K1 pool), in clusters
-  u64* tile_base; u32* tile_cnt; u32* det_flag;  // DET_TEMP: per-tile (place, count); flag = buffer too small
-  u16* dmap; const u64* row_off;   // DUMP_MAP only: row_off[r] = cells of rows < r in one sector; [n_rows] = per sector
-};
-
 // ---- mbarrier / bulk-copy / packed-max helpers (PTX; SASS: SYNCS.*, UBLKCP, VIMNMX3.U16x2) --
 __device__ __forceinline__ u32 smem_addr(const void* p) { u64 a; asm("cvta.to.shared.u64 %0, %1;" : "=l"(a) : "l"(p)); return (u32)a; }
 __device__ __forceinline__ void mbar_init(u64* bar, u32 count) {
@@ -921,11 +971,6 @@ struct K6Smem {
 // misc: [0] n_peaks  [3] first tile of the stage  [4] tiles in the stage  [5] row | sector << 8 |
 //       n_pads << 16  [6] time of row 0 of the first tile  [7] its slab  [8+2m],[9+2m] offset and
 //       size (16-byte units) of tile m's records in `rec`
-#define TPC_K6_GROUP 4u   // tiles (consecutive slabs of one bin) a ticket covers
-#define TPC_K6_PMW 9u
-__host__ __device__ inline u32 tpc_k6_smem_bytes(u32 pitch, u32 max_peaks) {
-  return (TPC_K6_CAP + TPC_TT * pitch / 2u + 4u + 2u + TPC_TT * (8u + TPC_K6_PMW) + TPC_TT + 2u + 16u + (max_peaks + 1u) / 2u) * 4u + 128u;
-}
 __device__ __forceinline__ K6Smem k6_smem(u32* p) {
   K6Smem s;
   s.rec = p; p += TPC_K6_CAP;
@@ -1592,11 +1637,22 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
   }
 // the chained-scan variants only run when K7-K9 could not deliver the ordered output (flag set)
 #define TPC_K6_IF_FLAG if (*a.det_flag == 0u) return;
+#if TPC_UNITS & TPC_U_TILES_FAST
 TPC_K6_ENTRY(k_cluster_tiles_fast, TPC_MODE_FAST, false, )
+#endif
+#if TPC_UNITS & TPC_U_TILES_DET
 TPC_K6_ENTRY(k_cluster_tiles_det, TPC_MODE_DET, false, TPC_K6_IF_FLAG)
 TPC_K6_ENTRY(k_cluster_tiles_det_temp, TPC_MODE_DET_TEMP, false, )
+#endif
+#if TPC_UNITS & TPC_U_TILES_DUMP
 TPC_K6_ENTRY(k_cluster_tiles_dump_map, TPC_MODE_DUMP_MAP, false, )
+#endif
 // reading Q10' (TPCCLUS_COG_GATED)
+#if TPC_UNITS & TPC_U_TILES_FAST_G
 TPC_K6_ENTRY(k_cluster_tiles_fast_gated, TPC_MODE_FAST, true, )
+#endif
+#if TPC_UNITS & TPC_U_TILES_DET_G
 TPC_K6_ENTRY(k_cluster_tiles_det_gated, TPC_MODE_DET, true, TPC_K6_IF_FLAG)
 TPC_K6_ENTRY(k_cluster_tiles_det_temp_gated, TPC_MODE_DET_TEMP, true, )
+#endif
+#endif   // TPC_UNITS != 0u

@@ -122,3 +122,19 @@ def test_exhaustive_3x3_all_262144_maps_strict_nonstrict_form():
     tall.reshape(len(maps), 5, 3)[:, :3, :] = maps
     f = t1.row_flags(tall, 6, 4).reshape(len(maps), 5, 3)[:, :3, :] & 1
     assert np.array_equal(f.astype(bool), ok)
+
+
+def test_sector_parallel_driver_equals_single_call():
+    """`t1.clusterize_by_sector` (the all-core baseline of bench.py and the full-frame GPU parity
+    tests) is the single-threaded routine applied sector by sector: same bytes, any thread count."""
+    from workloads import make_frame
+    fr = make_frame(2, sectors=[0, 5, 35], n_time=200)
+    d = fr.digits_numpy().view(t1.DIGIT)
+    full, st, _ = t1.clusterize(d, fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads)
+    assert st == 0 and len(full) > 1000
+    for threads in (1, 3):
+        tm = {}
+        res = t1.clusterize_by_sector(lambda s: d[d["sector"] == s], [0, 5, 35], fr.n_rows, fr.n_time, fr.n_pads,
+                                      threads=threads, timing=tm)
+        assert np.concatenate([res[s] for s in (0, 5, 35)]).tobytes() == full.tobytes()
+        assert tm["cores"] == threads and tm["digits"] == len(d)
