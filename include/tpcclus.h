@@ -91,8 +91,13 @@ enum {
                                    true total, the buffer holds `capacity` valid records (FAST:
                                    any subset; DETERMINISTIC: the first `capacity` in order) */
   TPCCLUS_STATUS_BAD_DIGITS = 2, /* at least one digit was out of range and ignored */
-  TPCCLUS_STATUS_NO_PACKED = 4   /* tpcclus_run_packed only: the frame has more clusters than the run
+  TPCCLUS_STATUS_NO_PACKED = 4,  /* tpcclus_run_packed only: the frame has more clusters than the run
                                     buffer holds (max_digits / 8); nothing was written but *n_clusters */
+  TPCCLUS_STATUS_INTERNAL = 0x80000000u /* a workspace capacity the library derived from max_digits was
+                                    exceeded on the device (a partition slice or the tile-record blob).
+                                    Cannot happen for n <= max_digits -- it would be a bug of the library;
+                                    digits were dropped and the output is invalid.  Provoked on purpose
+                                    only through tpcclus_debug_shrink (tests) */
 };
 
 /* return codes */
@@ -159,14 +164,15 @@ typedef struct {
  * and max_digits only).  Returns 0 for invalid or unsupported parameters.  Host call. */
 TPCCLUS_API uint64_t tpcclus_workspace_bytes(const tpcclus_params* params);
 
-/* Validates, copies the geometry, lays out the workspace, uploads nothing yet (the
- * parameter block goes to __constant__ memory at the head of every run(), stream-ordered,
- * so several handles with different geometry can share a process: PAPER.md 85).  With
- * TPCCLUS_RTC the kernels are compiled here for sm_100a by NVRTC and loaded as a module
- * (PAPER.md 64, 91).  Host call, synchronous.  *out is NULL on failure.
- * Generic (non-RTC) handles of one process share ONE __constant__ block: runs of handles with
- * DIFFERENT parameters must not overlap in time on different streams (same stream, or equal
- * parameters, or RTC handles -- which carry their constants in their own module -- are fine). */
+/* Validates, copies the geometry, lays out the workspace and brings the device code in (PAPER.md
+ * section 3, line 64): the kernels are built as separate compilation units, one GPU binary per kernel
+ * family, embedded in the library; create loads the units this handle can launch with the driver's
+ * module loader.  Each unit has its own __constant__ parameter block (PAPER.md 81); the handle
+ * registers every block it finds and fills all of them with the parameters (PAPER.md 83-85).  With
+ * TPCCLUS_RTC the units are compiled here for sm_100a by NVRTC instead, in parallel, with every
+ * parameter a literal, and loaded through the same loader (PAPER.md 89-93).
+ * Host call, synchronous.  *out is NULL on failure.  Modules and constant blocks are per handle:
+ * handles of any parameters may run concurrently on different streams. */
 TPCCLUS_API int tpcclus_create(const tpcclus_params* params, tpcclus_handle** out);
 
 /* Clusterizes one time frame: enqueues every step of the path (NS (1)..(5)) on
@@ -191,6 +197,13 @@ TPCCLUS_API int tpcclus_run_host(tpcclus_handle* h, const tpcclus_digit* h_digit
                                  void* cuda_stream);
 
 TPCCLUS_API int tpcclus_destroy(tpcclus_handle* h);
+
+/* The constant buffers may change between time frames (PAPER.md 79, 85): sets new thresholds and
+ * rewrites EVERY registered constant block of the handle (one per loaded unit), stream-ordered on
+ * `cuda_stream` -- runs enqueued on that stream before the call keep the old values, runs after it see
+ * the new ones.  thr_peak 1..1023, noise_eps 0..1023.  Refused (TPCCLUS_ERR_INVALID_ARG) for RTC
+ * handles, whose parameters are compiled in. */
+TPCCLUS_API int tpcclus_update_params(tpcclus_handle* h, uint16_t thr_peak, uint16_t noise_eps, void* cuda_stream);
 
 /* Static string for a return code.  Never NULL. */
 TPCCLUS_API const char* tpcclus_error_string(int code);
@@ -231,6 +244,15 @@ TPCCLUS_API int tpcclus_rtc_cache_hit(const tpcclus_handle* h);
  * TPCCLUS_STATUS_NO_PACKED is set and only *n_clusters is valid.  Enqueues only, like tpcclus_run. */
 TPCCLUS_API int tpcclus_run_packed(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n,
                                    const tpcclus_out_packed* out, void* cuda_stream);
+
+/* Number of constant blocks in the handle's registry (= loaded offline-compiled units; 0 for RTC
+ * handles), and the names of the loaded compilation units (static strings; returns the count). */
+TPCCLUS_API int tpcclus_constant_buffers(const tpcclus_handle* h);
+TPCCLUS_API int tpcclus_loaded_units(const tpcclus_handle* h, const char** names, int cap);
+
+/* Test hook: makes later runs pretend the partition slice (chunks per CTA) and the tile-record blob
+ * (records) are smaller than laid out (0 = as laid out), so that TPCCLUS_STATUS_INTERNAL can be seen. */
+TPCCLUS_API int tpcclus_debug_shrink(tpcclus_handle* h, uint32_t slice_cap, uint64_t blob_cap);
 
 /* Debug/parity hook for step a1 (the charge map): after a run(), rebuilds the dense
  * [sector][row][time][pad] uint16 map (O0) from the binned digits into d_map (DEVICE,

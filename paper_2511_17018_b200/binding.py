@@ -19,7 +19,7 @@ _LIB_PATH = os.path.join(_HERE, "libtpcclus.so")
 MODE_FAST, MODE_DETERMINISTIC = 0, 1
 RTC = 1
 COG_GATED = 2
-STATUS_OVERFLOW, STATUS_BAD_DIGITS, STATUS_NO_PACKED = 1, 2, 4
+STATUS_OVERFLOW, STATUS_BAD_DIGITS, STATUS_NO_PACKED, STATUS_INTERNAL = 1, 2, 4, 0x80000000
 FLAG_EDGE_PAD, FLAG_EDGE_TIME, FLAG_SATURATED = 1, 2, 4
 
 # include/tpcclus.h: tpcclus_digit (8 B) and tpcclus_cluster (32 B)
@@ -62,7 +62,8 @@ _lib = None
 EXPORTS = ("tpcclus_workspace_bytes", "tpcclus_workspace_bytes_host", "tpcclus_create", "tpcclus_run",
            "tpcclus_run_host", "tpcclus_destroy", "tpcclus_error_string", "tpcclus_last_error",
            "tpcclus_launches_per_run", "tpcclus_set_timing", "tpcclus_last_timing", "tpcclus_rtc_build_ms",
-           "tpcclus_debug_dense_map", "tpcclus_debug_det_fallback", "tpcclus_set_rtc_cache_dir", "tpcclus_rtc_cache_hit", "tpcclus_run_packed")
+           "tpcclus_debug_dense_map", "tpcclus_debug_det_fallback", "tpcclus_set_rtc_cache_dir", "tpcclus_rtc_cache_hit", "tpcclus_run_packed",
+           "tpcclus_update_params", "tpcclus_constant_buffers", "tpcclus_loaded_units", "tpcclus_debug_shrink")
 
 
 def lib() -> C.CDLL:
@@ -110,6 +111,14 @@ def lib() -> C.CDLL:
     L.tpcclus_rtc_cache_hit.argtypes = [C.c_void_p]
     L.tpcclus_debug_det_fallback.restype = C.c_int
     L.tpcclus_debug_det_fallback.argtypes = [C.c_void_p]
+    L.tpcclus_update_params.restype = C.c_int
+    L.tpcclus_update_params.argtypes = [C.c_void_p, C.c_uint16, C.c_uint16, C.c_void_p]
+    L.tpcclus_constant_buffers.restype = C.c_int
+    L.tpcclus_constant_buffers.argtypes = [C.c_void_p]
+    L.tpcclus_loaded_units.restype = C.c_int
+    L.tpcclus_loaded_units.argtypes = [C.c_void_p, P(C.c_char_p), C.c_int]
+    L.tpcclus_debug_shrink.restype = C.c_int
+    L.tpcclus_debug_shrink.argtypes = [C.c_void_p, C.c_uint32, C.c_uint64]
     _lib = L
     return L
 
@@ -265,6 +274,27 @@ class Clusterizer:
     @property
     def rtc_cache_hit(self):
         return int(lib().tpcclus_rtc_cache_hit(self._h)) == 1
+
+    def update_params(self, thr_peak, noise_eps, stream=None):
+        """tpcclus_update_params: new thresholds into every registered constant block, stream-ordered."""
+        st = (stream or self._torch.cuda.current_stream(self.device)).cuda_stream
+        rc = lib().tpcclus_update_params(self._h, int(thr_peak), int(noise_eps), C.c_void_p(st))
+        if rc != 0:
+            raise TpcclusError(rc, "tpcclus_update_params", (lib().tpcclus_last_error(self._h) or b"").decode())
+
+    @property
+    def constant_buffers(self):
+        return int(lib().tpcclus_constant_buffers(self._h))
+
+    def loaded_units(self):
+        names = (C.c_char_p * 32)()
+        k = lib().tpcclus_loaded_units(self._h, names, 32)
+        return [names[i].decode() for i in range(k)]
+
+    def debug_shrink(self, slice_cap=0, blob_cap=0):
+        rc = lib().tpcclus_debug_shrink(self._h, int(slice_cap), int(blob_cap))
+        if rc != 0:
+            raise TpcclusError(rc, "tpcclus_debug_shrink")
 
     def dense_map(self, stream=None):
         """Debug hook (step a1): the O0 map of the last run as a flat uint16 CUDA tensor in

@@ -2,9 +2,10 @@
 
     python -m paper_2511_17018_b200.build [--force]
 
-The kernel text (csrc/tpcclus_kernels.cuh) is compiled twice into the library: offline by
-nvcc (generic build, parameters in __constant__ memory) and embedded verbatim as a string
-for the NVRTC build that create(TPCCLUS_RTC) performs (PAPER.md 91: "the source code is
+The kernel text (csrc/tpcclus_kernels.cuh) goes into the library twice: offline, cut into
+compilation units that nvcc compiles one by one, in parallel, straight to GPU binaries
+(PAPER.md 64; generic build, parameters in each unit's __constant__ block), and verbatim as a
+string for the NVRTC build that create(TPCCLUS_RTC) performs (PAPER.md 91: "the source code is
 embedded in the library").
 """
 from __future__ import annotations
@@ -18,15 +19,18 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtpcclus.so")
 GEN_DIR = os.path.join(ROOT, "build")
-GEN = os.path.join(GEN_DIR, "tpcclus_kernel_source.c")
-SOURCES = [os.path.join(CSRC, "tpcclus.cu"), os.path.join(CSRC, "tpcclus_kernels.cuh"),
+GEN = os.path.join(GEN_DIR, "tpcclus_embedded.S")
+SOURCES = [os.path.join(CSRC, "tpcclus.cu"), os.path.join(CSRC, "tpcclus_kernels.cuh"), os.path.join(CSRC, "tpcclus_unit.cu"),
            os.path.join(ROOT, "include", "tpcclus.h")]
 
-NVCC_FLAGS = [
-    "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-    "--fmad=false", "--prec-div=true", "--prec-sqrt=true", "--ftz=false",   # PAPER.md 37-39
-    "-Xcompiler", "-fPIC,-fvisibility=hidden", "-shared", "-cudart", "static",
-]
+# compilation units (PAPER.md 64: one GPU binary per kernel family): name -> TPC_U_* bit of tpcclus_kernels.cuh
+UNITS = {"part_coarse": 0x001, "dir": 0x002, "part_fine": 0x004, "tiles_fast": 0x008, "tiles_det": 0x010,
+         "order": 0x020, "tiles_dump": 0x040, "tiles_fast_g": 0x080, "tiles_det_g": 0x100}
+
+ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
+DEVICE_FLAGS = [*ARCH, "-lineinfo", "-O3", "-std=c++17",
+                "--fmad=false", "--prec-div=true", "--prec-sqrt=true", "--ftz=false"]   # PAPER.md 37-39
+HOST_FLAGS = [*ARCH, "-O3", "-std=c++17", "-Xcompiler", "-fPIC,-fvisibility=hidden", "-shared", "-cudart", "static"]
 
 
 def _nvcc() -> str:
@@ -36,13 +40,32 @@ def _nvcc() -> str:
     return "nvcc"
 
 
-def _embed_source() -> None:
-    os.makedirs(GEN_DIR, exist_ok=True)
-    with open(os.path.join(CSRC, "tpcclus_kernels.cuh"), "rb") as f:
-        src = f.read()
-    text = "const char tpcclus_kernel_source[] = {" + ",".join(str(b) for b in src) + ",0};\n"
+def unit_cubin(name: str) -> str:
+    return os.path.join(GEN_DIR, "unit_%s.cubin" % name)
+
+
+def _compile_unit(name: str, verbose: bool) -> str:
+    """One unit straight to a GPU binary: nvcc -cubin for sm_100a (no PTX, no host code)."""
+    out = unit_cubin(name)
+    cmd = [_nvcc(), *DEVICE_FLAGS, *os.environ.get("TPC_EXTRA", "").split(), *(["-Xptxas", "-v"] if verbose else []),
+           "-DTPC_UNITS=%du" % UNITS[name], "-cubin", "-o", out, os.path.join(CSRC, "tpcclus_unit.cu")]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode != 0:
+        raise RuntimeError("nvcc failed for unit %s:\n%s\n%s" % (name, r.stdout, r.stderr))
+    return r.stderr
+
+
+def _embed() -> None:
+    """The unit binaries and the kernel text (for NVRTC; PAPER.md 91: "the source code is embedded in
+    the library") go into the library through one assembler file of .incbin directives."""
+    lines = ['.section .rodata', '.balign 16', '.global tpcclus_kernel_source', 'tpcclus_kernel_source:',
+             '.incbin "%s"' % os.path.join(CSRC, "tpcclus_kernels.cuh"), '.byte 0']
+    for name in UNITS:
+        lines += ['.balign 16', '.global tpcclus_cubin_%s' % name, 'tpcclus_cubin_%s:' % name,
+                  '.incbin "%s"' % unit_cubin(name), '.global tpcclus_cubin_%s_end' % name, 'tpcclus_cubin_%s_end:' % name]
+    lines.append('.section .note.GNU-stack,"",@progbits')
     with open(GEN, "w") as f:
-        f.write(text)
+        f.write("\n".join(lines) + "\n")
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -51,11 +74,18 @@ def build(force: bool = False, verbose: bool = False) -> str:
         newest = max(os.path.getmtime(s) for s in SOURCES + [os.path.abspath(__file__)])
         if os.path.getmtime(LIB) >= newest:
             return LIB
-    _embed_source()
+    os.makedirs(GEN_DIR, exist_ok=True)
+    from concurrent.futures import ThreadPoolExecutor
+    with ThreadPoolExecutor(max_workers=min(len(UNITS), os.cpu_count() or 1)) as ex:   # PAPER.md 64: the units build in parallel
+        logs = list(ex.map(lambda n: _compile_unit(n, verbose), UNITS))
+    if verbose:
+        for name, log in zip(UNITS, logs):
+            print("== unit %s\n%s" % (name, log), file=sys.stderr)
+    _embed()
+    obj = os.path.join(GEN_DIR, "tpcclus_embedded.o")
+    subprocess.check_call(["gcc", "-c", "-o", obj, GEN])
     tmp = LIB + ".tmp%d" % os.getpid()
-    cmd = [_nvcc(), *NVCC_FLAGS, *os.environ.get("TPC_EXTRA", "").split(), *(["-Xptxas", "-v"] if verbose else []), "-o", tmp,
-           os.path.join(CSRC, "tpcclus.cu"), GEN, "-ldl"]
-    subprocess.check_call(cmd)
+    subprocess.check_call([_nvcc(), *HOST_FLAGS, *os.environ.get("TPC_EXTRA", "").split(), "-o", tmp, os.path.join(CSRC, "tpcclus.cu"), obj, "-ldl"])
     os.replace(tmp, LIB)
     return LIB
 

@@ -1,11 +1,22 @@
 // tpcclus.cu -- host side of libtpcclus.so: the C ABI of include/tpcclus.h.
 //
 // Orchestration only: parameter validation, workspace layout, the launch sequence of
-// tpcclus_kernels.cuh, the stream-ordered __constant__ upload (PAPER.md 85) and the NVRTC
-// build of the same kernel text with constants baked in (PAPER.md 89-93; loaded through the
-// driver's module loader like the paper's per-kernel binaries, PAPER.md 64, 91).
-// No step of the path runs on the host; without a CUDA device every entry point that
-// would compute returns TPCCLUS_ERR_CUDA.
+// tpcclus_kernels.cuh, the module loader and the constant-buffer registry.  No step of the path
+// runs on the host; without a CUDA device every entry point that would compute returns
+// TPCCLUS_ERR_CUDA.
+//
+// How the device code gets here (section 3, lines 52-66, and section 5, lines 87-93):
+//   * The kernel text is cut into COMPILATION UNITS, one per kernel family (TPC_U_* in the .cuh).
+//     The build compiles each unit on its own, straight to a GPU binary (nvcc -cubin), and embeds
+//     the binaries in this library; a handle loads them with cuModuleLoadData (PAPER.md 64).
+//   * create(TPCCLUS_RTC) compiles the same units with NVRTC instead, every parameter a literal
+//     (PAPER.md 89-93), and loads them through the very same loader (PAPER.md 91).
+//   * Every offline-compiled unit carries its own copy of the __constant__ parameter block -- a
+//     non-RDC unit cannot see another unit's symbol (PAPER.md 81).  The handle's registry looks the
+//     symbol up in every module it loads, fills all copies at create and rewrites all of them when
+//     the parameters change (tpcclus_update_params; PAPER.md 83-85).  Modules are per handle, so
+//     handles with different parameters never share a constant block: any two handles may run
+//     concurrently on different streams.
 #include <cuda_runtime.h>
 #include <dlfcn.h>
 #include <fcntl.h>
@@ -16,13 +27,25 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
+#include <thread>
 #include <vector>
 
 #include "../../include/tpcclus.h"
+#define TPC_UNITS 0u   // declarations only: the kernels live in the embedded unit binaries
 #include "tpcclus_kernels.cuh"
 
-extern "C" const char tpcclus_kernel_source[];   // generated from tpcclus_kernels.cuh at build time
+extern "C" const char tpcclus_kernel_source[];   // the kernel text, embedded at build time (PAPER.md 91)
+
+// the unit binaries, embedded at build time (build/tpcclus_units.S: .incbin of build/unit_<name>.cubin)
+#define TPC_UNIT_LIST(X)                                                                              \
+  X(part_coarse, TPC_U_PART_COARSE) X(dir, TPC_U_DIR) X(part_fine, TPC_U_PART_FINE)                  \
+  X(tiles_fast, TPC_U_TILES_FAST) X(tiles_det, TPC_U_TILES_DET) X(order, TPC_U_ORDER)                \
+  X(tiles_dump, TPC_U_TILES_DUMP) X(tiles_fast_g, TPC_U_TILES_FAST_G) X(tiles_det_g, TPC_U_TILES_DET_G)
+#define X(name, bit) extern "C" const unsigned char tpcclus_cubin_##name[]; extern "C" const unsigned char tpcclus_cubin_##name##_end[];
+TPC_UNIT_LIST(X)
+#undef X
 
 namespace {
 
@@ -102,7 +125,9 @@ int make_geometry(const tpcclus_params* p, Geometry* g) {
   g->n_chunks_max = (uint64_t)g->g1 * cap;
   if (g->n_chunks_max > 0x00FFFFFFFFull) return TPCCLUS_ERR_INVALID_ARG;
   g->n_batches_max = g->n_chunks_max / TPC_CPB + nb + 1;
-  g->blob_cap = p->max_digits * (dup + 2) + g->n_batches_max * 8ull * q.n_sl + 64;   // K5 halo copies + run padding
+  // K5 writes every record once; per batch at most 3 zero records in front of each of its n_sl + 1
+  // A runs (16-byte alignment) and 7 at its end (32-byte alignment)
+  g->blob_cap = p->max_digits * dup + g->n_batches_max * (3ull * (q.n_sl + 1) + 8ull) + 64;
   g->idx_cap = g->n_batches_max * q.n_sl;
   g->n_tiles = q.n_bins * q.n_sl;
   g->n_scan_blocks = (g->n_tiles + TPC_SCAN_PER_CTA - 1) / TPC_SCAN_PER_CTA;
@@ -141,15 +166,21 @@ int make_geometry(const tpcclus_params* p, Geometry* g) {
   return TPCCLUS_OK;
 }
 
-// ---- lazily loaded driver / NVRTC entry points (RTC handles only) ------------------------
-struct Rtc {
-  void* libcuda = nullptr; void* libnvrtc = nullptr;
+// ---- driver API (module loader) and NVRTC entry points, resolved once per process ---------------
+struct Drv {
+  void* lib = nullptr;
   int (*cuModuleLoadData)(void**, const void*) = nullptr;
   int (*cuModuleUnload)(void*) = nullptr;
   int (*cuModuleGetFunction)(void**, void*, const char*) = nullptr;
+  int (*cuModuleGetGlobal_v2)(unsigned long long*, size_t*, void*, const char*) = nullptr;
   int (*cuFuncSetAttribute)(void*, int, int) = nullptr;
   int (*cuLaunchKernel)(void*, unsigned, unsigned, unsigned, unsigned, unsigned, unsigned, unsigned, void*, void**, void**) = nullptr;
   int (*cuGetErrorString)(int, const char**) = nullptr;
+  bool ok = false;
+  std::string why;
+};
+struct Nvrtc {
+  void* lib = nullptr;
   int (*nvrtcCreateProgram)(void**, const char*, const char*, int, const char* const*, const char* const*) = nullptr;
   int (*nvrtcCompileProgram)(void*, int, const char* const*) = nullptr;
   int (*nvrtcGetCUBINSize)(void*, size_t*) = nullptr;
@@ -162,47 +193,63 @@ struct Rtc {
   std::string why;
 };
 
-Rtc& rtc() {
-  static Rtc r;
-  static bool tried = false;
-  if (tried) return r;
-  tried = true;
-  r.libcuda = dlopen("libcuda.so.1", RTLD_NOW | RTLD_GLOBAL);
-  if (!r.libcuda) { r.why = "dlopen(libcuda.so.1) failed"; return r; }
-  // the toolkit's own NVRTC first (12.9: knows the 256-bit vector store), then whatever the process has
-  for (const char* name : {"/usr/local/cuda/lib64/libnvrtc.so.12", "/usr/local/cuda/targets/x86_64-linux/lib/libnvrtc.so.12",
-                           "libnvrtc.so.12", "libnvrtc.so"}) {
-    r.libnvrtc = dlopen(name, RTLD_NOW);
-    if (r.libnvrtc) break;
-  }
-  if (!r.libnvrtc) { r.why = "dlopen(libnvrtc) failed"; return r; }
-  bool all = true;
-#define SYM(lib, f) do { *(void**)(&r.f) = dlsym(r.lib, #f); if (!r.f) { all = false; r.why = "missing symbol " #f; } } while (0)
-  SYM(libcuda, cuModuleLoadData); SYM(libcuda, cuModuleUnload); SYM(libcuda, cuModuleGetFunction);
-  SYM(libcuda, cuFuncSetAttribute); SYM(libcuda, cuLaunchKernel); SYM(libcuda, cuGetErrorString);
-  SYM(libnvrtc, nvrtcCreateProgram); SYM(libnvrtc, nvrtcCompileProgram); SYM(libnvrtc, nvrtcGetCUBINSize);
-  SYM(libnvrtc, nvrtcGetCUBIN); SYM(libnvrtc, nvrtcGetProgramLogSize); SYM(libnvrtc, nvrtcGetProgramLog);
-  SYM(libnvrtc, nvrtcDestroyProgram); SYM(libnvrtc, nvrtcVersion);
-#undef SYM
-  r.ok = all;
+#define SYM(r, f) do { *(void**)(&(r).f) = dlsym((r).lib, #f); if (!(r).f) { all = false; (r).why = "missing symbol " #f; } } while (0)
+Drv& drv() {
+  static Drv r;
+  static std::once_flag once;
+  std::call_once(once, [] {
+    r.lib = dlopen("libcuda.so.1", RTLD_NOW | RTLD_GLOBAL);
+    if (!r.lib) { r.why = "dlopen(libcuda.so.1) failed"; return; }
+    bool all = true;
+    SYM(r, cuModuleLoadData); SYM(r, cuModuleUnload); SYM(r, cuModuleGetFunction); SYM(r, cuModuleGetGlobal_v2);
+    SYM(r, cuFuncSetAttribute); SYM(r, cuLaunchKernel); SYM(r, cuGetErrorString);
+    r.ok = all;
+  });
   return r;
 }
+Nvrtc& nvrtc() {
+  static Nvrtc r;
+  static std::once_flag once;
+  std::call_once(once, [] {
+    // the toolkit's own NVRTC first (12.9: knows the 256-bit vector store), then whatever the process has
+    for (const char* name : {"/usr/local/cuda/lib64/libnvrtc.so.12", "/usr/local/cuda/targets/x86_64-linux/lib/libnvrtc.so.12",
+                             "libnvrtc.so.12", "libnvrtc.so"}) {
+      r.lib = dlopen(name, RTLD_NOW);
+      if (r.lib) break;
+    }
+    if (!r.lib) { r.why = "dlopen(libnvrtc) failed"; return; }
+    bool all = true;
+    SYM(r, nvrtcCreateProgram); SYM(r, nvrtcCompileProgram); SYM(r, nvrtcGetCUBINSize); SYM(r, nvrtcGetCUBIN);
+    SYM(r, nvrtcGetProgramLogSize); SYM(r, nvrtcGetProgramLog); SYM(r, nvrtcDestroyProgram); SYM(r, nvrtcVersion);
+    r.ok = all;
+  });
+  return r;
+}
+#undef SYM
+std::string drv_error(int rc) {
+  const char* s = nullptr;
+  drv().cuGetErrorString(rc, &s);
+  return s ? s : "?";
+}
+
+// ---- compilation units and kernels -------------------------------------------------------------
+enum UnitId { U_PART_COARSE, U_DIR, U_PART_FINE, U_TILES_FAST, U_TILES_DET, U_ORDER, U_TILES_DUMP, U_TILES_FAST_G, U_TILES_DET_G, U_COUNT_ };
+struct UnitInfo { const char* name; uint32_t bit; const unsigned char* cubin; const unsigned char* cubin_end; };
+#define X(name, bit) {#name, bit, tpcclus_cubin_##name, tpcclus_cubin_##name##_end},
+const UnitInfo kUnits[U_COUNT_] = {TPC_UNIT_LIST(X)};
+#undef X
 
 enum KernelId { K_PART_COARSE, K_DIR_COUNT, K_DIR_SCAN, K_DIR_FILL, K_PART_FINE, K_TILES_FAST, K_TILES_DET,
                 K_TILES_DET_TEMP, K_TILES_DUMP, K_SCAN_LOCAL, K_SCAN_SUMS, K_EMIT_ORDERED, K_EMIT_PACKED,
                 K_TILES_FAST_G, K_TILES_DET_G, K_TILES_DET_TEMP_G, K_COUNT_ };
-const char* const kKernelNames[K_COUNT_] = {
-    "k_partition_coarse", "k_dir_count", "k_dir_scan", "k_dir_fill", "k_partition_fine", "k_cluster_tiles_fast",
-    "k_cluster_tiles_det", "k_cluster_tiles_det_temp", "k_cluster_tiles_dump_map", "k_scan_local", "k_scan_sums",
-    "k_emit_ordered", "k_emit_packed", "k_cluster_tiles_fast_gated", "k_cluster_tiles_det_gated",
-    "k_cluster_tiles_det_temp_gated"};
-const void* const kKernelPtrs[K_COUNT_] = {
-    (const void*)k_partition_coarse, (const void*)k_dir_count, (const void*)k_dir_scan, (const void*)k_dir_fill,
-    (const void*)k_partition_fine, (const void*)k_cluster_tiles_fast, (const void*)k_cluster_tiles_det,
-    (const void*)k_cluster_tiles_det_temp, (const void*)k_cluster_tiles_dump_map, (const void*)k_scan_local,
-    (const void*)k_scan_sums, (const void*)k_emit_ordered, (const void*)k_emit_packed,
-    (const void*)k_cluster_tiles_fast_gated, (const void*)k_cluster_tiles_det_gated,
-    (const void*)k_cluster_tiles_det_temp_gated};
+struct KernelInfo { const char* name; UnitId unit; int smem; };   // smem: 0 none/static, 1 K1, 5 K5, 6 K6
+const KernelInfo kKernels[K_COUNT_] = {
+    {"k_partition_coarse", U_PART_COARSE, 1}, {"k_dir_count", U_DIR, 0}, {"k_dir_scan", U_DIR, 0}, {"k_dir_fill", U_DIR, 0},
+    {"k_partition_fine", U_PART_FINE, 5}, {"k_cluster_tiles_fast", U_TILES_FAST, 6}, {"k_cluster_tiles_det", U_TILES_DET, 6},
+    {"k_cluster_tiles_det_temp", U_TILES_DET, 6}, {"k_cluster_tiles_dump_map", U_TILES_DUMP, 6},
+    {"k_scan_local", U_ORDER, 0}, {"k_scan_sums", U_ORDER, 0}, {"k_emit_ordered", U_ORDER, 0}, {"k_emit_packed", U_ORDER, 0},
+    {"k_cluster_tiles_fast_gated", U_TILES_FAST_G, 6}, {"k_cluster_tiles_det_gated", U_TILES_DET_G, 6},
+    {"k_cluster_tiles_det_temp_gated", U_TILES_DET_G, 6}};
 
 }  // namespace
 
@@ -211,12 +258,18 @@ struct tpcclus_handle {
   tpcclus_params params;   // copy; n_pads points into g.prm
   char* ws = nullptr;
   bool is_rtc = false;
-  void* module = nullptr;
+  void* module[U_COUNT_] = {};     // one loaded GPU binary per compilation unit (PAPER.md 64)
+  bool unit_cached[U_COUNT_] = {};
   void* fn[K_COUNT_] = {};
+  // constant-buffer registry (PAPER.md 81-85): the device address of every module's parameter block
+  struct ConstSym { UnitId unit; void* dptr; size_t bytes; };
+  std::vector<ConstSym> consts;
   double rtc_ms = 0.0;
   bool rtc_cache_hit = false;
   uint32_t smem_k1 = 0, smem_k5 = 0, smem_k6 = 0;
   uint32_t grid_k5 = 0, grid_k6 = 0;
+  uint32_t dbg_slice_cap = 0;      // test hook: a smaller K1 slice (tpcclus_debug_shrink)
+  uint64_t dbg_blob_cap = 0;
   bool timing = false;
   int n_timed = 0;
   const char* timed_name[kMaxKernels] = {};
@@ -234,33 +287,38 @@ int fail(tpcclus_handle* h, int code, const std::string& detail) {
 #define CUDA_TRY(h, expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) { cudaGetLastError(); \
   return fail(h, TPCCLUS_ERR_CUDA, std::string(#expr) + ": " + cudaGetErrorString(e_)); } } while (0)
 
-// One launch, generic (runtime API, offline-compiled kernel) or RTC (driver API, NVRTC module).
+// The entry points select the handle's device and put the caller's back on every way out.
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  cudaError_t enter(int device) {
+    if (cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); prev = -1; }
+    if (prev == device) return cudaSuccess;
+    cudaError_t e = cudaSetDevice(device);
+    switched = e == cudaSuccess;
+    return e;
+  }
+  ~DeviceGuard() { if (switched && prev >= 0) cudaSetDevice(prev); }
+};
+
+// One launch through the driver's module loader path: offline-compiled unit or NVRTC unit alike.
 int launch(tpcclus_handle* h, KernelId k, dim3 grid, dim3 block, uint32_t smem, cudaStream_t st, void** args) {
+  if (!h->fn[k]) return fail(h, TPCCLUS_ERR_CUDA, std::string("kernel not loaded: ") + kKernels[k].name);
   if (h->timing && h->n_timed < kMaxKernels) {
     if (h->n_timed == 0) cudaEventRecord(h->ev[0], st);
-    h->timed_name[h->n_timed] = kKernelNames[k];
+    h->timed_name[h->n_timed] = kKernels[k].name;
   }
-  if (h->is_rtc) {
-    int rc = rtc().cuLaunchKernel(h->fn[k], grid.x, grid.y, grid.z, block.x, block.y, block.z, smem, st, args, nullptr);
-    if (rc != 0) {
-      const char* s = nullptr; rtc().cuGetErrorString(rc, &s);
-      return fail(h, TPCCLUS_ERR_CUDA, std::string("cuLaunchKernel(") + kKernelNames[k] + "): " + (s ? s : "?"));
-    }
-  } else {
-    cudaError_t e = cudaLaunchKernel(kKernelPtrs[k], grid, block, args, smem, st);
-    if (e != cudaSuccess) {
-      cudaGetLastError();
-      return fail(h, TPCCLUS_ERR_CUDA, std::string("cudaLaunchKernel(") + kKernelNames[k] + "): " + cudaGetErrorString(e));
-    }
-  }
+  int rc = drv().cuLaunchKernel(h->fn[k], grid.x, grid.y, grid.z, block.x, block.y, block.z, smem, st, args, nullptr);
+  if (rc != 0) return fail(h, TPCCLUS_ERR_CUDA, std::string("cuLaunchKernel(") + kKernels[k].name + "): " + drv_error(rc));
   if (h->timing && h->n_timed < kMaxKernels) { ++h->n_timed; cudaEventRecord(h->ev[h->n_timed], st); }
   return TPCCLUS_OK;
 }
 
-// Text put in front of the kernel source for NVRTC: every parameter as a literal.
-std::string rtc_prologue(const TpcParams& q) {
+// Text put in front of the kernel source for NVRTC: every parameter as a literal, and the unit.
+std::string rtc_prologue(const TpcParams& q, uint32_t unit_bit) {
   char buf[256];
   std::string s = "#define TPC_RTC 1\n";
+  snprintf(buf, sizeof buf, "#define TPC_UNITS %uu\n", unit_bit); s += buf;
 #define DEF(f) do { snprintf(buf, sizeof buf, "#define TPC_" #f " %uu\n", q.f); s += buf; } while (0)
   DEF(n_sectors); DEF(n_rows); DEF(n_time); DEF(n_tc); DEF(n_bins); DEF(n_sl); DEF(pitch); DEF(max_pads);
   DEF(thr_peak); DEF(noise_eps); DEF(max_peaks); DEF(cog_gated);
@@ -271,27 +329,26 @@ std::string rtc_prologue(const TpcParams& q) {
   return s;
 }
 
-// NVRTC: kernel text -> cubin for sm_100a.
-int compile_cubin(const std::string& src, std::vector<char>* cubin) {
-  Rtc& r = rtc();
+// NVRTC: kernel text -> cubin for sm_100a.  Thread-safe (one program per call); errors in *err.
+int compile_cubin(const std::string& src, std::vector<char>* cubin, std::string* err) {
+  Nvrtc& r = nvrtc();
   void* prog = nullptr;
-  if (r.nvrtcCreateProgram(&prog, src.c_str(), "tpcclus_kernels.cu", 0, nullptr, nullptr) != 0)
-    return fail(nullptr, TPCCLUS_ERR_NVRTC, "nvrtcCreateProgram failed");
+  if (r.nvrtcCreateProgram(&prog, src.c_str(), "tpcclus_kernels.cu", 0, nullptr, nullptr) != 0) { *err = "nvrtcCreateProgram failed"; return TPCCLUS_ERR_NVRTC; }
   const char* opts[] = {"--gpu-architecture=sm_100a", "-std=c++17", "-default-device", "-lineinfo", "--fmad=false", "--prec-div=true",
                         "--prec-sqrt=true", "--ftz=false", "-DTPC_NO_ST256=1"};
   int rc = r.nvrtcCompileProgram(prog, 8, opts);
   if (rc != 0) {   // older NVRTC: retry without the 256-bit store
     r.nvrtcDestroyProgram(&prog);
     prog = nullptr;
-    if (r.nvrtcCreateProgram(&prog, src.c_str(), "tpcclus_kernels.cu", 0, nullptr, nullptr) != 0)
-      return fail(nullptr, TPCCLUS_ERR_NVRTC, "nvrtcCreateProgram failed");
+    if (r.nvrtcCreateProgram(&prog, src.c_str(), "tpcclus_kernels.cu", 0, nullptr, nullptr) != 0) { *err = "nvrtcCreateProgram failed"; return TPCCLUS_ERR_NVRTC; }
     rc = r.nvrtcCompileProgram(prog, 9, opts);
   }
   if (rc != 0) {
     size_t n = 0; r.nvrtcGetProgramLogSize(prog, &n);
     std::string log(n, '\0'); if (n) r.nvrtcGetProgramLog(prog, &log[0]);
     r.nvrtcDestroyProgram(&prog);
-    return fail(nullptr, TPCCLUS_ERR_NVRTC, "nvrtcCompileProgram failed:\n" + log);
+    *err = "nvrtcCompileProgram failed:\n" + log;
+    return TPCCLUS_ERR_NVRTC;
   }
   size_t n = 0; r.nvrtcGetCUBINSize(prog, &n);
   cubin->resize(n);
@@ -302,49 +359,61 @@ int compile_cubin(const std::string& src, std::vector<char>* cubin) {
 
 // On-disk cubin cache (PAPER.md 97: several processes per node share one run-time compilation,
 // serialised by a file lock).  Key = hash of the exact text handed to NVRTC (prologue with every
-// baked parameter + kernel source) and of the NVRTC version.  The compile happens under an
-// exclusive flock on <key>.lock; the cubin is written to a temporary name and renamed, so a
-// reader sees a whole file or none.  Any I/O problem just means "compile, do not cache".
+// baked parameter and the unit + kernel source) and of the NVRTC version.  The compile happens under
+// an exclusive flock on <key>.lock; the file is written under a temporary name and renamed, so a
+// reader sees a whole file or none.  File = 24-byte header (magic, payload length, FNV-1a of the
+// payload) + cubin: a truncated, corrupt or foreign file is deleted and compiled afresh.  Any I/O
+// problem just means "compile, do not cache".
+std::mutex g_cache_mutex;
 std::string g_cache_dir;   // set by tpcclus_set_rtc_cache_dir or $TPCCLUS_RTC_CACHE
 
-bool read_file(const std::string& path, std::vector<char>* out) {
+uint64_t fnv1a(const char* p, size_t n, uint64_t h = 1469598103934665603ull) {
+  for (size_t i = 0; i < n; ++i) { h ^= (unsigned char)p[i]; h *= 1099511628211ull; }
+  return h;
+}
+constexpr uint64_t kCacheMagic = 0x31434250434c4354ull;   // "TCLCPBC1"
+
+bool read_cached(const std::string& path, std::vector<char>* out) {
   FILE* f = fopen(path.c_str(), "rb");
   if (!f) return false;
-  fseek(f, 0, SEEK_END);
-  long n = ftell(f);
-  fseek(f, 0, SEEK_SET);
-  bool ok = n > 0;
-  if (ok) { out->resize((size_t)n); ok = fread(out->data(), 1, (size_t)n, f) == (size_t)n; }
+  uint64_t hdr[3] = {0, 0, 0};
+  bool ok = fread(hdr, 1, sizeof hdr, f) == sizeof hdr && hdr[0] == kCacheMagic && hdr[1] > 0 && hdr[1] < (1ull << 30);
+  if (ok) {
+    out->resize((size_t)hdr[1]);
+    ok = fread(out->data(), 1, out->size(), f) == out->size() && fgetc(f) == EOF && fnv1a(out->data(), out->size()) == hdr[2];
+  }
   fclose(f);
+  if (!ok) { out->clear(); remove(path.c_str()); }   // not ours, cut short or damaged: compile afresh
   return ok;
 }
 
-int cubin_for(const std::string& src, std::vector<char>* cubin, bool* hit) {
+int cubin_for(const std::string& src, std::vector<char>* cubin, bool* hit, std::string* err) {
   *hit = false;
-  std::string dir = g_cache_dir;
+  std::string dir;
+  { std::lock_guard<std::mutex> lk(g_cache_mutex); dir = g_cache_dir; }
   if (dir.empty()) { const char* e = getenv("TPCCLUS_RTC_CACHE"); if (e) dir = e; }
-  if (dir.empty()) return compile_cubin(src, cubin);
+  if (dir.empty()) return compile_cubin(src, cubin, err);
   int vmaj = 0, vmin = 0;
-  if (rtc().nvrtcVersion) rtc().nvrtcVersion(&vmaj, &vmin);
-  uint64_t hsh = 1469598103934665603ull;   // FNV-1a
-  auto mix = [&](const char* p, size_t n) { for (size_t i = 0; i < n; ++i) { hsh ^= (unsigned char)p[i]; hsh *= 1099511628211ull; } };
-  mix(src.data(), src.size());
-  char tag[64]; snprintf(tag, sizeof tag, "|nvrtc %d.%d|sm_100a", vmaj, vmin); mix(tag, strlen(tag));
+  if (nvrtc().nvrtcVersion) nvrtc().nvrtcVersion(&vmaj, &vmin);
+  uint64_t hsh = fnv1a(src.data(), src.size());
+  char tag[64]; snprintf(tag, sizeof tag, "|nvrtc %d.%d|sm_100a", vmaj, vmin);
+  hsh = fnv1a(tag, strlen(tag), hsh);
   char name[64]; snprintf(name, sizeof name, "/tpcclus_%016llx", (unsigned long long)hsh);
   const std::string base = dir + name, file = base + ".cubin", lock = base + ".lock";
-  if (read_file(file, cubin)) { *hit = true; return TPCCLUS_OK; }
+  if (read_cached(file, cubin)) { *hit = true; return TPCCLUS_OK; }
   int fd = open(lock.c_str(), O_CREAT | O_RDWR, 0644);
   if (fd >= 0) flock(fd, LOCK_EX);   // whoever comes second waits here, then finds the file
   int rc = TPCCLUS_OK;
-  if (fd >= 0 && read_file(file, cubin)) {
+  if (fd >= 0 && read_cached(file, cubin)) {
     *hit = true;
   } else {
-    rc = compile_cubin(src, cubin);
+    rc = compile_cubin(src, cubin, err);
     if (rc == TPCCLUS_OK && fd >= 0) {
-      char tmp[64]; snprintf(tmp, sizeof tmp, ".tmp%d", (int)getpid());
+      char tmp[64]; snprintf(tmp, sizeof tmp, ".tmp%d_%llx", (int)getpid(), (unsigned long long)(uintptr_t)cubin);
       FILE* f = fopen((file + tmp).c_str(), "wb");
       if (f) {
-        bool ok = fwrite(cubin->data(), 1, cubin->size(), f) == cubin->size();
+        const uint64_t hdr[3] = {kCacheMagic, (uint64_t)cubin->size(), fnv1a(cubin->data(), cubin->size())};
+        bool ok = fwrite(hdr, 1, sizeof hdr, f) == sizeof hdr && fwrite(cubin->data(), 1, cubin->size(), f) == cubin->size();
         ok = fclose(f) == 0 && ok;
         if (ok) rename((file + tmp).c_str(), file.c_str()); else remove((file + tmp).c_str());
       }
@@ -354,30 +423,86 @@ int cubin_for(const std::string& src, std::vector<char>* cubin, bool* hit) {
   return rc;
 }
 
-int build_rtc(tpcclus_handle* h) {
-  Rtc& r = rtc();
-  if (!r.ok) return fail(nullptr, TPCCLUS_ERR_NVRTC, "RTC unavailable: " + r.why);
-  auto t0 = std::chrono::steady_clock::now();
-  std::string src = rtc_prologue(h->g.prm) + tpcclus_kernel_source;
-  std::vector<char> cubin;
-  int rc = cubin_for(src, &cubin, &h->rtc_cache_hit);
-  if (rc != TPCCLUS_OK) return rc;
-  if (cudaFree(nullptr) != cudaSuccess) { cudaGetLastError(); return fail(nullptr, TPCCLUS_ERR_CUDA, "no CUDA context"); }
-  if ((rc = r.cuModuleLoadData(&h->module, cubin.data())) != 0) {
-    const char* s = nullptr; r.cuGetErrorString(rc, &s);
-    return fail(nullptr, TPCCLUS_ERR_CUDA, std::string("cuModuleLoadData: ") + (s ? s : "?"));
+// Loads one unit's GPU binary into the handle, resolves its kernels, sizes their dynamic shared
+// memory and REGISTERS its constant block (PAPER.md 83: "automatically register all constant memory
+// symbols"), filling it with the handle's parameters.
+int load_unit(tpcclus_handle* h, UnitId u, const void* image) {
+  Drv& d = drv();
+  int rc = d.cuModuleLoadData(&h->module[u], image);
+  if (rc != 0) return fail(nullptr, TPCCLUS_ERR_CUDA, std::string("cuModuleLoadData(") + kUnits[u].name + "): " + drv_error(rc));
+  for (int k = 0; k < K_COUNT_; ++k) {
+    if (kKernels[k].unit != u) continue;
+    if ((rc = d.cuModuleGetFunction(&h->fn[k], h->module[u], kKernels[k].name)) != 0)
+      return fail(nullptr, TPCCLUS_ERR_CUDA, std::string("cuModuleGetFunction(") + kKernels[k].name + "): " + drv_error(rc));
+    const uint32_t smem = kKernels[k].smem == 1 ? h->smem_k1 : kKernels[k].smem == 5 ? h->smem_k5 : kKernels[k].smem == 6 ? h->smem_k6 : 0u;
+    const int CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES = 8;
+    if (smem > 48u * 1024u && (rc = d.cuFuncSetAttribute(h->fn[k], CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES, (int)smem)) != 0)
+      return fail(nullptr, TPCCLUS_ERR_CUDA, std::string("cuFuncSetAttribute(") + kKernels[k].name + "): " + drv_error(rc));
   }
-  for (int k = 0; k < K_COUNT_; ++k)
-    if (r.cuModuleGetFunction(&h->fn[k], h->module, kKernelNames[k]) != 0)
-      return fail(nullptr, TPCCLUS_ERR_NVRTC, std::string("cuModuleGetFunction: ") + kKernelNames[k]);
-  const int CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES = 8;
-  struct { int k; uint32_t b; } sm[] = {{K_PART_COARSE, h->smem_k1}, {K_PART_FINE, h->smem_k5}, {K_TILES_FAST, h->smem_k6},
-                                        {K_TILES_DET, h->smem_k6}, {K_TILES_DET_TEMP, h->smem_k6}, {K_TILES_DUMP, h->smem_k6},
-                                        {K_TILES_FAST_G, h->smem_k6}, {K_TILES_DET_G, h->smem_k6}, {K_TILES_DET_TEMP_G, h->smem_k6}};
-  for (auto& e : sm)
-    if (r.cuFuncSetAttribute(h->fn[e.k], CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES, (int)e.b) != 0)
-      return fail(nullptr, TPCCLUS_ERR_CUDA, std::string("cuFuncSetAttribute: ") + kKernelNames[e.k]);
-  h->rtc_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+  unsigned long long dptr = 0; size_t bytes = 0;
+  if (d.cuModuleGetGlobal_v2(&dptr, &bytes, h->module[u], "c_prm") == 0) {   // RTC units have literals instead: nothing to register
+    if (bytes != sizeof(TpcParams)) return fail(nullptr, TPCCLUS_ERR_CUDA, std::string("constant block of unit ") + kUnits[u].name + " has the wrong size");
+    h->consts.push_back({u, (void*)(uintptr_t)dptr, bytes});
+    cudaError_t e = cudaMemcpy((void*)(uintptr_t)dptr, &h->g.prm, sizeof(TpcParams), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(nullptr, TPCCLUS_ERR_CUDA, std::string("constant upload: ") + cudaGetErrorString(e)); }
+  }
+  return TPCCLUS_OK;
+}
+
+// Brings the listed units into the handle: embedded binaries (generic) or NVRTC builds (RTC; the
+// units compile in parallel threads -- PAPER.md 64: "the compilation can be parallelized").
+int load_units(tpcclus_handle* h, const std::vector<UnitId>& want) {
+  if (!drv().ok) return fail(nullptr, TPCCLUS_ERR_CUDA, "driver API unavailable: " + drv().why);
+  std::vector<UnitId> units;
+  for (UnitId u : want) if (!h->module[u]) units.push_back(u);
+  if (units.empty()) return TPCCLUS_OK;
+  if (cudaFree(nullptr) != cudaSuccess) { cudaGetLastError(); return fail(nullptr, TPCCLUS_ERR_CUDA, "no CUDA context"); }
+  if (!h->is_rtc) {
+    for (UnitId u : units) { int rc = load_unit(h, u, kUnits[u].cubin); if (rc) return rc; }
+    return TPCCLUS_OK;
+  }
+  if (!nvrtc().ok) return fail(nullptr, TPCCLUS_ERR_NVRTC, "RTC unavailable: " + nvrtc().why);
+  auto t0 = std::chrono::steady_clock::now();
+  // With the on-disk cache, processes that start together with the same parameters queue up here:
+  // the first compiles all units, the others then find every unit in the cache (PAPER.md 97).
+  int lock_fd = -1;
+  {
+    std::string dir;
+    { std::lock_guard<std::mutex> lk(g_cache_mutex); dir = g_cache_dir; }
+    if (dir.empty()) { const char* e = getenv("TPCCLUS_RTC_CACHE"); if (e) dir = e; }
+    if (!dir.empty()) {
+      const std::string pro = rtc_prologue(h->g.prm, 0u);
+      char name[64]; snprintf(name, sizeof name, "/tpcclus_handle_%016llx.lock", (unsigned long long)fnv1a(pro.data(), pro.size()));
+      lock_fd = open((dir + name).c_str(), O_CREAT | O_RDWR, 0644);
+      if (lock_fd >= 0) flock(lock_fd, LOCK_EX);
+    }
+  }
+  struct Unlock { int fd; ~Unlock() { if (fd >= 0) { flock(fd, LOCK_UN); close(fd); } } } unlock{lock_fd};
+  const size_t n = units.size();
+  std::vector<std::vector<char>> cubins(n);
+  std::vector<int> rcs(n, TPCCLUS_OK);
+  std::vector<std::string> errs(n);
+  std::vector<char> hits(n, 0);
+  std::vector<std::thread> th;
+  for (size_t i = 0; i < n; ++i)
+    th.emplace_back([&, i] {
+      bool hit = false;
+      rcs[i] = cubin_for(rtc_prologue(h->g.prm, kUnits[units[i]].bit) + tpcclus_kernel_source, &cubins[i], &hit, &errs[i]);
+      hits[i] = hit;
+    });
+  for (auto& t : th) t.join();
+  bool all_hit = true;
+  for (size_t i = 0; i < n; ++i) {
+    if (rcs[i]) return fail(nullptr, rcs[i], std::string("unit ") + kUnits[units[i]].name + ": " + errs[i]);
+    all_hit = all_hit && hits[i];
+  }
+  for (size_t i = 0; i < n; ++i) {
+    int rc = load_unit(h, units[i], cubins[i].data());
+    if (rc) return rc;
+    h->unit_cached[units[i]] = hits[i] != 0;
+  }
+  h->rtc_cache_hit = all_hit;
+  h->rtc_ms += std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
   return TPCCLUS_OK;
 }
 
@@ -404,7 +529,8 @@ int tpcclus_create(const tpcclus_params* p, tpcclus_handle** out) {
   if (rc != TPCCLUS_OK) return fail(nullptr, rc, "invalid or unsupported parameters");
   if (!p->workspace || ((uintptr_t)p->workspace & 255u)) return fail(nullptr, TPCCLUS_ERR_INVALID_ARG, "workspace null or not 256-byte aligned");
   if (p->workspace_bytes < g.lay.total) return fail(nullptr, TPCCLUS_ERR_WORKSPACE_TOO_SMALL, "workspace too small");
-  CUDA_TRY(nullptr, cudaSetDevice(p->device));
+  DeviceGuard dg;
+  CUDA_TRY(nullptr, dg.enter(p->device));
   tpcclus_handle* h = new tpcclus_handle();
   h->g = g;
   h->params = *p;
@@ -415,25 +541,19 @@ int tpcclus_create(const tpcclus_params* p, tpcclus_handle** out) {
   h->smem_k6 = tpc_k6_smem_bytes(g.prm.pitch, g.prm.max_peaks);
   h->grid_k5 = g.g1;
   h->grid_k6 = g.g1 * TPC_K6_CTAS < g.n_tiles ? g.g1 * TPC_K6_CTAS : g.n_tiles;
-  auto bail = [&](int code) { std::string e = h->err.empty() ? g_create_error : h->err; delete h; g_create_error = e; return code; };
+  h->is_rtc = (p->flags & TPCCLUS_RTC) != 0;
+  auto bail = [&](int code) { std::string e = h->err.empty() ? g_create_error : h->err; tpcclus_destroy(h); g_create_error = e; return code; };
   // static table for the debug map hook
   std::vector<uint64_t> ro(p->n_rows + 1, 0);
   for (uint32_t r = 0; r < p->n_rows; ++r) ro[r + 1] = ro[r] + (uint64_t)p->n_time * p->n_pads[r];
   cudaError_t e = cudaMemcpy(h->ws + g.lay.row_off, ro.data(), 8ull * ro.size(), cudaMemcpyHostToDevice);
   if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("cudaMemcpy(row_off): ") + cudaGetErrorString(e); return bail(TPCCLUS_ERR_CUDA); }
-  if (p->flags & TPCCLUS_RTC) {
-    h->is_rtc = true;
-    rc = build_rtc(h);
-    if (rc != TPCCLUS_OK) return bail(rc);
-  } else {
-    struct { int k; uint32_t b; } sm[] = {{K_PART_COARSE, h->smem_k1}, {K_PART_FINE, h->smem_k5}, {K_TILES_FAST, h->smem_k6},
-                                          {K_TILES_DET, h->smem_k6}, {K_TILES_DET_TEMP, h->smem_k6}, {K_TILES_DUMP, h->smem_k6},
-                                        {K_TILES_FAST_G, h->smem_k6}, {K_TILES_DET_G, h->smem_k6}, {K_TILES_DET_TEMP_G, h->smem_k6}};
-    for (auto& s : sm) {
-      e = cudaFuncSetAttribute(kKernelPtrs[s.k], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s.b);
-      if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("cudaFuncSetAttribute(") + kKernelNames[s.k] + "): " + cudaGetErrorString(e); return bail(TPCCLUS_ERR_CUDA); }
-    }
-  }
+  // the units this handle can launch (the debug unit comes on demand); a handle of reading Q10'
+  // loads -- and, under RTC, compiles -- the gated tile units instead of the plain ones
+  const bool gated = g.prm.cog_gated != 0u;
+  rc = load_units(h, {U_PART_COARSE, U_DIR, U_PART_FINE, gated ? U_TILES_FAST_G : U_TILES_FAST,
+                      gated ? U_TILES_DET_G : U_TILES_DET, U_ORDER});
+  if (rc != TPCCLUS_OK) return bail(rc);
   for (int i = 0; i <= kMaxKernels; ++i)
     if (cudaEventCreate(&h->ev[i]) != cudaSuccess) { cudaGetLastError(); g_create_error = "cudaEventCreate failed"; return bail(TPCCLUS_ERR_CUDA); }
   *out = h;
@@ -442,10 +562,38 @@ int tpcclus_create(const tpcclus_params* p, tpcclus_handle** out) {
 
 int tpcclus_destroy(tpcclus_handle* h) {
   if (!h) return TPCCLUS_ERR_INVALID_ARG;
+  DeviceGuard dg;
+  dg.enter(h->params.device);
   for (int i = 0; i <= kMaxKernels; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
-  if (h->module) rtc().cuModuleUnload(h->module);
+  for (int u = 0; u < U_COUNT_; ++u) if (h->module[u]) drv().cuModuleUnload(h->module[u]);
   delete h;
   return TPCCLUS_OK;
+}
+
+// PAPER.md 79, 85: the constant buffers may change between time frames; the framework rewrites
+// ALL registered copies, in stream order, so runs enqueued before keep the old values.
+int tpcclus_update_params(tpcclus_handle* h, uint16_t thr_peak, uint16_t noise_eps, void* cuda_stream) {
+  if (!h) return TPCCLUS_ERR_INVALID_ARG;
+  h->err.clear();
+  if (thr_peak < 1 || thr_peak > 1023 || noise_eps > 1023) return fail(h, TPCCLUS_ERR_INVALID_ARG, "tpcclus_update_params: threshold out of range");
+  if (h->is_rtc) return fail(h, TPCCLUS_ERR_INVALID_ARG, "tpcclus_update_params: an RTC handle has its parameters compiled in (PAPER.md 89-91); create a new handle");
+  DeviceGuard dg;
+  CUDA_TRY(h, dg.enter(h->params.device));
+  h->g.prm.thr_peak = thr_peak; h->g.prm.noise_eps = noise_eps;
+  h->params.thr_peak = thr_peak; h->params.noise_eps = noise_eps;
+  for (const auto& c : h->consts)   // pageable source: staged by the driver before the call returns
+    CUDA_TRY(h, cudaMemcpyAsync(c.dptr, &h->g.prm, sizeof(TpcParams), cudaMemcpyHostToDevice, (cudaStream_t)cuda_stream));
+  return TPCCLUS_OK;
+}
+
+int tpcclus_constant_buffers(const tpcclus_handle* h) { return h ? (int)h->consts.size() : TPCCLUS_ERR_INVALID_ARG; }
+
+int tpcclus_loaded_units(const tpcclus_handle* h, const char** names, int cap) {
+  if (!h) return TPCCLUS_ERR_INVALID_ARG;
+  int n = 0;
+  for (int u = 0; u < U_COUNT_; ++u)
+    if (h->module[u]) { if (names && n < cap) names[n] = kUnits[u].name; ++n; }
+  return n;
 }
 
 const char* tpcclus_error_string(int code) {
@@ -490,6 +638,7 @@ double tpcclus_rtc_build_ms(const tpcclus_handle* h) { return h ? h->rtc_ms : 0.
 int tpcclus_rtc_cache_hit(const tpcclus_handle* h) { return h && h->rtc_cache_hit ? 1 : 0; }
 
 int tpcclus_set_rtc_cache_dir(const char* dir) {
+  std::lock_guard<std::mutex> lk(g_cache_mutex);
   g_cache_dir = dir ? dir : "";
   return TPCCLUS_OK;
 }
@@ -525,8 +674,6 @@ RunPtrs ptrs(tpcclus_handle* h) {
 int enqueue_binning(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n, u32* status, cudaStream_t st) {
   const Geometry& g = h->g;
   RunPtrs p = ptrs(h);
-  if (!h->is_rtc)   // PAPER.md 85: the constant buffer is rewritten for every time frame, in stream order
-    CUDA_TRY(h, cudaMemcpyToSymbolAsync(c_prm, &g.prm, sizeof(TpcParams), 0, cudaMemcpyHostToDevice, st));
   CUDA_TRY(h, cudaMemsetAsync(h->ws + g.lay.counters, 0, g.lay.counters_bytes, st));
   if (status != p.status) CUDA_TRY(h, cudaMemsetAsync(status, 0, 4, st));
   const uint64_t round = (uint64_t)TPC_K1_THREADS * TPC_K1_DPT;
@@ -534,7 +681,8 @@ int enqueue_binning(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n
   if (per_cta == 0) per_cta = round;
   const uint2* dig = (const uint2*)d_digits;
   u64 n64 = n;
-  u32 slice_cap = g.slice_cap;
+  u32 slice_cap = h->dbg_slice_cap ? h->dbg_slice_cap : g.slice_cap;
+  u64 blob_cap = h->dbg_blob_cap ? h->dbg_blob_cap : g.blob_cap;
   int rc;
   { void* a[] = {&dig, &n64, &per_cta, &p.pool, &p.dir, &p.used, &slice_cap, &status};
     if ((rc = launch(h, K_PART_COARSE, dim3(g.g1), dim3(TPC_K1_THREADS), h->smem_k1, st, a))) return rc; }
@@ -545,7 +693,7 @@ int enqueue_binning(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n
     if ((rc = launch(h, K_DIR_SCAN, dim3(1), dim3(TPC_SCAN_THREADS), smem_nb, st, a))) return rc; }
   { void* a[] = {&p.dir, &p.used, &slice_cap, &p.slice_cnt, &p.bin_chunk_start, &p.chunk_list};
     if ((rc = launch(h, K_DIR_FILL, dim3(g.g1), dim3(TPC_SCAN_THREADS), smem_nb, st, a))) return rc; }
-  { void* a[] = {&p.pool, &p.dir, &p.chunk_list, &p.bin_chunk_start, &p.batch_start, &p.batch_bin, &p.blob, &p.blob_cursor, &p.idx, &status};
+  { void* a[] = {&p.pool, &p.dir, &p.chunk_list, &p.bin_chunk_start, &p.batch_start, &p.batch_bin, &p.blob, &p.blob_cursor, &blob_cap, &p.idx, &status};
     if ((rc = launch(h, K_PART_FINE, dim3(h->grid_k5), dim3(TPC_K5_THREADS), h->smem_k5, st, a))) return rc; }
   return TPCCLUS_OK;
 }
@@ -568,7 +716,8 @@ static int run_impl(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n
       ((uintptr_t)o_clusters & 15u) || ((uintptr_t)o_n & 7u) || (packed && (!packed->row_index || ((uintptr_t)packed->row_index & 7u))))
     return fail(h, TPCCLUS_ERR_INVALID_ARG, "tpcclus_run: bad argument");
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  CUDA_TRY(h, cudaSetDevice(h->params.device));
+  DeviceGuard dg;
+  CUDA_TRY(h, dg.enter(h->params.device));
   h->n_timed = 0;
   RunPtrs p = ptrs(h);
   u32* status = o_status ? o_status : p.status;
@@ -635,7 +784,8 @@ int tpcclus_run_host(tpcclus_handle* h, const tpcclus_digit* h_digits, uint64_t 
       h->params.workspace_bytes < L.host_clusters + 32ull * capacity)
     return fail(h, TPCCLUS_ERR_INVALID_ARG, "tpcclus_run_host: bad argument or workspace not sized with tpcclus_workspace_bytes_host");
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  CUDA_TRY(h, cudaSetDevice(h->params.device));
+  DeviceGuard dg;
+  CUDA_TRY(h, dg.enter(h->params.device));
   tpcclus_digit* d_dig = (tpcclus_digit*)(h->ws + L.host_digits);
   tpcclus_out o;
   o.clusters = (tpcclus_cluster*)(h->ws + L.host_clusters);
@@ -661,14 +811,27 @@ int tpcclus_run_host(tpcclus_handle* h, const tpcclus_digit* h_digits, uint64_t 
 int tpcclus_debug_det_fallback(tpcclus_handle* h) {
   if (!h) return TPCCLUS_ERR_INVALID_ARG;
   uint32_t f = 0;
+  DeviceGuard dg;
+  CUDA_TRY(h, dg.enter(h->params.device));
   CUDA_TRY(h, cudaMemcpy(&f, h->ws + h->g.lay.det_flag, 4, cudaMemcpyDeviceToHost));   // synchronises
   return f != 0 ? 1 : 0;
+}
+
+int tpcclus_debug_shrink(tpcclus_handle* h, uint32_t slice_cap, uint64_t blob_cap) {
+  if (!h || slice_cap > h->g.slice_cap || blob_cap > h->g.blob_cap) return TPCCLUS_ERR_INVALID_ARG;
+  h->dbg_slice_cap = slice_cap;
+  h->dbg_blob_cap = blob_cap;
+  return TPCCLUS_OK;
 }
 
 int tpcclus_debug_dense_map(tpcclus_handle* h, uint16_t* d_map, void* cuda_stream) {
   if (!h || !d_map) return TPCCLUS_ERR_INVALID_ARG;
   if (!h->ran) return fail(h, TPCCLUS_ERR_INVALID_ARG, "tpcclus_debug_dense_map: no run() yet");
   cudaStream_t st = (cudaStream_t)cuda_stream;
+  DeviceGuard dg;
+  CUDA_TRY(h, dg.enter(h->params.device));
+  int rc = load_units(h, {U_TILES_DUMP});   // the debug unit is loaded (RTC: compiled) on first use
+  if (rc) { h->err = g_create_error; return rc; }
   const Geometry& g = h->g;
   RunPtrs p = ptrs(h);
   uint64_t cells = 0;
@@ -681,7 +844,7 @@ int tpcclus_debug_dense_map(tpcclus_handle* h, uint16_t* d_map, void* cuda_strea
   a.dmap = d_map; a.row_off = p.row_off; a.ticket = p.ticket; a.tile_state = p.tile_state; a.det_flag = p.det_flag;
   CUDA_TRY(h, cudaMemsetAsync(p.ticket, 0, 4, st));   // the run before used the tickets up
   void* ka[] = {&a};
-  int rc = launch(h, K_TILES_DUMP, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka);
+  rc = launch(h, K_TILES_DUMP, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka);
   h->timing = t;
   return rc;
 }

@@ -56,6 +56,7 @@ typedef unsigned char u8;
 
 #define TPC_STATUS_OVERFLOW 1u
 #define TPC_STATUS_BAD_DIGITS 2u
+#define TPC_STATUS_INTERNAL 0x80000000u   // a capacity the host derived from max_digits was exceeded: a bug, results invalid
 
 struct TpcParams {
   u32 n_sectors, n_rows, n_time;
@@ -340,14 +341,16 @@ __device__ __forceinline__ void k1_rounds(const K1Smem& s, const uint2* __restri
   auto decode = [&](const uint4 (&curd)[TPC_K1_DPT / 2], u32 (&bin)[TPC_K1_DPT], u32 (&rec)[TPC_K1_DPT], u32& pend,
                     u32 (&dbin)[TPC_K1_DPT], u32 (&drec)[TPC_K1_DPT], u32& dpend) {
     pend = 0u; dpend = 0u;
+    u32 vm = 0u;   // digits in range (whatever their charge)
 #pragma unroll
     for (int k = 0; k < TPC_K1_DPT; ++k) {
       const u32 w0 = (k & 1) ? curd[k >> 1].z : curd[k >> 1].x, w1 = (k & 1) ? curd[k >> 1].w : curd[k >> 1].y;
       u32 q = w0 & 0xFFFFu;
       const u32 t = w0 >> 16, pad = w1 & 0xFFu, row = (w1 >> 8) & 0xFFu, sec = (w1 >> 16) & 0xFFu;
-      // O0 / Q4: out of range -> ignored + flagged (pad >= n_pads[row] is caught by K6, where the row is uniform)
+      // O0 / Q4: out of range -> ignored + flagged (pad >= n_pads[row] is caught by K5, where the row is uniform)
       const bool valid = sec < S && row < R && t < T;
       bad |= !valid;
+      vm |= valid ? (1u << k) : 0u;
       q = q > 1023u ? 1023u : q;                                  // Q4: clamp
       const bool ok = valid && q != 0u;                           // Q4: zero charge ignored
       u32 tc = 0u, v = t;
@@ -363,6 +366,16 @@ __device__ __forceinline__ void k1_rounds(const K1Smem& s, const uint2* __restri
         } else if (ok && v + TPC_HALO >= TPC_TC && tc + 1u < NTC) {
           dbin[k] = b0 + 1u; drec[k] = pad | ((v + TPC_HALO - TPC_TC) << 8) | (q << 22); dpend |= 1u << k;
         }
+      }
+    }
+    // A digit in range with charge 0 is ignored (Q4) and never reaches K5, but O0 tests the range
+    // first: its pad is checked here.  Zero suppression drops such digits upstream, so this branch is
+    // taken for the zero padding behind the input's end and otherwise never: one test per round.
+    if (vm & ~pend) {
+#pragma unroll
+      for (int k = 0; k < TPC_K1_DPT; ++k) {
+        const u32 w0 = (k & 1) ? curd[k >> 1].z : curd[k >> 1].x, w1 = (k & 1) ? curd[k >> 1].w : curd[k >> 1].y;
+        if (((vm & ~pend) >> k & 1u) && (w0 | w1) != 0u && (w1 & 0xFFu) >= PRM_NPADS((w1 >> 8) & 0xFFu)) bad = true;
       }
     }
   };
@@ -449,7 +462,7 @@ k_partition_coarse(const uint2* __restrict__ digits, u64 n, u64 per_cta, uint4* 
   __syncthreads();
   if (threadIdx.x == 0) {
     u32 u = s.misc[0];
-    if (u > slice_cap) { u = slice_cap; atomicOr(status, 0x80000000u); }   // cannot happen (bound in DESIGN.md)
+    if (u > slice_cap) { u = slice_cap; atomicOr(status, TPC_STATUS_INTERNAL); }   // cannot happen (bound in DESIGN.md; provoked by tpcclus_debug_shrink)
     used[blockIdx.x] = u;
   }
 }
@@ -716,7 +729,7 @@ k_emit_packed(const uint4* __restrict__ temp, const u64* __restrict__ tile_base,
 extern "C" __global__ void __launch_bounds__(TPC_K5_THREADS, 1)
 k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, const u32* __restrict__ chunk_list,
                  const u32* __restrict__ bin_chunk_start, const u32* __restrict__ batch_start,
-                 const u32* __restrict__ batch_bin, u32* __restrict__ blob, u64* __restrict__ blob_cursor,
+                 const u32* __restrict__ batch_bin, u32* __restrict__ blob, u64* __restrict__ blob_cursor, u64 blob_cap,
                  u64* __restrict__ idx, u32* __restrict__ status) {
   extern __shared__ __align__(128) u32 smem_u32[];
   u32* buf = smem_u32;                       // [TPC_K5_BUF]
@@ -877,7 +890,11 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
     // lane): it costs no LSU wavefronts -- the resource the count and place phases are bound by --
     // and runs while the CTA already counts the next batch.
     const u64 gbase = s_gbase;                 // a multiple of 8 records (32 B)
-    if (threadIdx.x >= TPC_K5_THREADS - 32u) {
+    // the blob is sized for every record once plus the alignment gaps (host: blob_cap); should a batch
+    // not fit -- it cannot -- nothing is written, its tiles get empty runs and the status says so
+    const bool fits = gbase + (u64)((total + 7u) & ~7u) <= blob_cap;
+    if (!fits && threadIdx.x == 0) atomicOr(status, TPC_STATUS_INTERNAL);
+    if (fits && threadIdx.x >= TPC_K5_THREADS - 32u) {
       const u32 bytes = ((total + 7u) >> 3) * 32u, off = (threadIdx.x & 31u) * 4096u;
       if (off < bytes) {
         const u32 nby = bytes - off < 4096u ? bytes - off : 4096u;
@@ -889,7 +906,7 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
     if (threadIdx.x < nsl) {   // tile sl reads A_sl B_sl A_sl+1
       const u32 sl = threadIdx.x;
       const u32 beg = s_off[2u * sl], end = s_off[2u * sl + 3u];   // beg is a multiple of 4
-      idx[(u64)nsl * batch_start[b] + (u64)sl * nbatch_b + kb] = (gbase + beg) | ((u64)(end - beg) << 40);
+      idx[(u64)nsl * batch_start[b] + (u64)sl * nbatch_b + kb] = fits ? (gbase + beg) | ((u64)(end - beg) << 40) : 0ull;
     }
   }
   if (threadIdx.x >= TPC_K5_THREADS - 32u) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");

@@ -413,7 +413,7 @@ def test_rtc_cubin_cache(tp, cuda_device, tmp_path):
         assert p.exitcode == 0
     assert sorted(r[0] for r in res) == [False, True]            # one compiled, one loaded
     assert all(r[2] == exp.tobytes() for r in res)
-    assert len(list(tmp_path.glob("tpcclus_*.cubin"))) == 1
+    assert len(list(tmp_path.glob("tpcclus_*.cubin"))) == 6      # one binary per compilation unit
     tp.tpcclus_set_rtc_cache_dir(str(tmp_path))
     try:
         c = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, fr.n_digits, rtc=True)
@@ -423,7 +423,7 @@ def test_rtc_cubin_cache(tp, cuda_device, tmp_path):
         c = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, fr.n_digits, thr_peak=9, rtc=True)
         assert not c.rtc_cache_hit                                # thresholds are baked in: another key
         c.close()
-        assert len(list(tmp_path.glob("tpcclus_*.cubin"))) == 2
+        assert len(list(tmp_path.glob("tpcclus_*.cubin"))) == 12
     finally:
         tp.tpcclus_set_rtc_cache_dir(None)
 
@@ -614,3 +614,131 @@ def test_sparse_dense_tile_alternation(tp, cuda_device):
         det, fast, st = _run_both(tp, _digits_tensor(dd, cuda_device), 1, 2, T, [P, P])
         assert st == st_exp and det.tobytes() == exp.tobytes()
         _check_fast(fast, exp)
+
+
+def test_two_handles_two_streams_concurrently(tp, cuda_device):
+    """Modules and constant blocks are per handle (R6, PAPER.md 81-85): two generic handles of
+    different geometry AND thresholds run at the same time on two streams, many times over, and each
+    follows its own parameters.  (With one process-wide __constant__ block, as in round 1, the second
+    upload could land while the first handle's kernels were running.)"""
+    import torch
+    a = make_frame(0)                                  # 152 rows x 96 pads x 512
+    b = make_frame(2, device=cuda_device, sectors=[0, 1], n_time=700)   # ragged full geometry, another pitch and bin count
+    ca = tp.Clusterizer(a.n_sectors, a.n_rows, a.n_time, a.n_pads, a.n_digits, thr_peak=6, noise_eps=4)
+    cb = tp.Clusterizer(b.n_sectors, b.n_rows, b.n_time, b.n_pads, b.n_digits, thr_peak=11, noise_eps=1)
+    assert ca.constant_buffers == len(ca.loaded_units()) == 6 and "tiles_dump" not in ca.loaded_units()
+    exp_a, _ = _oracle(a.digits_numpy(), a.n_sectors, a.n_rows, a.n_time, a.n_pads, 6, 4)
+    exp_b, _ = _oracle(b.digits_numpy(), b.n_sectors, b.n_rows, b.n_time, b.n_pads, 11, 1)
+    da, db = a.digits.to(cuda_device), b.digits.to(cuda_device)
+    sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    outs = []
+    for i in range(6):
+        with torch.cuda.stream(sa):
+            ra = ca.run(da, tp.MODE_DETERMINISTIC if i % 2 else tp.MODE_FAST, stream=sa)
+            ra = (ra[0].clone(), ra[1].clone(), ra[2].clone())
+        with torch.cuda.stream(sb):
+            rb = cb.run(db, tp.MODE_DETERMINISTIC, stream=sb)
+            rb = (rb[0].clone(), rb[1].clone(), rb[2].clone())
+        outs.append((i, ra, rb))
+    torch.cuda.synchronize()
+    for i, ra, rb in outs:
+        assert int(ra[2].item()) == 0 and int(rb[2].item()) == 0
+        ga = ra[0][:int(ra[1].item())].cpu().numpy().view(tp.CLUSTER_DTYPE).reshape(-1)
+        gb = rb[0][:int(rb[1].item())].cpu().numpy().view(tp.CLUSTER_DTYPE).reshape(-1)
+        assert gb.tobytes() == exp_b.tobytes()
+        if i % 2:
+            assert ga.tobytes() == exp_a.tobytes()
+        else:
+            _check_fast(ga, exp_a)
+    ca.close(); cb.close()
+
+
+def test_update_params_rewrites_every_constant_block(tp, cuda_device):
+    """PAPER.md 79, 85: constant buffers may change between time frames and the framework rewrites all
+    registered copies.  One handle, thresholds changed between runs on one stream without any host
+    synchronisation: each run sees the values that were current when it was enqueued -- in every
+    unit (K5/K6 read thr/eps, the dump unit is loaded later and must come up with the current values)."""
+    import torch
+    fr = make_frame(1)
+    d = fr.digits.to(cuda_device)
+    c = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, fr.n_digits)
+    seq = [(6, 4), (20, 0), (3, 9), (6, 4)]
+    res = []
+    for thr, eps in seq:
+        c.update_params(thr, eps)
+        cl, n, st = c.run(d, tp.MODE_DETERMINISTIC)
+        res.append((cl.clone(), n.clone(), st.clone()))
+    torch.cuda.synchronize()
+    for (thr, eps), (cl, n, st) in zip(seq, res):
+        exp, _ = _oracle(fr.digits_numpy(), fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, thr, eps)
+        assert int(st.item()) == 0 and cl[:int(n.item())].cpu().numpy().tobytes() == exp.tobytes(), (thr, eps)
+    assert res[0][0][:int(res[0][1].item())].cpu().numpy().tobytes() != res[1][0][:int(res[1][1].item())].cpu().numpy().tobytes()
+    n0 = c.constant_buffers
+    c.dense_map()                                    # brings the debug unit in: one more registered block
+    assert c.constant_buffers == n0 + 1 and "tiles_dump" in c.loaded_units()
+    with pytest.raises(tp.TpcclusError):
+        c.update_params(0, 4)
+    c.close()
+    r = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, fr.n_digits, rtc=True)
+    assert r.constant_buffers == 0                   # literals instead of constant memory (PAPER.md 89-91)
+    with pytest.raises(tp.TpcclusError):
+        r.update_params(7, 4)
+    r.close()
+
+
+def test_internal_status_bit_and_zero_charge_bad_pad(tp, cuda_device):
+    """TPCCLUS_STATUS_INTERNAL (bit 31) is raised when a derived workspace capacity is exceeded -- it
+    cannot be by construction, so the test hook shrinks the capacities: K1's slice, then K5's blob.
+    And O0 tests a digit's range before its charge: a zero-charge digit with pad >= n_pads[row] is
+    flagged BAD_DIGITS like the oracle does (it never reaches K5, where pads are checked otherwise)."""
+    fr = make_frame(0)
+    d = fr.digits.to(cuda_device)
+    c = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, fr.n_digits)
+    exp, _ = _oracle(fr.digits_numpy(), fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads)
+    assert c.run_sync(d, tp.MODE_DETERMINISTIC)[2] == 0
+    c.debug_shrink(slice_cap=2)
+    assert c.run_sync(d, tp.MODE_DETERMINISTIC)[2] & tp.STATUS_INTERNAL
+    c.debug_shrink(blob_cap=1024)
+    assert c.run_sync(d, tp.MODE_FAST)[2] & tp.STATUS_INTERNAL
+    c.debug_shrink()
+    det, n, st = c.run_sync(d, tp.MODE_DETERMINISTIC)
+    assert st == 0 and det.tobytes() == exp.tobytes()
+    c.close()
+    pads = [16, 9, 12]
+    for rows in ([(0, 1, 9, 5, 0)], [(0, 1, 200, 5, 0), (0, 0, 3, 3, 40)], [(0, 1, 8, 5, 0), (0, 0, 3, 3, 40)]):
+        dd = t1.make_digits(rows)
+        e, st_e = _oracle(dd, 1, 3, 64, pads)
+        c = tp.Clusterizer(1, 3, 64, pads, 16)
+        for mode in (tp.MODE_DETERMINISTIC, tp.MODE_FAST):
+            got, n, st = c.run_sync(_digits_tensor(dd, cuda_device), mode)
+            assert st == st_e and n == len(e) and got.tobytes() == e.tobytes(), (rows, mode)
+        c.close()
+    assert st_e == 0          # the last case: pad 8 of a 9-pad row is in range
+
+
+def test_rtc_cache_survives_a_damaged_file(tp, cuda_device, tmp_path):
+    """A truncated or foreign file in the shared cache directory is not loaded: the header (magic,
+    length, checksum) does not match, the file is replaced by a fresh compile, results are unchanged."""
+    fr = make_frame(1)
+    exp, _ = _oracle(fr.digits_numpy(), fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads)
+    tp.tpcclus_set_rtc_cache_dir(str(tmp_path))
+    try:
+        c = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, fr.n_digits, rtc=True)
+        assert not c.rtc_cache_hit
+        c.close()
+        files = sorted(tmp_path.glob("tpcclus_*.cubin"))
+        assert len(files) == 6                        # one cached binary per compilation unit
+        files[0].write_bytes(files[0].read_bytes()[:1000])            # cut short
+        files[1].write_bytes(b"\x7fELF" + b"\0" * 4096)                # not ours
+        raw = bytearray(files[2].read_bytes()); raw[-1] ^= 0xFF
+        files[2].write_bytes(bytes(raw))                                # one byte flipped
+        c = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, fr.n_digits, rtc=True)
+        assert not c.rtc_cache_hit                    # three units were compiled again
+        assert c.run_sync(fr.digits.to(cuda_device), tp.MODE_DETERMINISTIC)[0].tobytes() == exp.tobytes()
+        c.close()
+        c = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, fr.n_digits, rtc=True)
+        assert c.rtc_cache_hit
+        c.close()
+    finally:
+        tp.tpcclus_set_rtc_cache_dir(None)
