@@ -8,8 +8,10 @@ One "step" = one pass of the whole hot path (K1..K6 
 DESIGN.md) over one Pb-Pb-like time frame (BASELINE.json configs[4]) that is already
 resident in HBM.  Prints ONE JSON line (contract in the task statement): metric value in
 digits/s, e2e through tpcclus_run_host (host buffers, copies inside the timed region),
-per-kernel roofline of the dominant kernel from CUDA events recorded on the run's stream,
-and the CPU oracle timed on a bounded sample of the same frame.
+per-kernel roofline of the dominant kernel from CUDA events recorded on the run's stream (a
+separate pass after the timed region), median and best step, the two ratios NS asks for
+(t_det / t_fast, t_generic / t_RTC) and the CPU oracle timed on bounded samples of the same
+frame, on one core and sector-parallel on all cores.
 
 N > 1 (torchrun): the path shards by time frame -- every rank clusterizes its own frame
 (seed + rank), no data-path collective (PAPER.md 97: one process per GPU, whole time
@@ -39,10 +41,29 @@ def _log(msg):
 
 
 METRIC = "TPC clusterizer digits/s on Pb-Pb-like time frame"
-# ncu --set full, CFG[4] shuffled FAST generic, one launch each (profiles/r01g_ncu_full_summary.txt)
-NCU_TRAFFIC_BYTES = {"k_partition_coarse": 12766072000 + 6480317000, "k_partition_fine": 9069988000 + 6489780000,
-                     "k_cluster_tiles_fast": 6544338000 + 1902176000}
 UNIT = "digits/s"
+
+
+def _ncu_traffic(k, order, rtc, mode):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the newest committed `ncu --set full`
+    capture (profiles/*_traffic.json, written by paper_2511_17018_b200/ncu_summary.py).  A capture
+    describes the kernel text it was taken on and the headline workload only: for any other text or
+    workload the field is null rather than stale."""
+    import glob
+    import hashlib
+    if not (k == 4 and order == "shuffled" and not rtc and mode == "fast"):
+        return {}, None
+    with open(os.path.join(ROOT, "paper_2511_17018_b200", "csrc", "tpcclus_kernels.cuh"), "rb") as f:
+        sha = hashlib.sha256(f.read()).hexdigest()
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_traffic.json")), reverse=True):
+        try:
+            with open(path) as f:
+                t = json.load(f)
+        except Exception:
+            continue
+        if t.get("kernel_text_sha256") == sha:
+            return t.get("traffic_bytes", {}), os.path.relpath(path, ROOT)
+    return {}, None
 
 
 def _peaks():
@@ -103,6 +124,21 @@ def _oracle_sample(fr_digits_np, fr, n_sample_sectors):
     tm = {}
     cl, st, cnt = t1.clusterize(sub, n_sample_sectors, fr.n_rows, fr.n_time, fr.n_pads, capacity=max(len(sub) // 4, 1024), timing=tm)
     return len(sub), cnt, tm["seconds"]
+
+
+def _sector_digits(digits, s):
+    """Digits of sector s of a device-resident frame, as a host array (the oracle's input)."""
+    return digits[((digits >> 48) & 0xFF) == s].cpu().numpy().view(np.uint64)
+
+
+def _oracle_allcores(digits, fr, n_sectors):
+    """The same T1 routine, unchanged, run sector-parallel on all host cores."""
+    from oracle import t1
+    secs = list(range(n_sectors))
+    host = {s: _sector_digits(digits, s) for s in secs}
+    tm = {}
+    res = t1.clusterize_by_sector(lambda s: host[s], secs, fr.n_rows, fr.n_time, fr.n_pads, timing=tm)
+    return tm["digits"], int(sum(len(v) for v in res.values())), tm["seconds"], tm["cores"]
 
 
 def aggregate_over_ranks(ms_local, units_local, device, world):
@@ -170,6 +206,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-ratios", action="store_true", help="skip the t_det/t_fast and t_generic/t_rtc loops")
     ap.add_argument("--cpu-sectors", type=int, default=2)
     args = ap.parse_args()
     if args.impl == "reference":
@@ -200,15 +237,17 @@ def main():
     _log("frame generated: %d digits" % n)
     mode = tp.MODE_FAST if args.mode == "fast" else tp.MODE_DETERMINISTIC
     packed = args.mode == "packed"   # deterministic path, 16-byte records + row index
+    warmup = max(args.warmup, 3)
     c = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, n, rtc=args.rtc, device=local)
     # size the output from a first (untimed) run
     probe_cap = max(n // 3, 1024)
     clusters = torch.empty((probe_cap, 16 if packed else 32), dtype=torch.uint8, device=dev)
 
-    def step():
+    def step(cz=None, md=None):
+        cz = cz or c
         if packed:
-            return c.run_packed(digits, clusters=clusters)[2:]
-        return c.run(digits, mode, clusters=clusters)[1:]
+            return cz.run_packed(digits, clusters=clusters)[2:]
+        return cz.run(digits, mode if md is None else md, clusters=clusters)[1:]
     nt, stt = step()
     torch.cuda.synchronize(dev)
     n_clusters, status = int(nt.item()), int(stt.item())
@@ -219,26 +258,55 @@ def main():
             dist.barrier()
         torch.cuda.synchronize(dev)
 
-    for _ in range(max(args.warmup, 3)):
+    def timed_loop(cz, md, steps):
+        """`steps` runs back to back on the current stream: (total ms between the bracketing events,
+        [ms of every single step]).  Only launches inside: nothing synchronises before the end."""
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+        ev[0].record()
+        for i in range(steps):
+            step(cz, md)
+            ev[i + 1].record()
+        torch.cuda.synchronize(dev)
+        return ev[0].elapsed_time(ev[steps]), [ev[i].elapsed_time(ev[i + 1]) for i in range(steps)]
+
+    for _ in range(warmup):
         step()
-    c.set_timing(True)
-    per_kernel = {}
     barrier()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with ClockSampler(local) as clk:
-        e0.record()
-        for _ in range(args.steps):
-            step()
-            for nm, ms in c.last_timing():      # events recorded on the run's stream, inside the timed region
-                per_kernel.setdefault(nm, []).append(ms)
-        e1.record()
+        ms_total, per_step = timed_loop(c, None, args.steps)
         barrier()
-    ms_total = e0.elapsed_time(e1)
-    c.set_timing(False)
     _log("timed region done: %.3f ms/step" % (ms_total / args.steps))
     ms_max, tot_digits = aggregate_over_ranks(ms_total, n, dev, world)
     ms_step = ms_max / args.steps
     value = tot_digits / (ms_step * 1e-3)
+
+    # ---- per-kernel device times: a separate pass (the library's events synchronise per run) --------
+    c.set_timing(True)
+    per_kernel = {}
+    for _ in range(min(args.steps, 5)):
+        step()
+        for nm, ms in c.last_timing():
+            per_kernel.setdefault(nm, []).append(ms)
+    c.set_timing(False)
+
+    # ---- the two ratios NS asks for: deterministic mode vs fast (PAPER.md 28), generic vs RTC (PAPER.md 118) ---
+    ratios = {}
+    if world == 1 and not args.no_ratios and args.mode == "fast" and not args.rtc:
+        for _ in range(warmup):
+            step(c, tp.MODE_DETERMINISTIC)
+        ms_det = timed_loop(c, tp.MODE_DETERMINISTIC, args.steps)[0] / args.steps
+        r = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, n, rtc=True, device=local)
+        for _ in range(warmup):
+            step(r, tp.MODE_FAST)
+        torch.cuda.synchronize(dev)
+        ms_rtc = timed_loop(r, tp.MODE_FAST, args.steps)[0] / args.steps
+        ms_fast = ms_total / args.steps
+        ratios = {"t_det_over_t_fast": ms_det / ms_fast, "t_generic_over_t_rtc": ms_fast / ms_rtc,
+                  "ms_det": ms_det, "ms_rtc": ms_rtc, "rtc_build_ms": r.rtc_build_ms,
+                  "note": "same resident frame, %d steps each after %d warm-ups; RTC build time excluded" % (args.steps, warmup)}
+        r.close()
+        del r
+        _log("ratios done: det %.3f ms, rtc %.3f ms" % (ms_det, ms_rtc))
 
     # ---- e2e: host buffers through tpcclus_run_host, copies inside the timed region -----------
     e2e = None
@@ -264,7 +332,7 @@ def main():
         e2e = {"value": tot_digits / sec_max, "unit": UNIT, "h2d_bytes_per_step": 8 * n,
                "d2h_bytes_per_step": 32 * n_clusters + 16, "ms_per_step": sec_max * 1e3,
                "api": "tpcclus_run_host (pinned host buffers)"}
-        del h_clusters
+        del h_clusters, h_digits
         _log("e2e done")
 
     if rank != 0:
@@ -283,9 +351,7 @@ def main():
         "k_emit_ordered": 64 * n_clusters,                       # DET: ordered copy of the runs
         "k_emit_packed": 48 * n_clusters,                        # packed: 32 B in, 16 B out
     }
-    # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full`
-    # capture of this very workload (profiles/r01d_README.md); null for any other workload
-    traffic = NCU_TRAFFIC_BYTES if (k == 4 and args.order == "shuffled" and not args.rtc) else {}
+    traffic, traffic_src = _ncu_traffic(k, args.order, args.rtc, args.mode)
     step_sum = sum(avg.values())
     per_kernel_roof = {}
     for nm in avg:
@@ -295,32 +361,50 @@ def main():
                                    "frac": ach / peak, "traffic": traffic.get(nm), "alg_bytes": alg[nm],
                                    "kernel_ms": avg[nm], "share_of_step": avg[nm] / step_sum}
     dom = max(per_kernel_roof, key=lambda nm: avg[nm]) if per_kernel_roof else None
-    roof = dict(per_kernel_roof[dom], peak_source=peak_src) if dom else None
+    roof = dict(per_kernel_roof[dom], peak_source=peak_src, traffic_source=traffic_src) if dom else None
     b_alg = 8 * n + 32 * n_clusters
     method = {"b_alg_bytes": b_alg, "achieved_gbs": b_alg / (ms_step * 1e-3) / 1e9,
               "frac_of_peak": b_alg / (ms_step * 1e-3) / 1e9 / peak}
+    if traffic and all(nm in traffic for nm in ("k_partition_coarse", "k_partition_fine", "k_cluster_tiles_fast")):
+        dram = sum(traffic.values())
+        method.update({"dram_bytes_per_step_ncu": dram, "dram_gbs": dram / (ms_step * 1e-3) / 1e9,
+                       "dram_frac_of_peak": dram / (ms_step * 1e-3) / 1e9 / peak})
 
-    cpu = None
+    cpu = cpu_all = None
     if not args.no_cpu_baseline:
-        h = fr.digits_numpy() if e2e is None else h_digits.numpy().view(np.uint64)
         ns = min(args.cpu_sectors, fr.n_sectors)
-        _log("cpu baseline: filtering sample")
-        nd, cnt, sec = _oracle_sample(h, fr, ns)
-        _log("cpu baseline done")
+        _log("cpu baseline: single thread")
+        from oracle import t1
+        host = np.concatenate([_sector_digits(digits, s) for s in range(ns)])
+        nd, cnt, sec = _oracle_sample(host, fr, ns)
         cpu = {"value": nd / sec, "unit": UNIT, "cores": 1, "kind": "oracle",
                "sample": "sectors 0..%d of this frame (%d digits, %d clusters) in %.1f s, single thread" % (ns - 1, nd, cnt, sec)}
+        cores = len(os.sched_getaffinity(0))
+        na = min(fr.n_sectors, cores)
+        _log("cpu baseline: %d sectors on %d cores" % (na, cores))
+        nd, cnt, sec, used = _oracle_allcores(digits, fr, na)
+        cpu_all = {"value": nd / sec, "unit": UNIT, "cores": used, "cores_available": cores, "kind": "oracle, sector-parallel",
+                   "sample": "sectors 0..%d of this frame (%d digits, %d clusters) in %.1f s wall, one thread per sector" % (na - 1, nd, cnt, sec)}
+        _log("cpu baseline done")
 
+    in_gb = 8 * n / 1e9
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+        "warmup": warmup, "ms_per_step": ms_step, "ms_median": float(np.median(per_step)), "ms_best": float(min(per_step)),
+        "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "int32+f32", "data": "synthetic",
         "config": {"workload": fr.meta["name"], "order": args.order, "mode": args.mode, "rtc": bool(args.rtc),
                    "n_digits": n, "n_clusters": n_clusters, "occupancy": fr.meta["occupancy"],
-                   "checksum": "%016x" % fr.meta["checksum"], "l2": "inputs (%.1f GB) larger than L2" % (8 * n / 1e9)},
+                   "checksum": "%016x" % fr.meta["checksum"],
+                   "l2": ("inputs (%.1f GB) larger than L2, no flush needed" % in_gb) if in_gb > 0.3 else
+                         ("inputs (%.4f GB) FIT in L2 (126 MB): launch-latency-bound, not a bandwidth number" % in_gb)},
         "clocks": clk.summary(), "e2e": e2e, "gpu_launches": c.launches_per_run(mode) * args.steps,
         "roofline": roof, "rooflines": per_kernel_roof, "method_roofline": method,
-        "kernels_ms": avg, "cpu_baseline": cpu,
+        "kernels_ms": avg, "cpu_baseline": cpu, "cpu_baseline_allcores": cpu_all,
     }
+    out.update({k2: v for k2, v in ratios.items() if k2 in ("t_det_over_t_fast", "t_generic_over_t_rtc")})
+    if ratios:
+        out["ratios"] = ratios
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
