@@ -981,7 +981,7 @@ struct K6Smem {
   u16* tile; u32* tile32;
   u64* bar;        // [0] full (producer -> consumers), [1] empty (consumers -> producer)
   u64* base;
-  u32* pmask;      // [TT][9]  O1 peaks, bit = pad + 2 (so pad - 2 of a 5x5 ring is bit >= 0)
+  u32* pmask;      // [TT][9]  O1 peaks, bit = pad + HALO = the cell's index in its map row
   u32* rowmask;    // [TT][8]  O2 survivors, bit = pad
   u32* rowpre; u32* misc; u16* peaks;
 };
@@ -1175,6 +1175,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
    for (u32 mt = 0u; mt < ntl; ++mt) {   // the tiles of this stage
     const u32 tile = tile0 + mt, total = s.misc[9u + 2u * mt];
     const u32* const rec = s.rec + s.misc[8u + 2u * mt] * 4u;
+    u32* const s_rec_w = s.rec + s.misc[8u + 2u * mt] * 4u;   // (the peak test keeps its candidate list in the consumed records)
     const bool last = mt + 1u == ntl;   // the staged records are released after the last tile's use of them
     if (total == 0u) {   // block-uniform: nothing in this tile; the map stays zero
       __syncwarp();
@@ -1246,7 +1247,11 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       mbar_wait(&s.bar[0], ph); ph ^= 1u;
     }
     // a tile staged in one round (the usual case) keeps its records for the peak test below
+#ifdef TPC_X_DENSE
+    const bool sparse = total * 4u <= TPC_K6_CONSUMERS && MODE != TPC_MODE_DUMP_MAP;
+#else
     const bool sparse = total <= TPC_K6_CAPU && MODE != TPC_MODE_DUMP_MAP;
+#endif
     if (!sparse) { __syncwarp(); if (last && lane_id() == 0u) mbar_arrive(&s.bar[1]); }
     csync();   // C: the map is complete
 
@@ -1315,8 +1320,8 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
             const u32 e = max(max(pu[k] & 0xFFFFu, pu[k] >> 16), nu[k]);
             const u32 l = max(max(pd[k] & 0xFFFFu, pd[k] >> 16), nd[k]);
             if (cand[k] && q > e && q >= l) {
-              const u32 bit = 1u << ((pad + 2u) & 31u);
-              const u32 old = atomicOr(&s.pmask[tl * TPC_K6_PMW + ((pad + 2u) >> 5)], bit);
+              const u32 bit = 1u << ((pad + TPC_HALO) & 31u);
+              const u32 old = atomicOr(&s.pmask[tl * TPC_K6_PMW + ((pad + TPC_HALO) >> 5)], bit);
               if (!(old & bit) && tl >= TPC_HALO && tl < TPC_TS + TPC_HALO) {   // a halo-row peak is emitted by its own tile
                 const u32 i = atomicAdd(&s.misc[0], 1u);
                 s.peaks[i] = (u16)((tl << 8) | pad);
@@ -1326,45 +1331,136 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
         }
         return viol;
       };
-      auto peak_pass = [&](const bool check) -> u32 {
-        u32 viol = 0u;
-        if (nrec <= TPC_K6_CONSUMERS) {
-          const u32 r1[1] = {tid < nrec ? rec[tid] : 0u};
-          viol = peak_recs(TpcInt<1>(), r1, check);
-        } else
+      // Tiles with more than one record per thread: two stages with a compaction in between, so that
+      // the rows above and below are only fetched -- by full warps -- for the records that won their own
+      // row.  Stage 1 (all records, 16-byte pieces): q >= thr, q > left, q >= right, and the cell holds
+      // this very charge (a smaller duplicate of the cell is out).  Its survivors, one record in five, are
+      // written back IN PLACE: warp w reads records [1024 k + 128 w, + 128) in its k-th step and keeps its
+      // list in those same regions, in order -- it never holds more survivors than it has read, so the
+      // list only ever covers records the warp has consumed itself: no other buffer, no block barrier.
+      // Stage 2 walks the list, 64 entries per warp step; a peak sets its bit in pmask and the peaks of
+      // owned rows join the tile's list with one shared atomic per warp step.
+      auto peak_big = [&]() {
+        const u32 lane = lane_id(), lt = (1u << lane) - 1u, wbase = (tid >> 5) * 128u;
+        u32 nlist = 0u;   // warp-uniform
+        for (u32 u0 = (tid >> 5) * 32u; u0 < total; u0 += TPC_K6_CONSUMERS) {
+          const u32 u = u0 + lane;
+          uint4 v = make_uint4(0u, 0u, 0u, 0u);
+          if (u < total) v = r4[u];
+          const u32 rr[4] = {v.x, v.y, v.z, v.w};
+          u32 pm[4], nm[4];
+          bool cand[4];
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            const u32 q = (rr[k] >> 16) & 0x3FFu, tl = k6_row(rr[k], sl), pad = rr[k] & 0xFFu;
+            cand[k] = q >= thr && tl - 1u < TPC_TT - 2u;   // (q = 0 for run padding)
+            const u32 x = pad + TPC_HALO, h = x & 1u, sh = 16u - 16u * h;
+            const u32* w = s.tile32 + (cand[k] ? tl * nW + (x >> 1) - 1u + h : 0u);   // the others: word 0, a broadcast
+            pm[k] = __funnelshift_r(w[0], w[1], sh); nm[k] = (w[1] >> sh) & 0xFFFFu;
+          }
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            const u32 q = (rr[k] >> 16) & 0x3FFu;
+            const bool win = cand[k] && (pm[k] >> 16) == q && q > (pm[k] & 0xFFFFu) && q >= nm[k];
+            const u32 m = __ballot_sync(0xFFFFFFFFu, win);   // (the ballot needs every lane's piece: all loads of this step are done)
+            if (win) {
+              const u32 p = nlist + __popc(m & lt);
+              s_rec_w[(p >> 7) * (TPC_K6_CONSUMERS * 4u) + wbase + (p & 127u)] = rr[k];
+            }
+            nlist += __popc(m);
+          }
+        }
+        __syncwarp();
+        for (u32 p0 = 0u; p0 < nlist; p0 += 64u) {
+          u32 r2[2], pu[2], nu[2], pd[2], nd[2];
+#pragma unroll
+          for (int k = 0; k < 2; ++k) {
+            const u32 p = p0 + 32u * (u32)k + lane;
+            r2[k] = p < nlist ? s_rec_w[(p >> 7) * (TPC_K6_CONSUMERS * 4u) + wbase + (p & 127u)] : 0u;
+          }
+#pragma unroll
+          for (int k = 0; k < 2; ++k) {
+            const u32 tl = k6_row(r2[k], sl), pad = r2[k] & 0xFFu;
+            const u32 x = pad + TPC_HALO, h = x & 1u, sh = 16u - 16u * h;
+            const u32* w = s.tile32 + (r2[k] != 0u ? (tl - 1u) * nW + (x >> 1) - 1u + h : 0u);
+            pu[k] = __funnelshift_r(w[0], w[1], sh); nu[k] = (w[1] >> sh) & 0xFFFFu;
+            w += 2u * nW;
+            pd[k] = __funnelshift_r(w[0], w[1], sh); nd[k] = (w[1] >> sh) & 0xFFFFu;
+          }
+#pragma unroll
+          for (int k = 0; k < 2; ++k) {
+            const u32 q = (r2[k] >> 16) & 0x3FFu, tl = k6_row(r2[k], sl), pad = r2[k] & 0xFFu;
+            const u32 e = max(max(pu[k] & 0xFFFFu, pu[k] >> 16), nu[k]);
+            const u32 l = max(max(pd[k] & 0xFFFFu, pd[k] >> 16), nd[k]);
+            bool own = false;
+            if (r2[k] != 0u && q > e && q >= l) {
+              const u32 bit = 1u << ((pad + TPC_HALO) & 31u);
+              const u32 old = atomicOr(&s.pmask[tl * TPC_K6_PMW + ((pad + TPC_HALO) >> 5)], bit);
+              own = !(old & bit) && tl >= TPC_HALO && tl < TPC_TS + TPC_HALO;   // a halo-row peak is emitted by its own tile
+            }
+            const u32 m = __ballot_sync(0xFFFFFFFFu, own);
+            if (m) {
+              u32 base = 0u;
+              if (lane == 0u) base = atomicAdd(&s.misc[0], (u32)__popc(m));
+              base = __shfl_sync(0xFFFFFFFFu, base, 0);
+              if (own) s.peaks[base + __popc(m & lt)] = (u16)((tl << 8) | pad);
+            }
+          }
+        }
+      };
+      // DET: have the plain stores of the scatter left a smaller duplicate on top of a cell (Q5)?
+      auto settle = [&]() {   // raise every cell to the maximum of its records; ends behind a barrier
+        for (;;) {
+          u32 any = 0u;
           for (u32 u = tid; u < total; u += TPC_K6_CONSUMERS) {
             const uint4 v = r4[u];
             const u32 rr[4] = {v.x, v.y, v.z, v.w};
-            viol |= peak_recs(TpcInt<4>(), rr, check);
-          }
-        return viol;
-      };
-      if (MODE == TPC_MODE_FAST) {
-        peak_pass(false);
-      } else {
-        d_done = true;
-        if (csync_or(peak_pass(true))) {   // rare: duplicates in this tile.  Settle the maxima, forget the peaks, test again.
-          for (;;) {
-            u32 any = 0u;
-            for (u32 u = tid; u < total; u += TPC_K6_CONSUMERS) {
-              const uint4 v = r4[u];
-              const u32 rr[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
-              for (int k = 0; k < 4; ++k) {
-                const u32 tl = k6_row(rr[k], sl);
-                if (rr[k] != 0u && tl < TPC_TT) {
-                  const u32 cell = tl * pitch + (rr[k] & 0xFFu) + TPC_HALO;
-                  const u16 q = (u16)((rr[k] >> 16) & 0x3FFu);
-                  if (s.tile[cell] < q) { s.tile[cell] = q; any = 1u; }
-                }
+            for (int k = 0; k < 4; ++k) {
+              const u32 tl = k6_row(rr[k], sl);
+              if (rr[k] != 0u && tl < TPC_TT) {
+                const u32 cell = tl * pitch + (rr[k] & 0xFFu) + TPC_HALO;
+                const u16 q = (u16)((rr[k] >> 16) & 0x3FFu);
+                if (s.tile[cell] < q) { s.tile[cell] = q; any = 1u; }
               }
             }
-            if (!csync_or(any)) break;
           }
+          if (!csync_or(any)) break;
+        }
+      };
+      if (nrec > TPC_K6_CONSUMERS) {
+        if (MODE != TPC_MODE_FAST) {
+          // the in-place list would destroy the records the settling needs: verify first (one more pass
+          // over the records and one more barrier per tile than FAST -- the price of Q5 in this mode)
+          u32 viol = 0u;
+          for (u32 u = tid; u < total; u += TPC_K6_CONSUMERS) {
+            const uint4 v = r4[u];
+            const u32 rr[4] = {v.x, v.y, v.z, v.w};
+            u32 c4[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+              const u32 tl = k6_row(rr[k], sl);
+              c4[k] = s.tile[(tl < TPC_TT ? tl * pitch : 0u) + (rr[k] & 0xFFu) + TPC_HALO];
+            }
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+              if (rr[k] != 0u && k6_row(rr[k], sl) < TPC_TT && c4[k] < ((rr[k] >> 16) & 0x3FFu)) viol = 1u;
+          }
+          if (csync_or(viol)) settle();   // rare: duplicates in this tile
+        }
+        peak_big();
+      } else if (MODE == TPC_MODE_FAST) {
+        const u32 r1[1] = {tid < nrec ? rec[tid] : 0u};
+        peak_recs(TpcInt<1>(), r1, false);
+      } else {
+        d_done = true;
+        const u32 r1[1] = {tid < nrec ? rec[tid] : 0u};
+        if (csync_or(peak_recs(TpcInt<1>(), r1, true))) {   // rare: duplicates in this tile.  Settle the maxima, forget the peaks, test again.
+          settle();
           for (u32 i = tid; i < TPC_TT * TPC_K6_PMW; i += TPC_K6_CONSUMERS) s.pmask[i] = 0u;
           if (tid == 0) s.misc[0] = 0u;
           csync();
-          peak_pass(false);
+          peak_recs(TpcInt<1>(), r1, false);
           csync();
         }
       }
@@ -1372,17 +1468,20 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       if (last && lane_id() == 0u) mbar_arrive(&s.bar[1]);   // this warp is done with the staged records
     } else
     // ---- O1: 3x3 peaks, dense scan on packed u16x2 words ----------------------------------
-    // A thread owns a group of 4 word columns (8 pads, one 128-bit load per row) of a strip of
+    // A thread owns a group of 4 word columns (8 cells, one 128-bit load per row) of a strip of
     // rows and walks down the time axis with a rolling 3-row window.  For the word C of row r:
     // L / R = the same two cells shifted one pad left / right, H(r) = max(L, C, R).  A cell is a
     // peak iff q > the 4 neighbours earlier in (t,p) order and q >= the 4 later ones (O1), i.e.
-    // q >= max(max(H(r-1), L(r)) + 1, H(r+1), R(r)); an empty cell never passes (the bound is
-    // >= 1) and thr_peak joins the same max.  Rows 1..TT-2 are tested: the owned rows plus the
-    // halo rows whose peaks O2 needs.  Guard cells are 0 and can never be flagged.  A peak sets
-    // its bit in pmask; the peaks of owned rows also go into the list the later phases walk.
+    // q > M1 = max(H(r-1), L(r)) and q >= M2 = max(H(r+1), R(r), thr_peak); an empty cell never
+    // passes (M2 >= 1).  Charges have 10 bits, so each 16-bit half carries a guard bit: with
+    // G = 0x80008000, (C | G) - M1 - 0x00010001 and (C | G) - M2 keep their guard bits exactly where
+    // the comparison holds, with plain 32-bit adds and no borrow between the halves.  The 8 result
+    // bits of a row are one byte of pmask (bit = cell index): a byte store, no atomics.  Rows
+    // 1..TT-2 are tested: the owned rows plus the halo rows whose peaks O2 needs.  Guard cells are 0
+    // and can never be flagged.  The peaks of owned rows are listed afterwards, from pmask.
     {
       const u32 nW = pitch >> 1;
-      const u32 ng = (((npads + 2u) >> 1) >> 2) + 1u;    // word groups covering cells 0..npads+2
+      const u32 ng = ((npads + TPC_HALO - 1u) >> 3) + 1u;   // 8-cell groups up to the last real pad's cell (npads + 2)
       const u32 strips = TPC_K6_CONSUMERS / ng;          // >= 1: npads <= 256 -> ng <= 33
       const u32 rp = (TPC_TT - 2u + strips - 1u) / strips;
       const u32 si = tid / ng, g = tid - si * ng;
@@ -1403,28 +1502,18 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
 #pragma unroll
           for (int k = 0; k < 4; ++k) w.H[k] = vmax2(vmax2(w.S[k], w.C[k]), w.S[k + 1]);
         };
+        u8* const pmb = (u8*)s.pmask + g;
         auto test = [&](const Row& up, const Row& mid, const Row& dn, u32 r) {
-          u32 X[4], any = 0u;
+          u32 byte = 0u;
 #pragma unroll
           for (int k = 0; k < 4; ++k) {
-            const u32 M = vmax2(vmax2(vmax2(up.H[k], mid.S[k]) + 0x00010001u, dn.H[k]), vmax2(mid.S[k + 1], thr2));
-            X[k] = vmax2(mid.C[k], M) ^ mid.C[k];        // a zero half = that cell beats its 8 neighbours
-            any |= (X[k] - 0x00010001u) & ~X[k] & 0x80008000u;   // pre-filter: some half may be zero
+            const u32 M1 = vmax2(up.H[k], mid.S[k]);
+            const u32 M2 = vmax2(vmax2(dn.H[k], mid.S[k + 1]), thr2);
+            const u32 cg = mid.C[k] | 0x80008000u;
+            const u32 x = ((cg - M1 - 0x00010001u) & (cg - M2) & 0x80008000u) >> 15;   // bit 0: the low cell is a peak, bit 16: the high cell
+            byte |= ((x | (x >> 15)) & 3u) << (2 * k);
           }
-          if (any) {
-#pragma unroll
-            for (int k = 0; k < 4; ++k)
-#pragma unroll
-              for (int h = 0; h < 2; ++h)
-                if (((X[k] >> (16 * h)) & 0xFFFFu) == 0u) {
-                  const u32 pad = 8u * g + 2u * (u32)k + (u32)h - TPC_HALO;
-                  atomicOr(&s.pmask[r * TPC_K6_PMW + ((pad + 2u) >> 5)], 1u << ((pad + 2u) & 31u));
-                  if (r >= TPC_HALO && r < TPC_TS + TPC_HALO) {   // a halo-row peak is emitted by its own tile
-                    const u32 i = atomicAdd(&s.misc[0], 1u);
-                    s.peaks[i] = (u16)((r << 8) | pad);
-                  }
-                }
-          }
+          pmb[r * (TPC_K6_PMW * 4u)] = (u8)byte;
         };
         const u32* q = s.tile32 + (r0 - 1u) * nW + 4u * g;
         Row ra, rb, rc;
@@ -1434,6 +1523,28 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
           load(q, rc); test(ra, rb, rc, r); if (++r >= r1) break; q += nW;
           load(q, ra); test(rb, rc, ra, r); if (++r >= r1) break; q += nW;
           load(q, rb); test(rc, ra, rb, r); if (++r >= r1) break; q += nW;
+        }
+      }
+      csync();   // D': pmask complete
+      // the peaks of the owned rows, listed from pmask: a warp per 32 mask words, one shared atomic per warp step
+      const u32 nwp = ((npads + TPC_HALO - 1u) >> 5) + 1u;   // mask words that can hold a peak
+      const u32 inv = 65536u / nwp + 1u;                      // i / nwp for i < 2^11 (exact: nwp <= 9)
+      const u32 lane = lane_id(), lt = (1u << lane) - 1u;
+      for (u32 i0 = (tid >> 5) * 32u; i0 < TPC_TS * nwp; i0 += TPC_K6_CONSUMERS) {
+        const u32 i = i0 + lane;
+        const u32 rw = (i * inv) >> 16, wd = i - rw * nwp;
+        u32 w = i < TPC_TS * nwp ? s.pmask[(rw + TPC_HALO) * TPC_K6_PMW + wd] : 0u;
+        for (;;) {
+          const u32 m = __ballot_sync(0xFFFFFFFFu, w != 0u);
+          if (!m) break;
+          u32 base = 0u;
+          if (lane == 0u) base = atomicAdd(&s.misc[0], (u32)__popc(m));
+          base = __shfl_sync(0xFFFFFFFFu, base, 0);
+          if (w != 0u) {
+            const u32 bpos = (u32)__ffs((int)w) - 1u;
+            w &= w - 1u;
+            s.peaks[base + __popc(m & lt)] = (u16)(((rw + TPC_HALO) << 8) | (wd * 32u + bpos - TPC_HALO));
+          }
         }
       }
     }
@@ -1446,7 +1557,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       const u32 e = s.peaks[i];
       const u32 tl = e >> 8, pad = e & 0xFFu;
       // the 5x5 ring of peak bits around (tl, pad): 5 bits per row, bit k <-> dp = k - 2
-      const u32 w0 = pad >> 5, sh = pad & 31u;   // bit (pad + 2) - 2 = pad
+      const u32 w0 = (pad + TPC_HALO - 2u) >> 5, sh = (pad + TPC_HALO - 2u) & 31u;   // bit of (pad - 2) = cell index pad + HALO - 2
       u32 ring = 0u;
 #pragma unroll
       for (int dt = -2; dt <= 2; ++dt) {
@@ -1636,7 +1747,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       if (my_r != 0u) {
         const u32 tl = k6_row(my_r, sl), pad = my_r & 0xFFu;
         s.tile[tl * pitch + pad + TPC_HALO] = 0;
-        s.pmask[tl * TPC_K6_PMW + ((pad + 2u) >> 5)] = 0u;
+        s.pmask[tl * TPC_K6_PMW + ((pad + TPC_HALO) >> 5)] = 0u;
         s.rowmask[tl * 8u + (pad >> 5)] = 0u;
       }
       if (tid == 0) s.misc[0] = 0u;
