@@ -118,7 +118,47 @@ def cluster_of(m, T, P, c, s, r, cog_gated=False):
     )
 
 
-def clusterize(digits, n_sectors, n_rows, n_time, n_pads, thr_peak=6, noise_eps=4, cog_gated=False):
+def cheb(a, b):
+    return max(abs(a[0] - b[0]), abs(a[1] - b[1]))
+
+
+def cluster_shared_of(m, T, P, c, sv, s, r):
+    """O3 + O4 in reading Q10'' (R8): a cell of c's window that also lies in the window of
+    partners of c -- survivors at Chebyshev distance exactly 2 from c -- is split by the integer weights
+    w_p(x) = (q_p >> 2 cheb(p, x)) + 1; c takes floor(q_x w_c / sum of the weights).  Peak cells are
+    never split: c keeps its own in full and takes nothing of a partner's."""
+    partners = [p for p in sv if cheb(p, c) == 2]
+    t_c, p_c = c
+    Q = Sp = St = Spp = Stt = 0
+    for dt, dp in product(range(-2, 3), repeat=2):
+        x = (t_c + dt, p_c + dp)
+        q = m.get(x, 0) if (0 <= x[0] < T and 0 <= x[1] < P) else 0
+        if q == 0:
+            continue
+        if x == c:
+            share = q                      # the peak cell is never split
+        elif x in partners:
+            share = 0                      # nor is a partner's
+        else:
+            weights = {p: (m[p] >> (2 * cheb(p, x))) + 1 for p in [c] + partners if cheb(p, x) <= 2}
+            share = (q * weights[c]) // sum(weights.values())
+        Q += share
+        Sp += share * dp
+        St += share * dt
+        Spp += share * dp * dp
+        Stt += share * dt * dt
+    Vp = Q * Spp - Sp * Sp
+    Vt = Q * Stt - St * St
+    fQ = F(Q)
+    flags = (1 if (p_c < 2 or p_c + 2 >= P) else 0) | (2 if (t_c < 2 or t_c + 2 >= T) else 0) | (4 if m[c] == 1023 else 0)
+    return dict(
+        pad_mean=F(F(p_c) + F(Sp) / fQ), time_mean=F(F(t_c) + F(St) / fQ), sigma_pad=F(np.sqrt(F(Vp)) / fQ),
+        sigma_time=F(np.sqrt(F(Vt)) / fQ), q_tot=Q, q_max=m[c], time_peak=t_c, pad_peak=p_c, row=r, sector=s,
+        flags=flags, reserved=0, sums=(Q, Sp, St, Spp, Stt, Vp, Vt),
+    )
+
+
+def clusterize(digits, n_sectors, n_rows, n_time, n_pads, thr_peak=6, noise_eps=4, cog_gated=False, cog_shared=False):
     """O0..O5.  Returns (list of cluster dicts in (sector,row,time,pad) order, bad_flag)."""
     maps, bad = build_maps(digits, n_sectors, n_rows, n_time, n_pads)
     out = []
@@ -128,7 +168,7 @@ def clusterize(digits, n_sectors, n_rows, n_time, n_pads, thr_peak=6, noise_eps=
         pk, rank = peaks_of(m, T, P, thr_peak)
         sv = survivors_of(m, pk, rank, noise_eps)
         for c in sorted(sv):  # (time, pad) ascending == O5 within a row
-            out.append(cluster_of(m, T, P, c, s, r, cog_gated))
+            out.append(cluster_shared_of(m, T, P, c, sv, s, r) if cog_shared else cluster_of(m, T, P, c, s, r, cog_gated))
     return out, bad
 
 

@@ -79,7 +79,7 @@ def lib():
 
 
 def clusterize(digits, n_sectors, n_rows, n_time, n_pads, thr_peak=6, noise_eps=4,
-               capacity=None, return_map=False, timing=None, cog_gated=False):
+               capacity=None, return_map=False, timing=None, cog_gated=False, cog_shared=False):
     """Run O0..O5.  ``digits``: array of dtype DIGIT (or uint64 / (n,8) uint8 view).
 
     Returns ``(clusters[DIGIT->CLUSTER array], status)`` (+ the O0 map if
@@ -103,7 +103,7 @@ def clusterize(digits, n_sectors, n_rows, n_time, n_pads, thr_peak=6, noise_eps=
     cnt = lib().oracle_clusterize_ex(
         n_sectors, n_rows, n_time, pads.ctypes.data, thr_peak, noise_eps,
         d.ctypes.data, n, out.ctypes.data, capacity, ctypes.byref(status),
-        dbg.ctypes.data if dbg is not None else None, 1 if cog_gated else 0,
+        dbg.ctypes.data if dbg is not None else None, 2 if cog_shared else (1 if cog_gated else 0),
     )
     if timing is not None:
         timing["seconds"] = time.perf_counter() - t0
@@ -140,7 +140,7 @@ def make_digits(rows):
 
 
 def clusterize_by_sector(digits_of, sectors, n_rows, n_time, n_pads, thr_peak=6, noise_eps=4, threads=None,
-                         timing=None, cog_gated=False):
+                         timing=None, cog_gated=False, cog_shared=False):
     """T1 run sector-parallel ("the same T1 code run sector-parallel ... on all host
     cores"): sectors never interact (O0, invariant I8 -- pinned in tests/test_oracle_multisector.py),
     so each sector is clusterized alone by the unchanged single-threaded C routine as a 1-sector
@@ -168,7 +168,7 @@ def clusterize_by_sector(digits_of, sectors, n_rows, n_time, n_pads, thr_peak=6,
     def one(s):
         d = inputs[s]
         cl, st, cnt = clusterize(d, 1, n_rows, n_time, n_pads, thr_peak, noise_eps,
-                                 capacity=max(len(d) // 4, 1024), cog_gated=cog_gated)
+                                 capacity=max(len(d) // 4, 1024), cog_gated=cog_gated, cog_shared=cog_shared)
         if cnt != len(cl) or st != 0:
             raise RuntimeError("oracle: sector %d: status %d, %d clusters for capacity %d" % (s, st, cnt, len(cl)))
         cl["sector"] = s

@@ -181,6 +181,73 @@ static void make_cluster(const row_map* m, uint32_t s, uint32_t r, int64_t t, in
   c->reserved = 0;
 }
 
+/* O3 + O4 in reading Q10'' (second half; R8): charge sharing between
+ * clusters whose windows overlap.  sv = the survivor set of O2 for this row map.  The PARTNERS of a
+ * survivor c are the survivors c' at Chebyshev distance exactly 2 (no two peaks are closer), i.e.
+ * those whose peak cell lies on the outer ring of c's window.  A cell x of c's window that also lies
+ * in the window of partners c'_1..c'_k is split with integer weights
+ *     w_p(x) = (q_p >> (2 * cheb(p, x))) + 1            (peak charge, quartered per bin of distance)
+ *     share_c(x) = floor(q_x * w_c(x) / (w_c(x) + sum_i w_c'_i(x)))
+ * and enters the sums of O3 with that share instead of q_x.  A cell no partner reaches keeps its
+ * full charge (the quotient is q_x * w / w).  A peak cell is never split: c keeps q_c in full (so
+ * Q >= q_c >= 1) and takes nothing of a partner's peak cell.  Everything stays an exact integer. */
+static int cheb(int64_t t1, int64_t p1, int64_t t2, int64_t p2) {
+  return imax(iabs((int)(t1 - t2)), iabs((int)(p1 - p2)));
+}
+
+static void make_cluster_shared(const row_map* m, const uint8_t* sv, uint32_t s, uint32_t r, int64_t t,
+                                int64_t p, orc_cluster* c) {
+  uint32_t Q = 0, Spp = 0, Stt = 0;
+  int32_t Sp = 0, St = 0;
+  uint32_t qc = cell(m, t, p);
+  for (int dt = -2; dt <= 2; ++dt)
+    for (int dp = -2; dp <= 2; ++dp) {
+      int64_t tx = t + dt, px = p + dp;
+      uint32_t q = cell(m, tx, px); /* Q8: clipped window */
+      if (q == 0) continue;
+      uint32_t wc = (qc >> (2 * cheb(t, p, tx, px))) + 1, den = wc;
+      int partner_peak = 0;
+      for (int et = -2; et <= 2; ++et)       /* the partners: survivors on the outer ring of c */
+        for (int ep = -2; ep <= 2; ++ep) {
+          if (imax(iabs(et), iabs(ep)) != 2) continue;
+          int64_t t2 = t + et, p2 = p + ep;
+          if (t2 < 0 || p2 < 0 || t2 >= (int64_t)m->T || p2 >= (int64_t)m->P) continue;
+          if (!sv[(size_t)t2 * m->P + (size_t)p2]) continue;
+          int d2 = cheb(t2, p2, tx, px);
+          if (d2 > 2) continue;                /* x is outside that partner's window */
+          if (d2 == 0) partner_peak = 1;       /* x is that partner's own peak cell */
+          den += (cell(m, t2, p2) >> (2 * d2)) + 1;
+        }
+      uint32_t share = q * wc / den;
+      if (dt == 0 && dp == 0) share = q;       /* the peak cell is c's alone ... */
+      if (partner_peak) share = 0;             /* ... and a partner's peak cell is the partner's */
+      Q += share;
+      Sp += (int32_t)share * dp;
+      St += (int32_t)share * dt;
+      Spp += share * (uint32_t)(dp * dp);
+      Stt += share * (uint32_t)(dt * dt);
+    }
+  float f[4];
+  oracle_finalize(Q, Sp, St, Spp, Stt, (uint32_t)p, (uint32_t)t, f);
+  memset(c, 0, sizeof *c);
+  c->pad_mean = f[0];
+  c->time_mean = f[1];
+  c->sigma_pad = f[2];
+  c->sigma_time = f[3];
+  c->q_tot = Q;
+  c->q_max = (uint16_t)qc;
+  c->time_peak = (uint16_t)t;
+  c->pad_peak = (uint8_t)p;
+  c->row = (uint8_t)r;
+  c->sector = (uint8_t)s;
+  uint8_t fl = 0;
+  if (p < 2 || p + 2 >= (int64_t)m->P) fl |= ORC_FLAG_EDGE_PAD;
+  if (t < 2 || t + 2 >= (int64_t)m->T) fl |= ORC_FLAG_EDGE_TIME;
+  if (c->q_max == 1023) fl |= ORC_FLAG_SATURATED;
+  c->flags = fl;
+  c->reserved = 0;
+}
+
 /*
  * Whole path O0..O5.  Returns the true number of clusters (also when it
  * exceeds `capacity`; then ORC_STATUS_OVERFLOW is set and only the first
@@ -223,8 +290,9 @@ int64_t oracle_clusterize_ex(uint32_t n_sectors, uint32_t n_rows, uint32_t n_tim
   uint64_t* fill = (uint64_t*)calloc((size_t)n_sectors + 1, sizeof(uint64_t));
   uint16_t* q = (uint16_t*)malloc((sector_cells ? sector_cells : 1) * sizeof(uint16_t));
   uint8_t* pk = (uint8_t*)malloc(sector_cells ? sector_cells : 1);
-  if (!first || !order || !fill || !q || !pk) {
-    free(row_off); free(first); free(order); free(fill); free(q); free(pk);
+  uint8_t* sv = (uint8_t*)malloc(sector_cells ? sector_cells : 1);
+  if (!first || !order || !fill || !q || !pk || !sv) {
+    free(row_off); free(first); free(order); free(fill); free(q); free(pk); free(sv);
     return -1;
   }
   for (uint64_t i = 0; i < n_digits; ++i) {
@@ -261,18 +329,24 @@ int64_t oracle_clusterize_ex(uint32_t n_sectors, uint32_t n_rows, uint32_t n_tim
       for (uint32_t t = 0; t < n_time; ++t)
         for (uint32_t p = 0; p < m.P; ++p)
           pkr[(size_t)t * m.P + p] = (uint8_t)is_peak(&m, t, p, thr_peak);
-      /* O2 + O3 + O4 + O5: survivors in (time,pad) order */
+      /* O2: survivor set (against the un-updated peak set) */
+      uint8_t* svr = sv + row_off[r];
+      for (uint32_t t = 0; t < n_time; ++t)
+        for (uint32_t p = 0; p < m.P; ++p)
+          svr[(size_t)t * m.P + p] = (uint8_t)(pkr[(size_t)t * m.P + p] && !is_suppressed(&m, pkr, t, p, noise_eps));
+      /* O3 + O4 + O5: survivors in (time,pad) order; cog_gated: 0 = Q10, 1 = Q10', 2 = Q10'' */
       for (uint32_t t = 0; t < n_time; ++t)
         for (uint32_t p = 0; p < m.P; ++p) {
-          if (!pkr[(size_t)t * m.P + p]) continue;
-          if (is_suppressed(&m, pkr, t, p, noise_eps)) continue;
-          if (n_out < capacity) make_cluster(&m, s, r, t, p, &out[n_out], cog_gated);
-          else st |= ORC_STATUS_OVERFLOW;
+          if (!svr[(size_t)t * m.P + p]) continue;
+          if (n_out < capacity) {
+            if (cog_gated == 2) make_cluster_shared(&m, svr, s, r, t, p, &out[n_out]);
+            else make_cluster(&m, s, r, t, p, &out[n_out], cog_gated);
+          } else st |= ORC_STATUS_OVERFLOW;
           ++n_out;
         }
     }
   }
-  free(row_off); free(first); free(order); free(fill); free(q); free(pk);
+  free(row_off); free(first); free(order); free(fill); free(q); free(pk); free(sv);
   if (status) *status = st;
   return (int64_t)n_out;
 }

@@ -41,10 +41,14 @@ typedef unsigned short u16;
 typedef unsigned char u8;
 
 // ---- fixed design constants ------------------------------------
+#ifndef TPC_TS
 #define TPC_TS 128u            // time bins a tile owns
+#endif
 #define TPC_HALO 3u            // halo: peaks at distance 2 need charges at distance 3 (O2)
 #define TPC_TT (TPC_TS + 2u * TPC_HALO)   // rows of a tile in shared memory
+#ifndef TPC_TC
 #define TPC_TC 16256u          // time bins per coarse time-chunk: 127*128, +6 halo < 2^14
+#endif
 #define TPC_STAGE 8u           // records (32 B) staged per coarse bin in K1
 #define TPC_CHUNK 64u          // records per pool chunk (256 B)
 #define TPC_CPB 256u           // chunks per K5 batch (<= 16384 records)
@@ -78,7 +82,9 @@ struct TpcParams {
 __host__ __device__ inline u32 tpc_k1_smem_bytes(u32 nb) {
   return (nb * (TPC_STAGE + 2u) + 4u * TPC_K1_SPILL + 8u) * 4u + TPC_K1_FQ * 2u;
 }
+#ifndef TPC_NSLMAX
 #define TPC_NSLMAX 128u   // >= slabs per bin: TPC_TC / TPC_TS = 127
+#endif
 #define TPC_NKEY (2u * TPC_NSLMAX + 32u)   // sort keys: 2 per slab + A of the slab after the last; multiple of 32
 #define TPC_K5_BUF (TPC_CPB * TPC_CHUNK + 4u * TPC_NSLMAX + 8u)   // u32 words: the records of a batch + alignment gaps + end padding
 __host__ __device__ inline u32 tpc_k5_smem_bytes() { return (TPC_K5_BUF + 2u * TPC_NKEY + 8u) * 4u; }
@@ -86,9 +92,13 @@ __host__ __device__ inline u32 tpc_k5_smem_bytes() { return (TPC_K5_BUF + 2u * T
 #define TPC_MODE_DET 1        // chained scan inside K6 (fallback: any number of clusters)
 #define TPC_MODE_DET_TEMP 2   // runs into the temporary buffer, K7-K9 order them (the usual path)
 #define TPC_MODE_DUMP_MAP 3
+#ifndef TPC_K6_CONSUMERS
 #define TPC_K6_CONSUMERS 256u                   // threads that compute
+#endif
 #define TPC_K6_THREADS (TPC_K6_CONSUMERS + 32u)  // + the producer warp
+#ifndef TPC_K6_CAP
 #define TPC_K6_CAP 4096u                         // records staged per round (16 KB)
+#endif
 #define TPC_K6_CAPU (TPC_K6_CAP / 4u)            // ... in 16-byte units
 #ifndef TPC_K6_CTAS
 #define TPC_K6_CTAS 3                            // resident CTAs per SM (shared memory and registers)
@@ -1033,7 +1043,10 @@ __device__ __forceinline__ u64 k6_chain(u64* state, u32 tile, u32 count) {
 
 // Tile row of a K5 record for the tile of slab `sl`: own slab -> m, next slab -> TS + m (its first
 // 6 rows close this tile); anything >= TPC_TT is a foreign record (up to 3 of them follow a run).
-__device__ __forceinline__ u32 k6_row(u32 r, u32 sl) { return ((r >> 8) & 0xFFu) ^ ((sl & 1u) << 7); }
+__device__ __forceinline__ u32 k6_row(u32 r, u32 sl) {
+  const u32 x = ((r >> 8) & 0xFFu) ^ ((sl & 1u) << 7);   // bit 7: the record belongs to the next slab
+  return TPC_TS == 128u ? x : (x & 127u) + (x >> 7) * TPC_TS;
+}
 
 // Producer warp: stages round `round` of a tile -- the 16-byte units [round*CAPU, (round+1)*CAPU)
 // of the concatenation of the tile's runs (one run per K5 batch of the bin, 16-byte aligned,
@@ -1552,9 +1565,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
     const u32 npk = s.misc[0];
 
     // ---- O2: suppression of the owned peaks against the un-updated peak set -----------------
-    bool survived = false;
-    for (u32 i = tid; i < npk; i += TPC_K6_CONSUMERS) {
-      const u32 e = s.peaks[i];
+    auto suppressed = [&](const u32 e) -> bool {
       const u32 tl = e >> 8, pad = e & 0xFFu;
       // the 5x5 ring of peak bits around (tl, pad): 5 bits per row, bit k <-> dp = k - 2
       const u32 w0 = (pad + TPC_HALO - 2u) >> 5, sh = (pad + TPC_HALO - 2u) & 31u;   // bit of (pad - 2) = cell index pad + HALO - 2
@@ -1593,7 +1604,111 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
               }
           }
       }
-      if (!dead) { atomicOr(&s.rowmask[tl * 8u + (pad >> 5)], 1u << (pad & 31u)); survived = true; }
+      return dead;
+    };
+    uint4 o0 = make_uint4(0u, 0u, 0u, 0u), o1 = make_uint4(0u, 0u, 0u, 0u);
+    // O3 + O4 for one surviving peak
+    auto cog_sums = [&](u32 e, uint4& c0, uint4& c1) {
+      const u32 tl = e >> 8, pad = e & 0xFFu;
+      const u16* c = s.tile + tl * pitch + pad + TPC_HALO;
+      // exact integer sums (Q12): per-row partial sums first, so the 25 loads and the adds of
+      // different rows are independent (short dependency chains; any order gives the same bits)
+      u32 Q = 0u, Spp = 0u, Stt = 0u;
+      int Sp = 0, St = 0;
+      if (!GATED) {   // Q10: every in-range cell, weight 1 (the reading is a kernel variant: no run-time test)
+#pragma unroll
+        for (int dt = -2; dt <= 2; ++dt) {
+          const u16* cr = c + dt * (int)pitch;
+          const u32 a = cr[-2], b = cr[-1], m = cr[0], d = cr[1], e2 = cr[2];
+          const u32 rq = (a + b) + (m + d) + e2;
+          const int rsp = (int)(2u * e2 + d) - (int)(2u * a + b);
+          const u32 rspp = 4u * (a + e2) + (b + d);
+          Q += rq; Sp += rsp; Spp += rspp;
+          St += (int)rq * dt; Stt += rq * (u32)(dt * dt);
+        }
+      } else {                 // Q10': an outer-ring cell counts only if the inner cell towards the peak holds charge
+        u32 w5[5][5];
+#pragma unroll
+        for (int dt = -2; dt <= 2; ++dt)
+#pragma unroll
+          for (int dp = -2; dp <= 2; ++dp) w5[dt + 2][dp + 2] = c[dt * (int)pitch + dp];
+#pragma unroll
+        for (int dt = -2; dt <= 2; ++dt)
+#pragma unroll
+          for (int dp = -2; dp <= 2; ++dp)
+            if (dt == -2 || dt == 2 || dp == -2 || dp == 2) {
+              const int it = dt < -1 ? -1 : (dt > 1 ? 1 : dt), ip = dp < -1 ? -1 : (dp > 1 ? 1 : dp);
+              if (w5[it + 2][ip + 2] == 0u) w5[dt + 2][dp + 2] = 0u;
+            }
+#pragma unroll
+        for (int dt = -2; dt <= 2; ++dt) {
+          const u32 a = w5[dt + 2][0], b = w5[dt + 2][1], m = w5[dt + 2][2], d = w5[dt + 2][3], e2 = w5[dt + 2][4];
+          const u32 rq = (a + b) + (m + d) + e2;
+          const int rsp = (int)(2u * e2 + d) - (int)(2u * a + b);
+          const u32 rspp = 4u * (a + e2) + (b + d);
+          Q += rq; Sp += rsp; Spp += rspp;
+          St += (int)rq * dt; Stt += rq * (u32)(dt * dt);
+        }
+      }
+      const int Vp = (int)(Q * Spp) - Sp * Sp, Vt = (int)(Q * Stt) - St * St;
+      const u32 qc = c[0];
+      const int t = t_base + (int)tl;
+      const float fQ = __uint2float_rn(Q);
+      const float pm = __fadd_rn(__uint2float_rn(pad), __fdiv_rn(__int2float_rn(Sp), fQ));
+      const float tm = __fadd_rn(__int2float_rn(t), __fdiv_rn(__int2float_rn(St), fQ));
+      const float sp = __fdiv_rn(__fsqrt_rn(__int2float_rn(Vp)), fQ);
+      const float st = __fdiv_rn(__fsqrt_rn(__int2float_rn(Vt)), fQ);
+      u32 fl = 0u;
+      if (pad < 2u || pad + 2u >= npads) fl |= 1u;
+      if (t < 2 || (u32)t + 2u >= PRM(n_time)) fl |= 2u;
+      if (qc == 1023u) fl |= 4u;
+      c0 = make_uint4(__float_as_uint(pm), __float_as_uint(tm), __float_as_uint(sp), __float_as_uint(st));
+      c1 = make_uint4(Q, qc | ((u32)t << 16), pad | (row << 8) | (sector << 16) | (fl << 24), 0u);
+    };
+    auto emit = [&](u64 slot, const uint4& c0, const uint4& c1) {
+      if (MODE == TPC_MODE_DET_TEMP) {
+        if (slot < a.temp_cap) { a.temp[slot * 2u] = c0; a.temp[slot * 2u + 1u] = c1; }
+      } else {
+        if (slot < a.capacity) { a.out[slot * 2u] = c0; a.out[slot * 2u + 1u] = c1; }
+        else atomicOr(a.status, TPC_STATUS_OVERFLOW);
+      }
+    };
+    if (MODE == TPC_MODE_FAST) {
+      // FAST: the order of the output is free (Q15), so nothing is ranked: every warp tests its peaks,
+      // reserves the places of its survivors with one global atomic -- in flight while the 5x5 sums
+      // are taken -- and writes them.  No survivor mask, no rank scan, no barrier before the emission.
+      const u32 lane = lane_id(), lt = (1u << lane) - 1u;
+      for (u32 i0 = (tid >> 5) * 32u; i0 < npk; i0 += TPC_K6_CONSUMERS) {
+        const u32 i = i0 + lane;
+        const u32 e = i < npk ? s.peaks[i] : 0u;
+        const bool keep = i < npk && !suppressed(e);
+        const u32 m = __ballot_sync(0xFFFFFFFFu, keep);
+        if (!m) continue;
+        u64 base = 0ull;
+        if (lane == 0u) base = atomicAdd(a.n_clusters, (u64)__popc(m));
+        if (keep) cog_sums(e, o0, o1);
+        base = __shfl_sync(0xFFFFFFFFu, base, 0);
+        if (keep) emit(base + __popc(m & lt), o0, o1);
+      }
+      // For the next tile (barrier A orders it before the scatter): barrier E -- nobody reads the map any
+      // more -- then a sparse tile undoes its own writes (every cell and peak bit sits at a record, and
+      // the thread that owns the record clears them) and any other tile is swept.
+      csync();   // E
+      if (total * 4u <= TPC_K6_CONSUMERS) {
+        if (my_r != 0u) {
+          const u32 tl = k6_row(my_r, sl), pad = my_r & 0xFFu;
+          s.tile[tl * pitch + pad + TPC_HALO] = 0;
+          s.pmask[tl * TPC_K6_PMW + ((pad + TPC_HALO) >> 5)] = 0u;
+        }
+        if (tid == 0) s.misc[0] = 0u;
+      } else
+        zero_tile();
+      continue;
+    }
+    bool survived = false;
+    for (u32 i = tid; i < npk; i += TPC_K6_CONSUMERS) {
+      const u32 e = s.peaks[i];
+      if (!suppressed(e)) { atomicOr(&s.rowmask[(e >> 8) * 8u + ((e & 0xFFu) >> 5)], 1u << (e & 31u)); survived = true; }
     }
     // F: survivor set complete.  With at most one peak per thread (the usual case) the barrier
     // itself counts the survivors, so the tile's base can be requested before the rank scan.
@@ -1650,7 +1765,6 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       }
     }
     // one cluster per thread held in registers across barrier G (further ones, npk > threads, after it)
-    uint4 o0 = make_uint4(0u, 0u, 0u, 0u), o1 = make_uint4(0u, 0u, 0u, 0u);
     u32 inrow = 0xFFFFFFFFu, my_tl = 0u;
     auto cog = [&](u32 e, uint4& c0, uint4& c1, u32& rk) -> bool {
       const u32 tl = e >> 8, pad = e & 0xFFu;
@@ -1659,69 +1773,8 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       if (!((mword >> bitpos) & 1u)) return false;   // suppressed
       rk = __popc(mword & ((1u << bitpos) - 1u));
       for (u32 k = 0; k < w; ++k) rk += __popc(s.rowmask[tl * 8u + k]);
-      const u16* c = s.tile + tl * pitch + pad + TPC_HALO;
-      // exact integer sums (Q12): per-row partial sums first, so the 25 loads and the adds of
-      // different rows are independent (short dependency chains; any order gives the same bits)
-      u32 Q = 0u, Spp = 0u, Stt = 0u;
-      int Sp = 0, St = 0;
-      if (!GATED) {   // Q10: every in-range cell, weight 1 (the reading is a kernel variant: no run-time test)
-#pragma unroll
-        for (int dt = -2; dt <= 2; ++dt) {
-          const u16* cr = c + dt * (int)pitch;
-          const u32 a = cr[-2], b = cr[-1], m = cr[0], d = cr[1], e2 = cr[2];
-          const u32 rq = (a + b) + (m + d) + e2;
-          const int rsp = (int)(2u * e2 + d) - (int)(2u * a + b);
-          const u32 rspp = 4u * (a + e2) + (b + d);
-          Q += rq; Sp += rsp; Spp += rspp;
-          St += (int)rq * dt; Stt += rq * (u32)(dt * dt);
-        }
-      } else {                 // Q10': an outer-ring cell counts only if the inner cell towards the peak holds charge
-        u32 w5[5][5];
-#pragma unroll
-        for (int dt = -2; dt <= 2; ++dt)
-#pragma unroll
-          for (int dp = -2; dp <= 2; ++dp) w5[dt + 2][dp + 2] = c[dt * (int)pitch + dp];
-#pragma unroll
-        for (int dt = -2; dt <= 2; ++dt)
-#pragma unroll
-          for (int dp = -2; dp <= 2; ++dp)
-            if (dt == -2 || dt == 2 || dp == -2 || dp == 2) {
-              const int it = dt < -1 ? -1 : (dt > 1 ? 1 : dt), ip = dp < -1 ? -1 : (dp > 1 ? 1 : dp);
-              if (w5[it + 2][ip + 2] == 0u) w5[dt + 2][dp + 2] = 0u;
-            }
-#pragma unroll
-        for (int dt = -2; dt <= 2; ++dt) {
-          const u32 a = w5[dt + 2][0], b = w5[dt + 2][1], m = w5[dt + 2][2], d = w5[dt + 2][3], e2 = w5[dt + 2][4];
-          const u32 rq = (a + b) + (m + d) + e2;
-          const int rsp = (int)(2u * e2 + d) - (int)(2u * a + b);
-          const u32 rspp = 4u * (a + e2) + (b + d);
-          Q += rq; Sp += rsp; Spp += rspp;
-          St += (int)rq * dt; Stt += rq * (u32)(dt * dt);
-        }
-      }
-      const int Vp = (int)(Q * Spp) - Sp * Sp, Vt = (int)(Q * Stt) - St * St;
-      const u32 qc = c[0];
-      const int t = t_base + (int)tl;
-      const float fQ = __uint2float_rn(Q);
-      const float pm = __fadd_rn(__uint2float_rn(pad), __fdiv_rn(__int2float_rn(Sp), fQ));
-      const float tm = __fadd_rn(__int2float_rn(t), __fdiv_rn(__int2float_rn(St), fQ));
-      const float sp = __fdiv_rn(__fsqrt_rn(__int2float_rn(Vp)), fQ);
-      const float st = __fdiv_rn(__fsqrt_rn(__int2float_rn(Vt)), fQ);
-      u32 fl = 0u;
-      if (pad < 2u || pad + 2u >= npads) fl |= 1u;
-      if (t < 2 || (u32)t + 2u >= PRM(n_time)) fl |= 2u;
-      if (qc == 1023u) fl |= 4u;
-      c0 = make_uint4(__float_as_uint(pm), __float_as_uint(tm), __float_as_uint(sp), __float_as_uint(st));
-      c1 = make_uint4(Q, qc | ((u32)t << 16), pad | (row << 8) | (sector << 16) | (fl << 24), 0u);
+      cog_sums(e, c0, c1);
       return true;
-    };
-    auto emit = [&](u64 slot, const uint4& c0, const uint4& c1) {
-      if (MODE == TPC_MODE_DET_TEMP) {
-        if (slot < a.temp_cap) { a.temp[slot * 2u] = c0; a.temp[slot * 2u + 1u] = c1; }
-      } else {
-        if (slot < a.capacity) { a.out[slot * 2u] = c0; a.out[slot * 2u + 1u] = c1; }
-        else atomicOr(a.status, TPC_STATUS_OVERFLOW);
-      }
     };
     if (tid < npk) {
       const u32 e = s.peaks[tid];
