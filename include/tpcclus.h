@@ -80,9 +80,14 @@ enum {
   TPCCLUS_RTC = 1, /* build the kernels with NVRTC at create(), geometry and thresholds baked
                       in as literals (PAPER.md 89-93); without it the offline-compiled kernels
                       read them from __constant__ memory (PAPER.md 79-85) */
-  TPCCLUS_COG_GATED = 2 /* reading Q10' of the centre of gravity: a cell of
+  TPCCLUS_COG_GATED = 2, /* reading Q10' of the centre of gravity: a cell of
                            the outer ring of the 5x5 window counts only if the inner cell between
                            it and the peak is non-empty.  Default off (Q10: every cell, weight 1) */
+  TPCCLUS_COG_SHARED = 4 /* reading Q10'' (second half; R8): a cell that lies in
+                            the 5x5 windows of a cluster and of its partners -- the surviving peaks at Chebyshev
+                            distance 2 -- is split between them with the integer weights (q_peak >> 2 d) + 1,
+                            d = distance of the cell from that peak; peak cells are never split.  Exclusive with
+                            TPCCLUS_COG_GATED (create returns TPCCLUS_ERR_INVALID_ARG for both).  Default off */
 };
 
 /* data-dependent conditions, OR-ed into *status on the device (never return codes) */
@@ -120,7 +125,7 @@ typedef struct {
   uint16_t thr_peak;      /* peak threshold, test is q >= thr_peak (Q6); default 6           */
   uint16_t noise_eps;     /* ridge tolerance of the suppression (O2, Q9); default 4          */
   uint64_t max_digits;    /* sizing only: largest n that run() will be given                 */
-  uint32_t flags;         /* TPCCLUS_RTC | TPCCLUS_COG_GATED                                 */
+  uint32_t flags;         /* TPCCLUS_RTC | TPCCLUS_COG_GATED | TPCCLUS_COG_SHARED            */
   int32_t device;         /* CUDA ordinal                                                    */
   void* workspace;        /* DEVICE, caller-owned, 256-byte aligned, lives as long as the handle */
   uint64_t workspace_bytes; /* >= tpcclus_workspace_bytes(params)                            */

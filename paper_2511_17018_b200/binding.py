@@ -19,6 +19,7 @@ _LIB_PATH = os.path.join(_HERE, "libtpcclus.so")
 MODE_FAST, MODE_DETERMINISTIC = 0, 1
 RTC = 1
 COG_GATED = 2
+COG_SHARED = 4
 STATUS_OVERFLOW, STATUS_BAD_DIGITS, STATUS_NO_PACKED, STATUS_INTERNAL = 1, 2, 4, 0x80000000
 FLAG_EDGE_PAD, FLAG_EDGE_TIME, FLAG_SATURATED = 1, 2, 4
 
@@ -168,7 +169,7 @@ class Clusterizer:
     """One handle + the torch tensors that own its device memory."""
 
     def __init__(self, n_sectors, n_rows, n_time, n_pads, max_digits, thr_peak=6, noise_eps=4, rtc=False,
-                 device=0, host_capacity=0, cog_gated=False):
+                 device=0, host_capacity=0, cog_gated=False, cog_shared=False):
         import torch
 
         if not torch.cuda.is_available():
@@ -179,7 +180,7 @@ class Clusterizer:
         self.n_pads = np.asarray(n_pads, dtype=np.uint16).copy()
         self.max_digits = int(max(1, max_digits))
         self.host_capacity = int(host_capacity)
-        flags = (RTC if rtc else 0) | (COG_GATED if cog_gated else 0)
+        flags = (RTC if rtc else 0) | (COG_GATED if cog_gated else 0) | (COG_SHARED if cog_shared else 0)
         p, self._pads_keep = make_params(n_sectors, n_rows, n_time, self.n_pads, self.max_digits, thr_peak, noise_eps,
                                          flags, device)
         nbytes = tpcclus_workspace_bytes_host(p, host_capacity) if host_capacity else tpcclus_workspace_bytes(p)

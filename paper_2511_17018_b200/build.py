@@ -24,8 +24,11 @@ SOURCES = [os.path.join(CSRC, "tpcclus.cu"), os.path.join(CSRC, "tpcclus_kernels
            os.path.join(ROOT, "include", "tpcclus.h")]
 
 # compilation units (PAPER.md 64: one GPU binary per kernel family): name -> TPC_U_* bit of tpcclus_kernels.cuh
-UNITS = {"part_coarse": 0x001, "dir": 0x002, "part_fine": 0x004, "tiles_fast": 0x008, "tiles_det": 0x010,
-         "order": 0x020, "tiles_dump": 0x040, "tiles_fast_g": 0x080, "tiles_det_g": 0x100}
+# (the units of reading Q10'' and the partition / debug units that feed them carry a time halo of 5: -DTPC_HALO=5u)
+UNITS = {"part_coarse": (0x001, 3), "dir": (0x002, 3), "part_fine": (0x004, 3), "tiles_fast": (0x008, 3), "tiles_det": (0x010, 3),
+         "order": (0x020, 3), "tiles_dump": (0x040, 3), "tiles_fast_g": (0x080, 3), "tiles_det_g": (0x100, 3),
+         "part_coarse_h5": (0x001, 5), "part_fine_h5": (0x004, 5), "tiles_dump_h5": (0x040, 5),
+         "tiles_fast_s": (0x200, 5), "tiles_det_s": (0x400, 5)}
 
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 DEVICE_FLAGS = [*ARCH, "-lineinfo", "-O3", "-std=c++17",
@@ -48,7 +51,8 @@ def _compile_unit(name: str, verbose: bool) -> str:
     """One unit straight to a GPU binary: nvcc -cubin for sm_100a (no PTX, no host code)."""
     out = unit_cubin(name)
     cmd = [_nvcc(), *DEVICE_FLAGS, *os.environ.get("TPC_EXTRA", "").split(), *(["-Xptxas", "-v"] if verbose else []),
-           "-DTPC_UNITS=%du" % UNITS[name], "-cubin", "-o", out, os.path.join(CSRC, "tpcclus_unit.cu")]
+           "-DTPC_UNITS=%du" % UNITS[name][0], "-DTPC_HALO=%du" % UNITS[name][1], "-cubin", "-o", out,
+           os.path.join(CSRC, "tpcclus_unit.cu")]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError("nvcc failed for unit %s:\n%s\n%s" % (name, r.stdout, r.stderr))

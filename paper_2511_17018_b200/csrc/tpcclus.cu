@@ -39,11 +39,15 @@
 extern "C" const char tpcclus_kernel_source[];   // the kernel text, embedded at build time (PAPER.md 91)
 
 // the unit binaries, embedded at build time (build/tpcclus_units.S: .incbin of build/unit_<name>.cubin)
+// X(name, TPC_U_* bit, time halo the unit is compiled with): the units of reading Q10'' -- its tile kernels and
+// the partition and debug units that feed them -- are built with TPC_HALO = 5 (paper_2511_17018_b200/build.py: UNITS)
 #define TPC_UNIT_LIST(X)                                                                              \
-  X(part_coarse, TPC_U_PART_COARSE) X(dir, TPC_U_DIR) X(part_fine, TPC_U_PART_FINE)                  \
-  X(tiles_fast, TPC_U_TILES_FAST) X(tiles_det, TPC_U_TILES_DET) X(order, TPC_U_ORDER)                \
-  X(tiles_dump, TPC_U_TILES_DUMP) X(tiles_fast_g, TPC_U_TILES_FAST_G) X(tiles_det_g, TPC_U_TILES_DET_G)
-#define X(name, bit) extern "C" const unsigned char tpcclus_cubin_##name[]; extern "C" const unsigned char tpcclus_cubin_##name##_end[];
+  X(part_coarse, TPC_U_PART_COARSE, 3) X(dir, TPC_U_DIR, 3) X(part_fine, TPC_U_PART_FINE, 3)          \
+  X(tiles_fast, TPC_U_TILES_FAST, 3) X(tiles_det, TPC_U_TILES_DET, 3) X(order, TPC_U_ORDER, 3)        \
+  X(tiles_dump, TPC_U_TILES_DUMP, 3) X(tiles_fast_g, TPC_U_TILES_FAST_G, 3) X(tiles_det_g, TPC_U_TILES_DET_G, 3) \
+  X(part_coarse_h5, TPC_U_PART_COARSE, 5) X(part_fine_h5, TPC_U_PART_FINE, 5) X(tiles_dump_h5, TPC_U_TILES_DUMP, 5) \
+  X(tiles_fast_s, TPC_U_TILES_FAST_S, 5) X(tiles_det_s, TPC_U_TILES_DET_S, 5)
+#define X(name, bit, halo) extern "C" const unsigned char tpcclus_cubin_##name[]; extern "C" const unsigned char tpcclus_cubin_##name##_end[];
 TPC_UNIT_LIST(X)
 #undef X
 
@@ -109,10 +113,12 @@ int make_geometry(const tpcclus_params* p, Geometry* g) {
   uint32_t tmin = p->n_time < TPC_TC ? p->n_time : TPC_TC;
   q.n_sl = (tmin + TPC_TS - 1) / TPC_TS;
   q.max_pads = maxp;
-  q.pitch = (maxp + 2 * TPC_HALO + 7) / 8 * 8;
+  q.pitch = (maxp + 2 * TPC_PG + 7) / 8 * 8;
   q.thr_peak = p->thr_peak; q.noise_eps = p->noise_eps;
-  q.cog_gated = (p->flags & TPCCLUS_COG_GATED) ? 1u : 0u;
-  q.max_peaks = ((TPC_TT - 2 + 1) / 2) * ((maxp + 1) / 2);   // no two peaks are 8-neighbours; rows 1..TT-2 are scanned
+  if ((p->flags & TPCCLUS_COG_GATED) && (p->flags & TPCCLUS_COG_SHARED)) return TPCCLUS_ERR_INVALID_ARG;   // one reading per handle
+  q.cog_mode = (p->flags & TPCCLUS_COG_SHARED) ? 2u : (p->flags & TPCCLUS_COG_GATED) ? 1u : 0u;
+  const uint32_t tt = TPC_TS + 2 * (q.cog_mode == 2u ? 5u : 3u);   // tile rows: the units of Q10'' carry a time halo of 5
+  q.max_peaks = ((tt - 2 + 1) / 2) * ((maxp + 1) / 2);   // no two peaks are 8-neighbours; rows 1..TT-2 are scanned
 
   g->max_digits = p->max_digits;
   g->g1 = (uint32_t)sm_count(p->device);
@@ -233,23 +239,30 @@ std::string drv_error(int rc) {
 }
 
 // ---- compilation units and kernels -------------------------------------------------------------
-enum UnitId { U_PART_COARSE, U_DIR, U_PART_FINE, U_TILES_FAST, U_TILES_DET, U_ORDER, U_TILES_DUMP, U_TILES_FAST_G, U_TILES_DET_G, U_COUNT_ };
-struct UnitInfo { const char* name; uint32_t bit; const unsigned char* cubin; const unsigned char* cubin_end; };
-#define X(name, bit) {#name, bit, tpcclus_cubin_##name, tpcclus_cubin_##name##_end},
+enum UnitId { U_PART_COARSE, U_DIR, U_PART_FINE, U_TILES_FAST, U_TILES_DET, U_ORDER, U_TILES_DUMP, U_TILES_FAST_G, U_TILES_DET_G,
+              U_PART_COARSE_H5, U_PART_FINE_H5, U_TILES_DUMP_H5, U_TILES_FAST_S, U_TILES_DET_S, U_COUNT_ };
+struct UnitInfo { const char* name; uint32_t bit; uint32_t halo; const unsigned char* cubin; const unsigned char* cubin_end; };
+#define X(name, bit, halo) {#name, bit, halo, tpcclus_cubin_##name, tpcclus_cubin_##name##_end},
 const UnitInfo kUnits[U_COUNT_] = {TPC_UNIT_LIST(X)};
 #undef X
 
+// The kernels a handle launches (one slot each) and the unit that provides the slot's kernel for each
+// reading of the centre of gravity: {Q10, Q10' gated, Q10'' shared}.
 enum KernelId { K_PART_COARSE, K_DIR_COUNT, K_DIR_SCAN, K_DIR_FILL, K_PART_FINE, K_TILES_FAST, K_TILES_DET,
-                K_TILES_DET_TEMP, K_TILES_DUMP, K_SCAN_LOCAL, K_SCAN_SUMS, K_EMIT_ORDERED, K_EMIT_PACKED,
-                K_TILES_FAST_G, K_TILES_DET_G, K_TILES_DET_TEMP_G, K_COUNT_ };
-struct KernelInfo { const char* name; UnitId unit; int smem; };   // smem: 0 none/static, 1 K1, 5 K5, 6 K6
+                K_TILES_DET_TEMP, K_TILES_DUMP, K_SCAN_LOCAL, K_SCAN_SUMS, K_EMIT_ORDERED, K_EMIT_PACKED, K_COUNT_ };
+struct KernelInfo { const char* name[3]; UnitId unit[3]; int smem; };   // smem: 0 none/static, 1 K1, 5 K5, 6 K6
+#define SAME3(x) {x, x, x}
 const KernelInfo kKernels[K_COUNT_] = {
-    {"k_partition_coarse", U_PART_COARSE, 1}, {"k_dir_count", U_DIR, 0}, {"k_dir_scan", U_DIR, 0}, {"k_dir_fill", U_DIR, 0},
-    {"k_partition_fine", U_PART_FINE, 5}, {"k_cluster_tiles_fast", U_TILES_FAST, 6}, {"k_cluster_tiles_det", U_TILES_DET, 6},
-    {"k_cluster_tiles_det_temp", U_TILES_DET, 6}, {"k_cluster_tiles_dump_map", U_TILES_DUMP, 6},
-    {"k_scan_local", U_ORDER, 0}, {"k_scan_sums", U_ORDER, 0}, {"k_emit_ordered", U_ORDER, 0}, {"k_emit_packed", U_ORDER, 0},
-    {"k_cluster_tiles_fast_gated", U_TILES_FAST_G, 6}, {"k_cluster_tiles_det_gated", U_TILES_DET_G, 6},
-    {"k_cluster_tiles_det_temp_gated", U_TILES_DET_G, 6}};
+    {SAME3("k_partition_coarse"), {U_PART_COARSE, U_PART_COARSE, U_PART_COARSE_H5}, 1},
+    {SAME3("k_dir_count"), SAME3(U_DIR), 0}, {SAME3("k_dir_scan"), SAME3(U_DIR), 0}, {SAME3("k_dir_fill"), SAME3(U_DIR), 0},
+    {SAME3("k_partition_fine"), {U_PART_FINE, U_PART_FINE, U_PART_FINE_H5}, 5},
+    {{"k_cluster_tiles_fast", "k_cluster_tiles_fast_gated", "k_cluster_tiles_fast_shared"}, {U_TILES_FAST, U_TILES_FAST_G, U_TILES_FAST_S}, 6},
+    {{"k_cluster_tiles_det", "k_cluster_tiles_det_gated", "k_cluster_tiles_det_shared"}, {U_TILES_DET, U_TILES_DET_G, U_TILES_DET_S}, 6},
+    {{"k_cluster_tiles_det_temp", "k_cluster_tiles_det_temp_gated", "k_cluster_tiles_det_temp_shared"}, {U_TILES_DET, U_TILES_DET_G, U_TILES_DET_S}, 6},
+    {SAME3("k_cluster_tiles_dump_map"), {U_TILES_DUMP, U_TILES_DUMP, U_TILES_DUMP_H5}, 6},
+    {SAME3("k_scan_local"), SAME3(U_ORDER), 0}, {SAME3("k_scan_sums"), SAME3(U_ORDER), 0},
+    {SAME3("k_emit_ordered"), SAME3(U_ORDER), 0}, {SAME3("k_emit_packed"), SAME3(U_ORDER), 0}};
+#undef SAME3
 
 }  // namespace
 
@@ -258,6 +271,8 @@ struct tpcclus_handle {
   tpcclus_params params;   // copy; n_pads points into g.prm
   char* ws = nullptr;
   bool is_rtc = false;
+  int cog = 0;                     // reading of the centre of gravity: 0 Q10, 1 Q10' gated, 2 Q10'' shared
+  uint32_t halo = 3;               // time halo of the handle's units (5 under Q10'')
   void* module[U_COUNT_] = {};     // one loaded GPU binary per compilation unit (PAPER.md 64)
   bool unit_cached[U_COUNT_] = {};
   void* fn[K_COUNT_] = {};
@@ -303,25 +318,25 @@ struct DeviceGuard {
 
 // One launch through the driver's module loader path: offline-compiled unit or NVRTC unit alike.
 int launch(tpcclus_handle* h, KernelId k, dim3 grid, dim3 block, uint32_t smem, cudaStream_t st, void** args) {
-  if (!h->fn[k]) return fail(h, TPCCLUS_ERR_CUDA, std::string("kernel not loaded: ") + kKernels[k].name);
+  if (!h->fn[k]) return fail(h, TPCCLUS_ERR_CUDA, std::string("kernel not loaded: ") + kKernels[k].name[h->cog]);
   if (h->timing && h->n_timed < kMaxKernels) {
     if (h->n_timed == 0) cudaEventRecord(h->ev[0], st);
-    h->timed_name[h->n_timed] = kKernels[k].name;
+    h->timed_name[h->n_timed] = kKernels[k].name[h->cog];
   }
   int rc = drv().cuLaunchKernel(h->fn[k], grid.x, grid.y, grid.z, block.x, block.y, block.z, smem, st, args, nullptr);
-  if (rc != 0) return fail(h, TPCCLUS_ERR_CUDA, std::string("cuLaunchKernel(") + kKernels[k].name + "): " + drv_error(rc));
+  if (rc != 0) return fail(h, TPCCLUS_ERR_CUDA, std::string("cuLaunchKernel(") + kKernels[k].name[h->cog] + "): " + drv_error(rc));
   if (h->timing && h->n_timed < kMaxKernels) { ++h->n_timed; cudaEventRecord(h->ev[h->n_timed], st); }
   return TPCCLUS_OK;
 }
 
 // Text put in front of the kernel source for NVRTC: every parameter as a literal, and the unit.
-std::string rtc_prologue(const TpcParams& q, uint32_t unit_bit) {
+std::string rtc_prologue(const TpcParams& q, uint32_t unit_bit, uint32_t halo) {
   char buf[256];
   std::string s = "#define TPC_RTC 1\n";
-  snprintf(buf, sizeof buf, "#define TPC_UNITS %uu\n", unit_bit); s += buf;
+  snprintf(buf, sizeof buf, "#define TPC_UNITS %uu\n#define TPC_HALO %uu\n", unit_bit, halo); s += buf;
 #define DEF(f) do { snprintf(buf, sizeof buf, "#define TPC_" #f " %uu\n", q.f); s += buf; } while (0)
   DEF(n_sectors); DEF(n_rows); DEF(n_time); DEF(n_tc); DEF(n_bins); DEF(n_sl); DEF(pitch); DEF(max_pads);
-  DEF(thr_peak); DEF(noise_eps); DEF(max_peaks); DEF(cog_gated);
+  DEF(thr_peak); DEF(noise_eps); DEF(max_peaks); DEF(cog_mode);
 #undef DEF
   s += "__device__ const unsigned short TPC_NPADS_TABLE[256] = {";
   for (int r = 0; r < 256; ++r) { snprintf(buf, sizeof buf, "%u,", (unsigned)q.n_pads[r]); s += buf; }
@@ -431,13 +446,13 @@ int load_unit(tpcclus_handle* h, UnitId u, const void* image) {
   int rc = d.cuModuleLoadData(&h->module[u], image);
   if (rc != 0) return fail(nullptr, TPCCLUS_ERR_CUDA, std::string("cuModuleLoadData(") + kUnits[u].name + "): " + drv_error(rc));
   for (int k = 0; k < K_COUNT_; ++k) {
-    if (kKernels[k].unit != u) continue;
-    if ((rc = d.cuModuleGetFunction(&h->fn[k], h->module[u], kKernels[k].name)) != 0)
-      return fail(nullptr, TPCCLUS_ERR_CUDA, std::string("cuModuleGetFunction(") + kKernels[k].name + "): " + drv_error(rc));
+    if (kKernels[k].unit[h->cog] != u) continue;
+    if ((rc = d.cuModuleGetFunction(&h->fn[k], h->module[u], kKernels[k].name[h->cog])) != 0)
+      return fail(nullptr, TPCCLUS_ERR_CUDA, std::string("cuModuleGetFunction(") + kKernels[k].name[h->cog] + "): " + drv_error(rc));
     const uint32_t smem = kKernels[k].smem == 1 ? h->smem_k1 : kKernels[k].smem == 5 ? h->smem_k5 : kKernels[k].smem == 6 ? h->smem_k6 : 0u;
     const int CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES = 8;
     if (smem > 48u * 1024u && (rc = d.cuFuncSetAttribute(h->fn[k], CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES, (int)smem)) != 0)
-      return fail(nullptr, TPCCLUS_ERR_CUDA, std::string("cuFuncSetAttribute(") + kKernels[k].name + "): " + drv_error(rc));
+      return fail(nullptr, TPCCLUS_ERR_CUDA, std::string("cuFuncSetAttribute(") + kKernels[k].name[h->cog] + "): " + drv_error(rc));
   }
   unsigned long long dptr = 0; size_t bytes = 0;
   if (d.cuModuleGetGlobal_v2(&dptr, &bytes, h->module[u], "c_prm") == 0) {   // RTC units have literals instead: nothing to register
@@ -471,7 +486,7 @@ int load_units(tpcclus_handle* h, const std::vector<UnitId>& want) {
     { std::lock_guard<std::mutex> lk(g_cache_mutex); dir = g_cache_dir; }
     if (dir.empty()) { const char* e = getenv("TPCCLUS_RTC_CACHE"); if (e) dir = e; }
     if (!dir.empty()) {
-      const std::string pro = rtc_prologue(h->g.prm, 0u);
+      const std::string pro = rtc_prologue(h->g.prm, 0u, h->halo);
       char name[64]; snprintf(name, sizeof name, "/tpcclus_handle_%016llx.lock", (unsigned long long)fnv1a(pro.data(), pro.size()));
       lock_fd = open((dir + name).c_str(), O_CREAT | O_RDWR, 0644);
       if (lock_fd >= 0) flock(lock_fd, LOCK_EX);
@@ -487,7 +502,7 @@ int load_units(tpcclus_handle* h, const std::vector<UnitId>& want) {
   for (size_t i = 0; i < n; ++i)
     th.emplace_back([&, i] {
       bool hit = false;
-      rcs[i] = cubin_for(rtc_prologue(h->g.prm, kUnits[units[i]].bit) + tpcclus_kernel_source, &cubins[i], &hit, &errs[i]);
+      rcs[i] = cubin_for(rtc_prologue(h->g.prm, kUnits[units[i]].bit, kUnits[units[i]].halo) + tpcclus_kernel_source, &cubins[i], &hit, &errs[i]);
       hits[i] = hit;
     });
   for (auto& t : th) t.join();
@@ -538,7 +553,9 @@ int tpcclus_create(const tpcclus_params* p, tpcclus_handle** out) {
   h->ws = (char*)p->workspace;
   h->smem_k1 = tpc_k1_smem_bytes(g.prm.n_bins);
   h->smem_k5 = tpc_k5_smem_bytes();
-  h->smem_k6 = tpc_k6_smem_bytes(g.prm.pitch, g.prm.max_peaks);
+  h->cog = (int)g.prm.cog_mode;
+  h->halo = h->cog == 2 ? 5u : 3u;
+  h->smem_k6 = tpc_k6_smem_bytes(g.prm.pitch, g.prm.max_peaks, h->halo);
   h->grid_k5 = g.g1;
   h->grid_k6 = g.g1 * TPC_K6_CTAS < g.n_tiles ? g.g1 * TPC_K6_CTAS : g.n_tiles;
   h->is_rtc = (p->flags & TPCCLUS_RTC) != 0;
@@ -548,11 +565,10 @@ int tpcclus_create(const tpcclus_params* p, tpcclus_handle** out) {
   for (uint32_t r = 0; r < p->n_rows; ++r) ro[r + 1] = ro[r] + (uint64_t)p->n_time * p->n_pads[r];
   cudaError_t e = cudaMemcpy(h->ws + g.lay.row_off, ro.data(), 8ull * ro.size(), cudaMemcpyHostToDevice);
   if (e != cudaSuccess) { cudaGetLastError(); g_create_error = std::string("cudaMemcpy(row_off): ") + cudaGetErrorString(e); return bail(TPCCLUS_ERR_CUDA); }
-  // the units this handle can launch (the debug unit comes on demand); a handle of reading Q10'
-  // loads -- and, under RTC, compiles -- the gated tile units instead of the plain ones
-  const bool gated = g.prm.cog_gated != 0u;
-  rc = load_units(h, {U_PART_COARSE, U_DIR, U_PART_FINE, gated ? U_TILES_FAST_G : U_TILES_FAST,
-                      gated ? U_TILES_DET_G : U_TILES_DET, U_ORDER});
+  // the units this handle can launch (the debug unit comes on demand); a handle of reading Q10' or Q10''
+  // loads -- and, under RTC, compiles -- that reading's units instead of the plain ones
+  rc = load_units(h, {kKernels[K_PART_COARSE].unit[h->cog], U_DIR, kKernels[K_PART_FINE].unit[h->cog],
+                      kKernels[K_TILES_FAST].unit[h->cog], kKernels[K_TILES_DET].unit[h->cog], U_ORDER});
   if (rc != TPCCLUS_OK) return bail(rc);
   for (int i = 0; i <= kMaxKernels; ++i)
     if (cudaEventCreate(&h->ev[i]) != cudaSuccess) { cudaGetLastError(); g_create_error = "cudaEventCreate failed"; return bail(TPCCLUS_ERR_CUDA); }
@@ -732,16 +748,15 @@ static int run_impl(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n
   a.tile_base = p.tile_base; a.tile_cnt = p.tile_cnt; a.det_flag = p.det_flag;
   a.dmap = nullptr; a.row_off = p.row_off;
   void* ka[] = {&a};
-  const bool gated = h->g.prm.cog_gated != 0u;   // reading Q10': its own kernel variants
   if (mode == TPCCLUS_MODE_FAST) {
     CUDA_TRY(h, cudaMemsetAsync(o_n, 0, 8, st));
-    if ((rc = launch(h, gated ? K_TILES_FAST_G : K_TILES_FAST, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
+    if ((rc = launch(h, K_TILES_FAST, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
   } else {
     // ordered output (PAPER.md 47-50): runs into the temporary buffer, scan of the tile counts,
     // ordered copy.  Should the buffer be too small (more than max_digits/8 clusters) the flag is
     // set, K9 does nothing and the chained-scan K6 redoes the frame; otherwise that launch exits at once.
     const Geometry& g = h->g;
-    if ((rc = launch(h, gated ? K_TILES_DET_TEMP_G : K_TILES_DET_TEMP, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
+    if ((rc = launch(h, K_TILES_DET_TEMP, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
     u32 nt = g.n_tiles, nblk = g.n_scan_blocks;
     { void* s[] = {&p.tile_cnt, &p.tile_local, &p.block_sum, &nt};
       if ((rc = launch(h, K_SCAN_LOCAL, dim3(nblk), dim3(TPC_SCAN_THREADS), 0, st, s))) return rc; }
@@ -757,7 +772,7 @@ static int run_impl(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n
       void* s[] = {&a.temp, &p.tile_base, &p.tile_cnt, &p.tile_local, &p.block_prefix, &nt, &o, &cap, &p.det_flag, &status};
       if ((rc = launch(h, K_EMIT_ORDERED, dim3(g.g1 * 8u), dim3(256), 0, st, s))) return rc;
       CUDA_TRY(h, cudaMemsetAsync(p.ticket, 0, 4, st));
-      if ((rc = launch(h, gated ? K_TILES_DET_G : K_TILES_DET, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
+      if ((rc = launch(h, K_TILES_DET, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
     }
   }
   h->ran = true;
@@ -830,7 +845,7 @@ int tpcclus_debug_dense_map(tpcclus_handle* h, uint16_t* d_map, void* cuda_strea
   cudaStream_t st = (cudaStream_t)cuda_stream;
   DeviceGuard dg;
   CUDA_TRY(h, dg.enter(h->params.device));
-  int rc = load_units(h, {U_TILES_DUMP});   // the debug unit is loaded (RTC: compiled) on first use
+  int rc = load_units(h, {kKernels[K_TILES_DUMP].unit[h->cog]});   // the debug unit is loaded (RTC: compiled) on first use
   if (rc) { h->err = g_create_error; return rc; }
   const Geometry& g = h->g;
   RunPtrs p = ptrs(h);

@@ -30,10 +30,11 @@
 #define TPC_U_TILES_DUMP 0x040u    // k_cluster_tiles_dump_map (debug hook of step a1)
 #define TPC_U_TILES_FAST_G 0x080u  // reading Q10' variants
 #define TPC_U_TILES_DET_G 0x100u
+#define TPC_U_TILES_FAST_S 0x200u  // reading Q10'' variants (compiled with TPC_HALO = 5, like the partition units they run behind)
+#define TPC_U_TILES_DET_S 0x400u
 #ifndef TPC_UNITS
 #define TPC_UNITS 0xFFFFFFFFu
 #endif
-#define TPC_U_ANY_TILES (TPC_U_TILES_FAST | TPC_U_TILES_DET | TPC_U_TILES_DUMP | TPC_U_TILES_FAST_G | TPC_U_TILES_DET_G)
 
 typedef unsigned int u32;
 typedef unsigned long long u64;
@@ -44,7 +45,10 @@ typedef unsigned char u8;
 #ifndef TPC_TS
 #define TPC_TS 128u            // time bins a tile owns
 #endif
-#define TPC_HALO 3u            // halo: peaks at distance 2 need charges at distance 3 (O2)
+#ifndef TPC_HALO
+#define TPC_HALO 3u            // time halo: peaks at distance 2 need charges at distance 3 (O2); the units of reading
+#endif                         // Q10'' are compiled with 5 (survivors at distance 2 need peaks at 4, charges at 5)
+#define TPC_PG 3u              // zero guard pads on each side of a map row (no pad-edge branches)
 #define TPC_TT (TPC_TS + 2u * TPC_HALO)   // rows of a tile in shared memory
 #ifndef TPC_TC
 #define TPC_TC 16256u          // time bins per coarse time-chunk: 127*128, +6 halo < 2^14
@@ -71,7 +75,7 @@ struct TpcParams {
   u32 max_pads;
   u32 thr_peak, noise_eps;
   u32 max_peaks;   // capacity of the per-tile peak list
-  u32 cog_gated;   // Q10' (host side only: selects the *_gated kernel variants)
+  u32 cog_mode;    // 0 = Q10, 1 = Q10' gated, 2 = Q10'' shared (host side only: selects the kernel variants)
   u16 n_pads[256];
 };
 
@@ -116,8 +120,9 @@ struct K6Args {
 
 #define TPC_K6_GROUP 4u   // tiles (consecutive slabs of one bin) a ticket covers
 #define TPC_K6_PMW 9u
-__host__ __device__ inline u32 tpc_k6_smem_bytes(u32 pitch, u32 max_peaks) {
-  return (TPC_K6_CAP + TPC_TT * pitch / 2u + 4u + 2u + TPC_TT * (8u + TPC_K6_PMW) + TPC_TT + 2u + 16u + (max_peaks + 1u) / 2u) * 4u + 128u;
+__host__ __device__ inline u32 tpc_k6_smem_bytes(u32 pitch, u32 max_peaks, u32 halo) {   // halo: the TPC_HALO of the handle's units
+  const u32 tt = TPC_TS + 2u * halo;
+  return (TPC_K6_CAP + tt * pitch / 2u + 4u + 2u + tt * (8u + TPC_K6_PMW) + tt + 2u + 16u + (max_peaks + 1u) / 2u) * 4u + 128u;
 }
 
 #ifdef TPC_RTC
@@ -1079,7 +1084,9 @@ __device__ __forceinline__ u32 k6_stage(const K6Smem& s, const K6Args& a, u64 ib
 }
 
 template <int V> struct TpcInt { static constexpr int v = V; };
-template <int MODE, bool GATED>
+// COG: the reading of the centre of gravity -- 0 = Q10 (every cell, weight 1), 1 = Q10' (outer ring gated),
+// 2 = Q10'' (charge shared with the surviving peaks on the outer ring; needs TPC_HALO >= 5)
+template <int MODE, int COG>
 __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
   const K6Smem s = k6_smem(smem);
   const u32 nb = PRM(n_bins), nsl = PRM(n_sl), pitch = PRM(pitch);
@@ -1087,6 +1094,10 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
   const u32 thr = PRM(thr_peak), eps = PRM(noise_eps);
   const u32 tile_words = TPC_TT * pitch / 2u;
   const u32 tid = threadIdx.x;
+  // rows whose peaks are listed and tested for survival: the owned rows; under Q10'' two more on each
+  // side, whose survivors the owned clusters share charge with (they are emitted by their own tiles)
+  static_assert(COG != 2 || TPC_HALO >= 5u, "reading Q10'' needs a time halo of 5");
+  constexpr u32 LIST_LO = COG == 2 ? TPC_HALO - 2u : TPC_HALO, LIST_HI = COG == 2 ? TPC_TS + TPC_HALO + 2u : TPC_TS + TPC_HALO;
 
   if (tid == 0) {
     mbar_init(&s.bar[0], 1u);                       // full: the producer's arrive (+ tx bytes)
@@ -1217,7 +1228,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
         if (nu * 4u <= TPC_K6_CONSUMERS) {   // a sparse tile: one record per thread, spread over all warps
           const u32 r = tid < nu * 4u ? rec[tid] : 0u;
           const u32 tl = k6_row(r, sl);
-          if (r != 0u && tl < TPC_TT) { s.tile[tl * pitch + (r & 0xFFu) + TPC_HALO] = (u16)((r >> 16) & 0x3FFu); my_r = r; }
+          if (r != 0u && tl < TPC_TT) { s.tile[tl * pitch + (r & 0xFFu) + TPC_PG] = (u16)((r >> 16) & 0x3FFu); my_r = r; }
         } else
         for (u32 u = tid; u < nu; u += TPC_K6_CONSUMERS) {
           const uint4 v = r4[u];
@@ -1226,7 +1237,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
           for (int k = 0; k < 4; ++k)
             if (rr[k] != 0u) {   // 0 = batch padding (every real record has q >= 1)
               const u32 tl = k6_row(rr[k], sl);
-              if (tl < TPC_TT) s.tile[tl * pitch + (rr[k] & 0xFFu) + TPC_HALO] = (u16)((rr[k] >> 16) & 0x3FFu);
+              if (tl < TPC_TT) s.tile[tl * pitch + (rr[k] & 0xFFu) + TPC_PG] = (u16)((rr[k] >> 16) & 0x3FFu);
             }
         }
       }
@@ -1244,7 +1255,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
             for (int k = 0; k < 4; ++k) {
               const u32 tl = k6_row(rr[k], sl);
               if (rr[k] != 0u && tl < TPC_TT) {
-                const u32 cell = tl * pitch + (rr[k] & 0xFFu) + TPC_HALO;
+                const u32 cell = tl * pitch + (rr[k] & 0xFFu) + TPC_PG;
                 const u16 q = (u16)((rr[k] >> 16) & 0x3FFu);
                 if (s.tile[cell] < q) { s.tile[cell] = q; any = 1u; }
               }
@@ -1274,7 +1285,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
         u32 tl = i / npads + TPC_HALO, p = i % npads;
         int t = t_base + (int)tl;
         if (t < (int)PRM(n_time))
-          a.dmap[(u64)sector * sector_cells + a.row_off[row] + (u64)t * npads + p] = s.tile[tl * pitch + p + TPC_HALO];
+          a.dmap[(u64)sector * sector_cells + a.row_off[row] + (u64)t * npads + p] = s.tile[tl * pitch + p + TPC_PG];
       }
       csync();
       zero_tile();
@@ -1311,8 +1322,8 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
           for (int k = 0; k < K; ++k) {
             const u32 q = (rr[k] >> 16) & 0x3FFu, tl = k6_row(rr[k], sl), pad = rr[k] & 0xFFu;
             cand[k] = q >= thr && tl - 1u < TPC_TT - 2u;   // (q = 0 for run padding)
-            if (check && !cand[k] && rr[k] != 0u && tl < TPC_TT && s.tile[tl * pitch + pad + TPC_HALO] < q) viol = 1u;
-            const u32 x = pad + TPC_HALO, h = x & 1u, sh = 16u - 16u * h;
+            if (check && !cand[k] && rr[k] != 0u && tl < TPC_TT && s.tile[tl * pitch + pad + TPC_PG] < q) viol = 1u;
+            const u32 x = pad + TPC_PG, h = x & 1u, sh = 16u - 16u * h;
             const u32* w = s.tile32 + (cand[k] ? tl * nW + (x >> 1) - 1u + h : 0u);
             pm[k] = __funnelshift_r(w[0], w[1], sh); nm[k] = (w[1] >> sh) & 0xFFFFu;
           }
@@ -1321,7 +1332,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
             const u32 q = (rr[k] >> 16) & 0x3FFu, tl = k6_row(rr[k], sl), pad = rr[k] & 0xFFu;
             if (check && cand[k] && (pm[k] >> 16) < q) viol = 1u;   // the cell holds a smaller duplicate of this record (Q5)
             cand[k] = cand[k] && (pm[k] >> 16) == q && q > (pm[k] & 0xFFFFu) && q >= nm[k];   // (!= q: a smaller duplicate of this cell)
-            const u32 x = pad + TPC_HALO, h = x & 1u, sh = 16u - 16u * h;
+            const u32 x = pad + TPC_PG, h = x & 1u, sh = 16u - 16u * h;
             const u32* w = s.tile32 + (cand[k] ? (tl - 1u) * nW + (x >> 1) - 1u + h : 0u);
             pu[k] = __funnelshift_r(w[0], w[1], sh); nu[k] = (w[1] >> sh) & 0xFFFFu;
             w += 2u * nW;
@@ -1333,9 +1344,9 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
             const u32 e = max(max(pu[k] & 0xFFFFu, pu[k] >> 16), nu[k]);
             const u32 l = max(max(pd[k] & 0xFFFFu, pd[k] >> 16), nd[k]);
             if (cand[k] && q > e && q >= l) {
-              const u32 bit = 1u << ((pad + TPC_HALO) & 31u);
-              const u32 old = atomicOr(&s.pmask[tl * TPC_K6_PMW + ((pad + TPC_HALO) >> 5)], bit);
-              if (!(old & bit) && tl >= TPC_HALO && tl < TPC_TS + TPC_HALO) {   // a halo-row peak is emitted by its own tile
+              const u32 bit = 1u << ((pad + TPC_PG) & 31u);
+              const u32 old = atomicOr(&s.pmask[tl * TPC_K6_PMW + ((pad + TPC_PG) >> 5)], bit);
+              if (!(old & bit) && tl >= LIST_LO && tl < LIST_HI) {   // a halo-row peak is emitted by its own tile
                 const u32 i = atomicAdd(&s.misc[0], 1u);
                 s.peaks[i] = (u16)((tl << 8) | pad);
               }
@@ -1367,7 +1378,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
           for (int k = 0; k < 4; ++k) {
             const u32 q = (rr[k] >> 16) & 0x3FFu, tl = k6_row(rr[k], sl), pad = rr[k] & 0xFFu;
             cand[k] = q >= thr && tl - 1u < TPC_TT - 2u;   // (q = 0 for run padding)
-            const u32 x = pad + TPC_HALO, h = x & 1u, sh = 16u - 16u * h;
+            const u32 x = pad + TPC_PG, h = x & 1u, sh = 16u - 16u * h;
             const u32* w = s.tile32 + (cand[k] ? tl * nW + (x >> 1) - 1u + h : 0u);   // the others: word 0, a broadcast
             pm[k] = __funnelshift_r(w[0], w[1], sh); nm[k] = (w[1] >> sh) & 0xFFFFu;
           }
@@ -1394,7 +1405,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
 #pragma unroll
           for (int k = 0; k < 2; ++k) {
             const u32 tl = k6_row(r2[k], sl), pad = r2[k] & 0xFFu;
-            const u32 x = pad + TPC_HALO, h = x & 1u, sh = 16u - 16u * h;
+            const u32 x = pad + TPC_PG, h = x & 1u, sh = 16u - 16u * h;
             const u32* w = s.tile32 + (r2[k] != 0u ? (tl - 1u) * nW + (x >> 1) - 1u + h : 0u);
             pu[k] = __funnelshift_r(w[0], w[1], sh); nu[k] = (w[1] >> sh) & 0xFFFFu;
             w += 2u * nW;
@@ -1407,9 +1418,9 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
             const u32 l = max(max(pd[k] & 0xFFFFu, pd[k] >> 16), nd[k]);
             bool own = false;
             if (r2[k] != 0u && q > e && q >= l) {
-              const u32 bit = 1u << ((pad + TPC_HALO) & 31u);
-              const u32 old = atomicOr(&s.pmask[tl * TPC_K6_PMW + ((pad + TPC_HALO) >> 5)], bit);
-              own = !(old & bit) && tl >= TPC_HALO && tl < TPC_TS + TPC_HALO;   // a halo-row peak is emitted by its own tile
+              const u32 bit = 1u << ((pad + TPC_PG) & 31u);
+              const u32 old = atomicOr(&s.pmask[tl * TPC_K6_PMW + ((pad + TPC_PG) >> 5)], bit);
+              own = !(old & bit) && tl >= LIST_LO && tl < LIST_HI;   // a halo-row peak is emitted by its own tile
             }
             const u32 m = __ballot_sync(0xFFFFFFFFu, own);
             if (m) {
@@ -1432,7 +1443,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
             for (int k = 0; k < 4; ++k) {
               const u32 tl = k6_row(rr[k], sl);
               if (rr[k] != 0u && tl < TPC_TT) {
-                const u32 cell = tl * pitch + (rr[k] & 0xFFu) + TPC_HALO;
+                const u32 cell = tl * pitch + (rr[k] & 0xFFu) + TPC_PG;
                 const u16 q = (u16)((rr[k] >> 16) & 0x3FFu);
                 if (s.tile[cell] < q) { s.tile[cell] = q; any = 1u; }
               }
@@ -1453,7 +1464,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
               const u32 tl = k6_row(rr[k], sl);
-              c4[k] = s.tile[(tl < TPC_TT ? tl * pitch : 0u) + (rr[k] & 0xFFu) + TPC_HALO];
+              c4[k] = s.tile[(tl < TPC_TT ? tl * pitch : 0u) + (rr[k] & 0xFFu) + TPC_PG];
             }
 #pragma unroll
             for (int k = 0; k < 4; ++k)
@@ -1494,7 +1505,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
     // and can never be flagged.  The peaks of owned rows are listed afterwards, from pmask.
     {
       const u32 nW = pitch >> 1;
-      const u32 ng = ((npads + TPC_HALO - 1u) >> 3) + 1u;   // 8-cell groups up to the last real pad's cell (npads + 2)
+      const u32 ng = ((npads + TPC_PG - 1u) >> 3) + 1u;   // 8-cell groups up to the last real pad's cell (npads + 2)
       const u32 strips = TPC_K6_CONSUMERS / ng;          // >= 1: npads <= 256 -> ng <= 33
       const u32 rp = (TPC_TT - 2u + strips - 1u) / strips;
       const u32 si = tid / ng, g = tid - si * ng;
@@ -1540,13 +1551,13 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       }
       csync();   // D': pmask complete
       // the peaks of the owned rows, listed from pmask: a warp per 32 mask words, one shared atomic per warp step
-      const u32 nwp = ((npads + TPC_HALO - 1u) >> 5) + 1u;   // mask words that can hold a peak
+      const u32 nwp = ((npads + TPC_PG - 1u) >> 5) + 1u;   // mask words that can hold a peak
       const u32 inv = 65536u / nwp + 1u;                      // i / nwp for i < 2^11 (exact: nwp <= 9)
       const u32 lane = lane_id(), lt = (1u << lane) - 1u;
-      for (u32 i0 = (tid >> 5) * 32u; i0 < TPC_TS * nwp; i0 += TPC_K6_CONSUMERS) {
+      for (u32 i0 = (tid >> 5) * 32u; i0 < (LIST_HI - LIST_LO) * nwp; i0 += TPC_K6_CONSUMERS) {
         const u32 i = i0 + lane;
         const u32 rw = (i * inv) >> 16, wd = i - rw * nwp;
-        u32 w = i < TPC_TS * nwp ? s.pmask[(rw + TPC_HALO) * TPC_K6_PMW + wd] : 0u;
+        u32 w = i < (LIST_HI - LIST_LO) * nwp ? s.pmask[(rw + LIST_LO) * TPC_K6_PMW + wd] : 0u;
         for (;;) {
           const u32 m = __ballot_sync(0xFFFFFFFFu, w != 0u);
           if (!m) break;
@@ -1556,7 +1567,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
           if (w != 0u) {
             const u32 bpos = (u32)__ffs((int)w) - 1u;
             w &= w - 1u;
-            s.peaks[base + __popc(m & lt)] = (u16)(((rw + TPC_HALO) << 8) | (wd * 32u + bpos - TPC_HALO));
+            s.peaks[base + __popc(m & lt)] = (u16)(((rw + LIST_LO) << 8) | (wd * 32u + bpos - TPC_PG));
           }
         }
       }
@@ -1568,7 +1579,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
     auto suppressed = [&](const u32 e) -> bool {
       const u32 tl = e >> 8, pad = e & 0xFFu;
       // the 5x5 ring of peak bits around (tl, pad): 5 bits per row, bit k <-> dp = k - 2
-      const u32 w0 = (pad + TPC_HALO - 2u) >> 5, sh = (pad + TPC_HALO - 2u) & 31u;   // bit of (pad - 2) = cell index pad + HALO - 2
+      const u32 w0 = (pad + TPC_PG - 2u) >> 5, sh = (pad + TPC_PG - 2u) & 31u;   // bit of (pad - 2) = cell index pad + HALO - 2
       u32 ring = 0u;
 #pragma unroll
       for (int dt = -2; dt <= 2; ++dt) {
@@ -1578,7 +1589,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       }
       bool dead = false;
       if (ring) {   // some peak at Chebyshev distance exactly 2
-        const u16* c = s.tile + tl * pitch + pad + TPC_HALO;
+        const u16* c = s.tile + tl * pitch + pad + TPC_PG;
         const u32 qc = c[0];
         u32 nq[3][3];
 #pragma unroll
@@ -1607,15 +1618,67 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       return dead;
     };
     uint4 o0 = make_uint4(0u, 0u, 0u, 0u), o1 = make_uint4(0u, 0u, 0u, 0u);
+    const auto owned = [&](u32 e) -> bool { return COG != 2 || ((e >> 8) >= TPC_HALO && (e >> 8) < TPC_TS + TPC_HALO); };
+    const auto survivor = [&](u32 e) -> bool { return (s.rowmask[(e >> 8) * 8u + ((e & 0xFFu) >> 5)] >> (e & 31u)) & 1u; };
+    // Q10'' (R8): the sums O3 with the charge of every cell that a partner's window also holds
+    // split by the integer weights w_p(x) = (q_p >> 2 cheb(p, x)) + 1.  Partners = the survivors on the
+    // outer ring of the window, read from rowmask (complete: barrier F).  Peak cells are never split.
+    auto shared_sums = [&](u32 tl, u32 pad, const u16* c, u32& Q, int& Sp, int& St, u32& Spp, u32& Stt) -> bool {
+      const u32 st0 = (pad > 2u ? pad : 2u) - 2u, w0 = st0 >> 5, sh = st0 & 31u;   // window bits pad-2 .. pad+2 of the survivor rows
+      u32 ring = 0u;
+#pragma unroll
+      for (int dt = -2; dt <= 2; ++dt) {
+        const u32* rm = s.rowmask + (tl + dt) * 8u + w0;
+        u32 win = __funnelshift_r(rm[0], w0 < 7u ? rm[1] : 0u, sh);
+        if (pad < 2u) win <<= 2u - pad;   // pads -2, -1 do not exist
+        ring |= (win & ((dt == -2 || dt == 2) ? 0x1Fu : 0x11u)) << (5 * (dt + 2));
+      }
+      if (ring == 0u) return false;
+      const u32 qc = c[0];
+      u32 q5[25], den[25], kill = 0u;
+#pragma unroll
+      for (int k = 0; k < 25; ++k) {
+        const int dt = k / 5 - 2, dp = k % 5 - 2, d = max(abs(dt), abs(dp));
+        q5[k] = c[dt * (int)pitch + dp];
+        den[k] = (qc >> (2 * d)) + 1u;
+      }
+      while (ring) {
+        const int b = __ffs((int)ring) - 1;
+        ring &= ring - 1u;
+        const int et = b / 5 - 2, ep = b - (b / 5) * 5 - 2;
+        const u32 qp = c[et * (int)pitch + ep];
+#pragma unroll
+        for (int k = 0; k < 25; ++k) {
+          const int dt = k / 5 - 2, dp = k % 5 - 2;
+          const int d2 = max(abs(et - dt), abs(ep - dp));
+          if (d2 <= 2) den[k] += (qp >> (2 * d2)) + 1u;
+          if (d2 == 0) kill |= 1u << k;
+        }
+      }
+#pragma unroll
+      for (int k = 0; k < 25; ++k) {
+        const int dt = k / 5 - 2, dp = k % 5 - 2, d = max(abs(dt), abs(dp));
+        const u32 wc = (qc >> (2 * d)) + 1u;
+        u32 sh_q = q5[k];
+        if (k != 12 && den[k] != wc) sh_q = q5[k] * wc / den[k];
+        if ((kill >> k) & 1u) sh_q = 0u;
+        Q += sh_q; Sp += (int)sh_q * dp; St += (int)sh_q * dt;
+        Spp += sh_q * (u32)(dp * dp); Stt += sh_q * (u32)(dt * dt);
+      }
+      return true;
+    };
     // O3 + O4 for one surviving peak
     auto cog_sums = [&](u32 e, uint4& c0, uint4& c1) {
       const u32 tl = e >> 8, pad = e & 0xFFu;
-      const u16* c = s.tile + tl * pitch + pad + TPC_HALO;
+      const u16* c = s.tile + tl * pitch + pad + TPC_PG;
       // exact integer sums (Q12): per-row partial sums first, so the 25 loads and the adds of
       // different rows are independent (short dependency chains; any order gives the same bits)
       u32 Q = 0u, Spp = 0u, Stt = 0u;
       int Sp = 0, St = 0;
-      if (!GATED) {   // Q10: every in-range cell, weight 1 (the reading is a kernel variant: no run-time test)
+      bool done = false;
+      if (COG == 2) done = shared_sums(tl, pad, c, Q, Sp, St, Spp, Stt);   // Q10'': false when the peak has no partner
+      if (done) {
+      } else if (COG != 1) {   // Q10: every in-range cell, weight 1 (the reading is a kernel variant: no run-time test)
 #pragma unroll
         for (int dt = -2; dt <= 2; ++dt) {
           const u16* cr = c + dt * (int)pitch;
@@ -1678,10 +1741,17 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       // reserves the places of its survivors with one global atomic -- in flight while the 5x5 sums
       // are taken -- and writes them.  No survivor mask, no rank scan, no barrier before the emission.
       const u32 lane = lane_id(), lt = (1u << lane) - 1u;
+      if (COG == 2) {   // Q10'': the survivor set of all listed rows first (the partners of the owned clusters), barrier F
+        for (u32 i = tid; i < npk; i += TPC_K6_CONSUMERS) {
+          const u32 e = s.peaks[i];
+          if (!suppressed(e)) atomicOr(&s.rowmask[(e >> 8) * 8u + ((e & 0xFFu) >> 5)], 1u << (e & 31u));
+        }
+        csync();
+      }
       for (u32 i0 = (tid >> 5) * 32u; i0 < npk; i0 += TPC_K6_CONSUMERS) {
         const u32 i = i0 + lane;
         const u32 e = i < npk ? s.peaks[i] : 0u;
-        const bool keep = i < npk && !suppressed(e);
+        const bool keep = i < npk && (COG == 2 ? owned(e) && survivor(e) : !suppressed(e));
         const u32 m = __ballot_sync(0xFFFFFFFFu, keep);
         if (!m) continue;
         u64 base = 0ull;
@@ -1697,8 +1767,9 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       if (total * 4u <= TPC_K6_CONSUMERS) {
         if (my_r != 0u) {
           const u32 tl = k6_row(my_r, sl), pad = my_r & 0xFFu;
-          s.tile[tl * pitch + pad + TPC_HALO] = 0;
-          s.pmask[tl * TPC_K6_PMW + ((pad + TPC_HALO) >> 5)] = 0u;
+          s.tile[tl * pitch + pad + TPC_PG] = 0;
+          s.pmask[tl * TPC_K6_PMW + ((pad + TPC_PG) >> 5)] = 0u;
+          if (COG == 2) s.rowmask[tl * 8u + (pad >> 5)] = 0u;
         }
         if (tid == 0) s.misc[0] = 0u;
       } else
@@ -1708,7 +1779,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
     bool survived = false;
     for (u32 i = tid; i < npk; i += TPC_K6_CONSUMERS) {
       const u32 e = s.peaks[i];
-      if (!suppressed(e)) { atomicOr(&s.rowmask[(e >> 8) * 8u + ((e & 0xFFu) >> 5)], 1u << (e & 31u)); survived = true; }
+      if (!suppressed(e)) { atomicOr(&s.rowmask[(e >> 8) * 8u + ((e & 0xFFu) >> 5)], 1u << (e & 31u)); if (owned(e)) survived = true; }
     }
     // F: survivor set complete.  With at most one peak per thread (the usual case) the barrier
     // itself counts the survivors, so the tile's base can be requested before the rank scan.
@@ -1741,7 +1812,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
         for (int k = 0; k < 5; ++k) {
           const uint4 x = v[2 * k], y = v[2 * k + 1];
           const u32 n = (__popc(x.x) + __popc(x.y)) + (__popc(x.z) + __popc(x.w)) + ((__popc(y.x) + __popc(y.y)) + (__popc(y.z) + __popc(y.w)));
-          cnt[k] = lane * 5u + (u32)k < TPC_TT ? n : 0u; t += cnt[k];
+          cnt[k] = (lane * 5u + (u32)k >= TPC_HALO && lane * 5u + (u32)k < TPC_TS + TPC_HALO) ? n : 0u; t += cnt[k];   // survivors only sit in listed rows, clusters in owned ones
         }
       }
       u32 inc = t;
@@ -1770,7 +1841,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       const u32 tl = e >> 8, pad = e & 0xFFu;
       const u32 w = pad >> 5, bitpos = pad & 31u;
       const u32 mword = s.rowmask[tl * 8u + w];
-      if (!((mword >> bitpos) & 1u)) return false;   // suppressed
+      if (!((mword >> bitpos) & 1u) || !owned(e)) return false;   // suppressed, or a partner in a halo row
       rk = __popc(mword & ((1u << bitpos) - 1u));
       for (u32 k = 0; k < w; ++k) rk += __popc(s.rowmask[tl * 8u + k]);
       cog_sums(e, c0, c1);
@@ -1799,8 +1870,8 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
     if (total * 4u <= TPC_K6_CONSUMERS) {   // block-uniform (the condition of the sparse scatter)
       if (my_r != 0u) {
         const u32 tl = k6_row(my_r, sl), pad = my_r & 0xFFu;
-        s.tile[tl * pitch + pad + TPC_HALO] = 0;
-        s.pmask[tl * TPC_K6_PMW + ((pad + TPC_HALO) >> 5)] = 0u;
+        s.tile[tl * pitch + pad + TPC_PG] = 0;
+        s.pmask[tl * TPC_K6_PMW + ((pad + TPC_PG) >> 5)] = 0u;
         s.rowmask[tl * 8u + (pad >> 5)] = 0u;
       }
       if (tid == 0) s.misc[0] = 0u;
@@ -1810,30 +1881,38 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
   }
 }
 
-#define TPC_K6_ENTRY(name, MODE, GATED, GUARD)                                                          \
+#define TPC_K6_ENTRY(name, MODE, COG, GUARD)                                                            \
   extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, TPC_K6_CTAS) name(K6Args a) {             \
     extern __shared__ __align__(128) u32 smem_u32[];                                                    \
     GUARD                                                                                               \
-    k6_body<MODE, GATED>(a, smem_u32);                                                                  \
+    k6_body<MODE, COG>(a, smem_u32);                                                                  \
   }
 // the chained-scan variants only run when K7-K9 could not deliver the ordered output (flag set)
 #define TPC_K6_IF_FLAG if (*a.det_flag == 0u) return;
 #if TPC_UNITS & TPC_U_TILES_FAST
-TPC_K6_ENTRY(k_cluster_tiles_fast, TPC_MODE_FAST, false, )
+TPC_K6_ENTRY(k_cluster_tiles_fast, TPC_MODE_FAST, 0, )
 #endif
 #if TPC_UNITS & TPC_U_TILES_DET
-TPC_K6_ENTRY(k_cluster_tiles_det, TPC_MODE_DET, false, TPC_K6_IF_FLAG)
-TPC_K6_ENTRY(k_cluster_tiles_det_temp, TPC_MODE_DET_TEMP, false, )
+TPC_K6_ENTRY(k_cluster_tiles_det, TPC_MODE_DET, 0, TPC_K6_IF_FLAG)
+TPC_K6_ENTRY(k_cluster_tiles_det_temp, TPC_MODE_DET_TEMP, 0, )
 #endif
 #if TPC_UNITS & TPC_U_TILES_DUMP
-TPC_K6_ENTRY(k_cluster_tiles_dump_map, TPC_MODE_DUMP_MAP, false, )
+TPC_K6_ENTRY(k_cluster_tiles_dump_map, TPC_MODE_DUMP_MAP, 0, )
 #endif
 // reading Q10' (TPCCLUS_COG_GATED)
 #if TPC_UNITS & TPC_U_TILES_FAST_G
-TPC_K6_ENTRY(k_cluster_tiles_fast_gated, TPC_MODE_FAST, true, )
+TPC_K6_ENTRY(k_cluster_tiles_fast_gated, TPC_MODE_FAST, 1, )
 #endif
 #if TPC_UNITS & TPC_U_TILES_DET_G
-TPC_K6_ENTRY(k_cluster_tiles_det_gated, TPC_MODE_DET, true, TPC_K6_IF_FLAG)
-TPC_K6_ENTRY(k_cluster_tiles_det_temp_gated, TPC_MODE_DET_TEMP, true, )
+TPC_K6_ENTRY(k_cluster_tiles_det_gated, TPC_MODE_DET, 1, TPC_K6_IF_FLAG)
+TPC_K6_ENTRY(k_cluster_tiles_det_temp_gated, TPC_MODE_DET_TEMP, 1, )
+#endif
+// reading Q10'' (TPCCLUS_COG_SHARED): these units -- and the partition units of such a handle -- are compiled with TPC_HALO = 5
+#if TPC_UNITS & TPC_U_TILES_FAST_S
+TPC_K6_ENTRY(k_cluster_tiles_fast_shared, TPC_MODE_FAST, 2, )
+#endif
+#if TPC_UNITS & TPC_U_TILES_DET_S
+TPC_K6_ENTRY(k_cluster_tiles_det_shared, TPC_MODE_DET, 2, TPC_K6_IF_FLAG)
+TPC_K6_ENTRY(k_cluster_tiles_det_temp_shared, TPC_MODE_DET_TEMP, 2, )
 #endif
 #endif   // TPC_UNITS != 0u

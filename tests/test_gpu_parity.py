@@ -742,3 +742,71 @@ def test_rtc_cache_survives_a_damaged_file(tp, cuda_device, tmp_path):
         c.close()
     finally:
         tp.tpcclus_set_rtc_cache_dir(None)
+
+
+def test_cog_shared_reading(tp, cuda_device):
+    """Reading Q10'' (TPCCLUS_COG_SHARED, second half; R8): charge sharing
+    between clusters whose windows overlap, byte for byte against the oracle in the same reading --
+    deterministic, fast, generic and RTC.  A handle of this reading runs units compiled with a time
+    halo of 5 (partition, tiles, debug map): the a1 map, a frame longer than one coarse time-chunk
+    (halo copies across the chunk border) and the densest peak pattern go through them too."""
+    frames = [make_frame(1), make_frame(0), make_frame(4, device=cuda_device, sectors=[3, 20], n_time=300)]
+    for fr in frames:
+        d_np = fr.digits_numpy()
+        exp, st, n = t1.clusterize(d_np.view(t1.DIGIT), fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, cog_shared=True)
+        plain, _ = _oracle(d_np, fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads)
+        assert len(exp) == len(plain)
+        if fr.meta["config"] != 0:
+            assert exp.tobytes() != plain.tobytes()      # the reading matters on the crowded frames
+        for rtc in (False, True):
+            c = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, fr.n_digits, rtc=rtc, cog_shared=True)
+            det = c.run_sync(fr.digits.to(cuda_device), tp.MODE_DETERMINISTIC)[0]
+            fast = c.run_sync(fr.digits.to(cuda_device), tp.MODE_FAST)[0]
+            if not rtc:
+                assert set(c.loaded_units()) == {"part_coarse_h5", "dir", "part_fine_h5", "tiles_fast_s", "tiles_det_s", "order"}
+                _, _, _, m = t1.clusterize(d_np.view(t1.DIGIT), fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, return_map=True)
+                assert np.array_equal(c.dense_map().cpu().numpy().view(np.uint16), m)      # step a1 through the halo-5 units
+            c.close()
+            assert det.tobytes() == exp.tobytes(), (fr.meta["name"], rtc)
+            _check_fast(fast, exp)
+    with pytest.raises(tp.TpcclusError):
+        tp.Clusterizer(1, 16, 256, [64] * 16, 1000, cog_gated=True, cog_shared=True)
+    # three coarse time-chunks, clusters planted on both chunk borders with partners two bins apart
+    rng = np.random.default_rng(19)
+    T, pads = 40000, [24, 40]
+    rows = []
+    for tb in (16256, 32512):
+        for dt in range(-8, 9, 2):
+            for r in (0, 1):
+                rows.append((0, r, 10, tb + dt, int(rng.integers(30, 200))))
+                rows.append((0, r, 12, tb + dt, int(rng.integers(30, 200))))
+                rows.append((0, r, 11, tb + dt, int(rng.integers(3, 9))))
+    seen = {(x[1], x[2], x[3]) for x in rows}
+    for _ in range(20000):
+        key = (int(rng.integers(0, 2)), int(rng.integers(0, 24)), int(rng.integers(0, T)))
+        if key not in seen:
+            seen.add(key)
+            rows.append((0, key[0], key[1], key[2], int(rng.integers(1, 120))))
+    d = t1.make_digits(rows)
+    d = d[rng.permutation(len(d))]
+    exp, st_exp, _ = t1.clusterize(d, 1, 2, T, pads, cog_shared=True)
+    c = tp.Clusterizer(1, 2, T, pads, len(d), cog_shared=True)
+    det, n, st = c.run_sync(_digits_tensor(d, cuda_device), tp.MODE_DETERMINISTIC)
+    fast = c.run_sync(_digits_tensor(d, cuda_device), tp.MODE_FAST)[0]
+    c.close()
+    assert st == st_exp == 0 and det.tobytes() == exp.tobytes()
+    _check_fast(fast, exp)
+    # checkerboard of equal charges: every cell a survivor with up to 8 partners; and heavy ties
+    T, P = 300, 138
+    rows = [(0, 0, p, t, 50) for t in range(0, T, 2) for p in range(0, P, 2)]
+    q = rng.integers(5, 10, size=(T, P))
+    rows += [(0, 1, p, t, int(q[t, p])) for t in range(T) for p in range(P)]
+    d = t1.make_digits(rows)
+    d = d[rng.permutation(len(d))]
+    exp, _, _ = t1.clusterize(d, 1, 2, T, [P, P], cog_shared=True)
+    c = tp.Clusterizer(1, 2, T, [P, P], len(d), cog_shared=True)
+    det = c.run_sync(_digits_tensor(d, cuda_device), tp.MODE_DETERMINISTIC)[0]
+    fast = c.run_sync(_digits_tensor(d, cuda_device), tp.MODE_FAST)[0]
+    c.close()
+    assert det.tobytes() == exp.tobytes()
+    _check_fast(fast, exp)
