@@ -129,7 +129,7 @@ int make_geometry(const tpcclus_params* p, Geometry* g) {
   if (cap > 0x0FFFFFFFull) return TPCCLUS_ERR_INVALID_ARG;
   g->slice_cap = (uint32_t)cap;
   g->n_chunks_max = (uint64_t)g->g1 * cap;
-  if (g->n_chunks_max > 0x00FFFFFFFFull) return TPCCLUS_ERR_INVALID_ARG;
+  if (g->n_chunks_max > (1ull << 26)) return TPCCLUS_ERR_INVALID_ARG;   // chunk ids are 26 bits in the chunk lists (4.3e9 records)
   g->n_batches_max = g->n_chunks_max / TPC_CPB + nb + 1;
   // K5 writes every record once; per batch at most 3 zero records in front of each of its n_sl + 1
   // A runs (16-byte alignment) and 7 at its end (32-byte alignment)

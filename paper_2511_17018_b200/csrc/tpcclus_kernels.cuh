@@ -356,7 +356,6 @@ __device__ __forceinline__ void k1_rounds(const K1Smem& s, const uint2* __restri
   auto decode = [&](const uint4 (&curd)[TPC_K1_DPT / 2], u32 (&bin)[TPC_K1_DPT], u32 (&rec)[TPC_K1_DPT], u32& pend,
                     u32 (&dbin)[TPC_K1_DPT], u32 (&drec)[TPC_K1_DPT], u32& dpend) {
     pend = 0u; dpend = 0u;
-    u32 vm = 0u;   // digits in range (whatever their charge)
 #pragma unroll
     for (int k = 0; k < TPC_K1_DPT; ++k) {
       const u32 w0 = (k & 1) ? curd[k >> 1].z : curd[k >> 1].x, w1 = (k & 1) ? curd[k >> 1].w : curd[k >> 1].y;
@@ -365,9 +364,12 @@ __device__ __forceinline__ void k1_rounds(const K1Smem& s, const uint2* __restri
       // O0 / Q4: out of range -> ignored + flagged (pad >= n_pads[row] is caught by K5, where the row is uniform)
       const bool valid = sec < S && row < R && t < T;
       bad |= !valid;
-      vm |= valid ? (1u << k) : 0u;
       q = q > 1023u ? 1023u : q;                                  // Q4: clamp
-      const bool ok = valid && q != 0u;                           // Q4: zero charge ignored
+      // Q4: a digit with charge 0 is ignored -- but O0 tests its range first, and the pad is only known to be
+      // in range in K5: such a digit travels there as a record with q = 0, is checked and dropped.  Only the
+      // all-zero word (charge 0 at sector 0, row 0, pad 0, time 0: in range, nothing to flag; also what the
+      // padding behind the input's end reads as) ends here.  Zero suppression makes both cases rare upstream.
+      const bool ok = valid && (w0 | w1) != 0u;
       u32 tc = 0u, v = t;
       if (MULTI_TC) { tc = t / TPC_TC; v = t - tc * TPC_TC; }
       const u32 b0 = MULTI_TC ? (sec * R + row) * NTC + tc : sec * R + row;
@@ -381,16 +383,6 @@ __device__ __forceinline__ void k1_rounds(const K1Smem& s, const uint2* __restri
         } else if (ok && v + TPC_HALO >= TPC_TC && tc + 1u < NTC) {
           dbin[k] = b0 + 1u; drec[k] = pad | ((v + TPC_HALO - TPC_TC) << 8) | (q << 22); dpend |= 1u << k;
         }
-      }
-    }
-    // A digit in range with charge 0 is ignored (Q4) and never reaches K5, but O0 tests the range
-    // first: its pad is checked here.  Zero suppression drops such digits upstream, so this branch is
-    // taken for the zero padding behind the input's end and otherwise never: one test per round.
-    if (vm & ~pend) {
-#pragma unroll
-      for (int k = 0; k < TPC_K1_DPT; ++k) {
-        const u32 w0 = (k & 1) ? curd[k >> 1].z : curd[k >> 1].x, w1 = (k & 1) ? curd[k >> 1].w : curd[k >> 1].y;
-        if (((vm & ~pend) >> k & 1u) && (w0 | w1) != 0u && (w1 & 0xFFu) >= PRM_NPADS((w1 >> 8) & 0xFFu)) bad = true;
       }
     }
   };
@@ -584,7 +576,10 @@ k_dir_fill(const u32* __restrict__ dir, const u32* __restrict__ used, u32 slice_
   const u32 id0 = blockIdx.x * slice_cap;
   // (bound by the scattered 4-byte stores: eight directory loads in flight per thread changed nothing)
   for (u32 c = threadIdx.x; c < n; c += TPC_SCAN_THREADS)
-    chunk_list[atomicAdd(&smem_u32[dir[id0 + c] >> 8], 1u)] = id0 + c;
+  {   // entry = chunk id [0:26) | (records - 1) [26:32): K5 gets the count with the id instead of from a scattered 4-byte read of dir[]
+    const u32 d = dir[id0 + c];
+    chunk_list[atomicAdd(&smem_u32[d >> 8], 1u)] = (id0 + c) | (((d & 0xFFu) - 1u) << 26);
+  }
 }
 #endif
 
@@ -740,6 +735,11 @@ k_emit_packed(const uint4* __restrict__ temp, const u64* __restrict__ tile_base,
 // tl >= TPC_TT means "not mine".  Tile sl OWNS rows tl in [3, TS+3).
 // ==========================================================================================
 
+// sort key of a record with u = slab * TS + m: 2 * slab + (m >= 2 HALO).  For 128-bin slabs without a compare:
+// (u >> 7) + ((u + 128 - 2 HALO) >> 7), the second term being slab + (m >= 2 HALO).
+__device__ __forceinline__ u32 k5_key(u32 u) {
+  return TPC_TS == 128u ? (u >> 7) + ((u + 128u - 2u * TPC_HALO) >> 7) : 2u * (u / TPC_TS) + ((u % TPC_TS) >= 2u * TPC_HALO ? 1u : 0u);
+}
 #if TPC_UNITS & TPC_U_PART_FINE
 extern "C" __global__ void __launch_bounds__(TPC_K5_THREADS, 1)
 k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, const u32* __restrict__ chunk_list,
@@ -783,8 +783,9 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
       const u32 sub = (threadIdx.x + (u32)i * TPC_K5_THREADS) & 15u;
-      v[i] = make_uint4(0u, 0u, 0u, 0u); nrec[i] = 0u;
-      if (cid[i] != 0xFFFFFFFFu) { nrec[i] = dir[cid[i]] & 0xFFu; v[i] = ld_stream_u4(pool + (u64)cid[i] * 16u + sub); }
+      v[i] = make_uint4(0u, 0u, 0u, 0u);
+      nrec[i] = cid[i];   // the count sits in the entry's top bits; decoded where it is used (measured: 4.93 -> 4.66 ms against decoding it here)
+      if (cid[i] != 0xFFFFFFFFu) v[i] = ld_stream_u4(pool + (u64)(cid[i] & 0x03FFFFFFu) * 16u + sub);
     }
   };
   Batch cur_b, nxt_b;
@@ -817,7 +818,7 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
       const u32 sub = (threadIdx.x + (u32)i * TPC_K5_THREADS) & 15u;
       // K1 writes whole 32-byte sectors and zero-fills the last one: a piece is valid or not as a whole
       uint4 v = vn[i];
-      if (sub * 4u >= nrecn[i]) v = make_uint4(0u, 0u, 0u, 0u);
+      if (nrecn[i] == 0xFFFFFFFFu || sub * 4u >= (nrecn[i] >> 26) + 1u) v = make_uint4(0u, 0u, 0u, 0u);
       u32 r4[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
@@ -826,7 +827,7 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
         u32 rk = 0u;
         {
           const u32 u = (r >> 8) & 0x3FFFu;
-          const u32 key = r != 0u ? 2u * (u / TPC_TS) + ((u % TPC_TS) >= 2u * TPC_HALO ? 1u : 0u) : 0xFFFFFFFFu;   // <= 2 * nsl (u < TC + 6)
+          const u32 key = r != 0u ? k5_key(u) : 0xFFFFFFFFu;   // <= 2 * nsl (u < TC + 2 HALO)
           // time-ordered input (readout order) puts the 32 records of a warp step into ONE run: then a
           // single atomic serves the warp; otherwise (shuffled input: ~28 different keys) one per record
           int same = 0;
@@ -885,10 +886,12 @@ k_partition_fine(const uint4* __restrict__ pool, const u32* __restrict__ dir, co
       const u32 r = rec[k];
       if (r != 0u) {
         const u32 u = (r >> 8) & 0x3FFFu;
-        const u32 sl1 = u / TPC_TS, m = u % TPC_TS;
-        const u32 key = 2u * sl1 + (m >= 2u * TPC_HALO ? 1u : 0u);
+        const u32 key = k5_key(u);
         const u32 rk = (rank[k >> 1] >> ((k & 1) * 16)) & 0xFFFFu;
-        buf[s_off[key] + rk] = (r & 0xFFu) | ((m | ((sl1 & 1u) << 7)) << 8) | ((r >> 22) << 16);
+        // tile record: pad | (m | parity << 7) << 8 | q << 16.  With 128-bin slabs m | parity << 7 is simply the low byte of u,
+        // which already sits in bits [8:16) of the coarse record
+        const u32 f = TPC_TS == 128u ? (r & 0xFFFFu) : ((r & 0xFFu) | (((u % TPC_TS) | (((u / TPC_TS) & 1u) << 7)) << 8));
+        buf[s_off[key] + rk] = f | ((r >> 22) << 16);
       }
     }
     if (threadIdx.x >= TPC_K5_THREADS - TPC_NKEY) s_cnt[threadIdx.x - (TPC_K5_THREADS - TPC_NKEY)] = 0u;   // for the next batch
@@ -1228,14 +1231,14 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
         if (nu * 4u <= TPC_K6_CONSUMERS) {   // a sparse tile: one record per thread, spread over all warps
           const u32 r = tid < nu * 4u ? rec[tid] : 0u;
           const u32 tl = k6_row(r, sl);
-          if (r != 0u && tl < TPC_TT) { s.tile[tl * pitch + (r & 0xFFu) + TPC_PG] = (u16)((r >> 16) & 0x3FFu); my_r = r; }
+          if (r >= (1u << 16) && tl < TPC_TT) { s.tile[tl * pitch + (r & 0xFFu) + TPC_PG] = (u16)((r >> 16) & 0x3FFu); my_r = r; }   // (q = 0: Q4, ignored)
         } else
         for (u32 u = tid; u < nu; u += TPC_K6_CONSUMERS) {
           const uint4 v = r4[u];
           const u32 rr[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
           for (int k = 0; k < 4; ++k)
-            if (rr[k] != 0u) {   // 0 = batch padding (every real record has q >= 1)
+            if (rr[k] >= (1u << 16)) {   // q >= 1; not batch padding (0) nor a zero-charge digit (Q4: ignored; K5 has checked its range)
               const u32 tl = k6_row(rr[k], sl);
               if (tl < TPC_TT) s.tile[tl * pitch + (rr[k] & 0xFFu) + TPC_PG] = (u16)((rr[k] >> 16) & 0x3FFu);
             }

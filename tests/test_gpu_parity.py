@@ -715,6 +715,21 @@ def test_internal_status_bit_and_zero_charge_bad_pad(tp, cuda_device):
             assert st == st_e and n == len(e) and got.tobytes() == e.tobytes(), (rows, mode)
         c.close()
     assert st_e == 0          # the last case: pad 8 of a 9-pad row is in range
+    # a zero-charge digit on a cell that also holds a real digit is no duplicate: it is ignored (Q4) in both
+    # modes and both orders, in a sparse tile (one record per thread) and in a crowded one
+    rng = np.random.default_rng(5)
+    for n_fill in (0, 900):
+        cells = rng.choice(100 * 12, size=n_fill, replace=False) + 12 * 20
+        rows = [(0, 2, int(c % 12), int(c // 12), int(rng.integers(3, 90))) for c in cells if (int(c % 12), int(c // 12)) != (5, 5)]
+        for pair in ([(0, 2, 5, 5, 0), (0, 2, 5, 5, 40)], [(0, 2, 5, 5, 40), (0, 2, 5, 5, 0)]):
+            dd = t1.make_digits(pair + rows + [(0, 2, 7, 9, 0)])
+            e, st_e = _oracle(dd, 1, 3, 128, pads)
+            c = tp.Clusterizer(1, 3, 128, pads, len(dd))
+            for mode in (tp.MODE_FAST, tp.MODE_DETERMINISTIC, tp.MODE_FAST):
+                got, n, st = c.run_sync(_digits_tensor(dd, cuda_device), mode)
+                assert st == st_e == 0 and n == len(e)
+                assert got[np.argsort(_key(got))].tobytes() == e.tobytes(), (n_fill, mode)
+            c.close()
 
 
 def test_rtc_cache_survives_a_damaged_file(tp, cuda_device, tmp_path):
