@@ -258,7 +258,9 @@ template <int K, bool FIRST, class F = K1Nothing>
 __device__ __forceinline__ bool k1_pass(const K1Smem& s, u32& cur, u32& nsp, const u32 (&bin)[K], const u32 (&rec)[K],
                                         u32 (&slot)[K], u32& pend, u32 slice_base, u32 slice_cap,
                                         uint4* pool, u32* dir, F between = F()) {
-  const u32 lane = lane_id(), warp = threadIdx.x >> 5, lt = (1u << lane) - 1u;
+  u32 tid_ = threadIdx.x;
+  asm volatile("" : "+r"(tid_));   // opaque: read the thread id once instead of re-deriving everything from S2R under register pressure
+  const u32 lane = tid_ & 31u, warp = tid_ >> 5, lt = (1u << lane) - 1u;
   u16* fq = s.fq + warp * TPC_K1_WFQ;
   u32* sp_in = s.spill + ((cur * (TPC_K1_THREADS / 32) + warp) * TPC_K1_WSP) * 2u;
   u32* sp_out = s.spill + (((cur ^ 1u) * (TPC_K1_THREADS / 32) + warp) * TPC_K1_WSP) * 2u;

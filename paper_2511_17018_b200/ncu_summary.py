@@ -95,13 +95,45 @@ def summarise_launches(path: str, tag: str) -> None:
             f.write("%s, %d, %.4f, %.1f %%\n" % (n, len(x), sum(x) / len(x) / 1e6, 100 * sum(x) / len(x) / tot))
 
 
+SASS_PATTERNS = ["UBLKCP", "UBLKPF", "SYNCS", "FENCE.VIEW.ASYNC", "STG.E.ENL2.256", "LDG.E.NA", "VIMNMX", "ATOMS", "ATOMG", "REDG",
+                 "VOTE", "SHFL", "BAR.", "LDS", "STS", "HMMA", "UTC"]
+
+
+def summarise_sass(tag: str) -> None:
+    """Counts of the SASS mnemonics that show what the kernels are made of (bulk copies, mbarriers,
+    packed min/max, shared atomics; no tensor-core instruction) per kernel, from the unit binaries the
+    build leaves in build/unit_*.cubin (`python -m paper_2511_17018_b200.build`)."""
+    import glob
+    import re
+    out = ["cuobjdump -sass build/unit_<name>.cubin, per kernel: instructions, registers (ptxas), and occurrences of the mnemonics",
+           "that matter (UBLKCP/UBLKPF = cp.async.bulk / prefetch, SYNCS = mbarrier, VIMNMX = packed u16x2 max, ENL2.256 = 32-byte store)", ""]
+    for cub in sorted(glob.glob(os.path.join(ROOT, "build", "unit_*.cubin"))):
+        sass = subprocess.run(["cuobjdump", "-sass", cub], capture_output=True, text=True, check=True).stdout
+        res = subprocess.run(["cuobjdump", "-res-usage", cub], capture_output=True, text=True).stdout
+        regs = dict(re.findall(r"Function (\w+):\s*\n\s*REG:(\d+)", res))
+        out.append("== %s (arch %s)" % (os.path.basename(cub), ",".join(sorted(set(re.findall(r"code for (sm_\w+)", sass))))))
+        for fn, body in re.findall(r"Function : (\w+)\n(.*?)(?=\n\s*Function : |\Z)", sass, flags=re.S):
+            ins = re.findall(r"^\s+/\*[0-9a-f]{4,}\*/\s+(.*?);", body, flags=re.M)
+            counts = []
+            for pat in SASS_PATTERNS:
+                n = sum(1 for x in ins if pat in x)
+                if n:
+                    counts.append("%s %d" % (pat, n))
+            out.append("  %-34s %5d instructions, %s registers | %s" % (fn, len(ins), regs.get(fn, "?"), ", ".join(counts)))
+    with open(os.path.join(ROOT, "profiles", "%s_sass_summary.txt" % tag), "w") as f:
+        f.write("\n".join(out) + "\n")
+
+
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--tag", required=True)
     ap.add_argument("--rep")
     ap.add_argument("--launches")
     ap.add_argument("--note", default="CFG[4] shuffled FAST generic")
+    ap.add_argument("--sass", action="store_true", help="write profiles/<tag>_sass_summary.txt from build/unit_*.cubin")
     a = ap.parse_args()
+    if a.sass:
+        summarise_sass(a.tag)
     if a.rep:
         print(json.dumps(summarise_rep(a.rep, a.tag, a.note)["traffic_bytes"]))
     if a.launches:
