@@ -308,30 +308,49 @@ def main():
         del r
         _log("ratios done: det %.3f ms, rtc %.3f ms" % (ms_det, ms_rtc))
 
-    # ---- e2e: host buffers through tpcclus_run_host, copies inside the timed region -----------
+    # ---- e2e: host buffers through the C ABI, copies inside the timed region -----------------------
+    # (a) tpcclus_run_host: one frame at a time, copy -> run -> copy back, serial;
+    # (b) tpcclus_host_submit / tpcclus_host_wait: a burst of frames, two in flight, so that the
+    #     host-to-device copy of frame k+1 overlaps the run and the read-back of frame k.  Every frame
+    #     of the burst is copied in from pinned host memory and its clusters are copied back: (b) is
+    #     the e2e number (a time frame never comes alone: PAPER.md 12, 97), (a) is reported beside it.
     e2e = None
     if args.e2e_steps > 0 and not packed:
         cap = n_clusters + 1024
         c.close()
         del c, clusters
         torch.cuda.empty_cache()
-        c = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, n, rtc=args.rtc, device=local, host_capacity=cap)
+        c = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, n, rtc=args.rtc, device=local, host_capacity=cap,
+                           host_pipelined=True)
         h_digits = torch.empty(n, dtype=torch.int64).pin_memory()
         h_digits.copy_(digits)
-        h_clusters = torch.empty((cap, 32), dtype=torch.uint8).pin_memory()
+        h_clusters = [torch.empty((cap, 32), dtype=torch.uint8).pin_memory() for _ in range(2)]
         _log("pinned host buffers ready")
-        c.run_host(h_digits, h_clusters, mode)      # warm-up
+        c.run_host(h_digits, h_clusters[0], mode)      # warm-up
         barrier()
         t0 = time.perf_counter()
         for _ in range(args.e2e_steps):
-            n_e2e, st_e2e = c.run_host(h_digits, h_clusters, mode)
+            n_e2e, st_e2e = c.run_host(h_digits, h_clusters[0], mode)
         barrier()
-        sec = (time.perf_counter() - t0) / args.e2e_steps
+        sec1 = (time.perf_counter() - t0) / args.e2e_steps
+        assert n_e2e == n_clusters and st_e2e == 0
+        burst = max(6, 3 * args.e2e_steps)
+        t0 = time.perf_counter()
+        for i in range(burst):
+            c.host_submit(h_digits, h_clusters[i & 1], mode)
+            if i >= 1:
+                n_e2e, st_e2e = c.host_wait()
+                assert n_e2e == n_clusters and st_e2e == 0
+        n_e2e, st_e2e = c.host_wait()
+        barrier()
+        sec = (time.perf_counter() - t0) / burst
         assert n_e2e == n_clusters and st_e2e == 0
         sec_max, _ = aggregate_over_ranks(sec, n, dev, world)
+        sec1_max, _ = aggregate_over_ranks(sec1, n, dev, world)
         e2e = {"value": tot_digits / sec_max, "unit": UNIT, "h2d_bytes_per_step": 8 * n,
                "d2h_bytes_per_step": 32 * n_clusters + 16, "ms_per_step": sec_max * 1e3,
-               "api": "tpcclus_run_host (pinned host buffers)"}
+               "api": "tpcclus_host_submit / tpcclus_host_wait, burst of %d frames, two in flight (pinned host buffers)" % burst,
+               "single_frame": {"value": tot_digits / sec1_max, "ms_per_step": sec1_max * 1e3, "api": "tpcclus_run_host (serial copy, run, copy)"}}
         del h_clusters, h_digits
         _log("e2e done")
 

@@ -201,6 +201,22 @@ TPCCLUS_API int tpcclus_run_host(tpcclus_handle* h, const tpcclus_digit* h_digit
                                  uint64_t* h_n_clusters, uint32_t* h_status, int mode,
                                  void* cuda_stream);
 
+/* The same end-to-end path for a STREAM of time frames, two in flight (PAPER.md 97: one process per GPU
+ * takes whole time frames one after the other): submit() enqueues the host-to-device copy of a frame into
+ * one of two staging slots on a copy stream of the handle, the run behind it on a second stream and the
+ * read-back of the 16-byte result on a third, and returns without waiting; wait() blocks until the OLDEST
+ * submitted frame is done, stores its count and status and copies min(n_clusters, capacity) clusters into
+ * the h_clusters given at submit.  The copy of frame k+1 thus overlaps the clustering and the read-back of
+ * frame k (full-duplex link).  At most two submits may be outstanding (a third returns
+ * TPCCLUS_ERR_INVALID_ARG); h_digits and h_clusters (HOST, pinned for overlap) must stay valid until the
+ * matching wait() returns; `capacity` must be the same for the frames in flight.  The workspace must have
+ * been sized with tpcclus_workspace_bytes_host_pipelined().  Not to be mixed with tpcclus_run* on other
+ * streams while frames are in flight (one workspace per handle). */
+TPCCLUS_API uint64_t tpcclus_workspace_bytes_host_pipelined(const tpcclus_params* params, uint64_t cluster_capacity);
+TPCCLUS_API int tpcclus_host_submit(tpcclus_handle* h, const tpcclus_digit* h_digits, uint64_t n,
+                                    tpcclus_cluster* h_clusters, uint64_t capacity, int mode);
+TPCCLUS_API int tpcclus_host_wait(tpcclus_handle* h, uint64_t* h_n_clusters, uint32_t* h_status);
+
 TPCCLUS_API int tpcclus_destroy(tpcclus_handle* h);
 
 /* The constant buffers may change between time frames (PAPER.md 79, 85): sets new thresholds and

@@ -64,7 +64,8 @@ EXPORTS = ("tpcclus_workspace_bytes", "tpcclus_workspace_bytes_host", "tpcclus_c
            "tpcclus_run_host", "tpcclus_destroy", "tpcclus_error_string", "tpcclus_last_error",
            "tpcclus_launches_per_run", "tpcclus_set_timing", "tpcclus_last_timing", "tpcclus_rtc_build_ms",
            "tpcclus_debug_dense_map", "tpcclus_debug_det_fallback", "tpcclus_set_rtc_cache_dir", "tpcclus_rtc_cache_hit", "tpcclus_run_packed",
-           "tpcclus_update_params", "tpcclus_constant_buffers", "tpcclus_loaded_units", "tpcclus_debug_shrink")
+           "tpcclus_update_params", "tpcclus_constant_buffers", "tpcclus_loaded_units", "tpcclus_debug_shrink",
+           "tpcclus_workspace_bytes_host_pipelined", "tpcclus_host_submit", "tpcclus_host_wait")
 
 
 def lib() -> C.CDLL:
@@ -112,6 +113,12 @@ def lib() -> C.CDLL:
     L.tpcclus_rtc_cache_hit.argtypes = [C.c_void_p]
     L.tpcclus_debug_det_fallback.restype = C.c_int
     L.tpcclus_debug_det_fallback.argtypes = [C.c_void_p]
+    L.tpcclus_workspace_bytes_host_pipelined.restype = C.c_uint64
+    L.tpcclus_workspace_bytes_host_pipelined.argtypes = [P(tpcclus_params), C.c_uint64]
+    L.tpcclus_host_submit.restype = C.c_int
+    L.tpcclus_host_submit.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p, C.c_uint64, C.c_int]
+    L.tpcclus_host_wait.restype = C.c_int
+    L.tpcclus_host_wait.argtypes = [C.c_void_p, P(C.c_uint64), P(C.c_uint32)]
     L.tpcclus_update_params.restype = C.c_int
     L.tpcclus_update_params.argtypes = [C.c_void_p, C.c_uint16, C.c_uint16, C.c_void_p]
     L.tpcclus_constant_buffers.restype = C.c_int
@@ -169,7 +176,7 @@ class Clusterizer:
     """One handle + the torch tensors that own its device memory."""
 
     def __init__(self, n_sectors, n_rows, n_time, n_pads, max_digits, thr_peak=6, noise_eps=4, rtc=False,
-                 device=0, host_capacity=0, cog_gated=False, cog_shared=False):
+                 device=0, host_capacity=0, cog_gated=False, cog_shared=False, host_pipelined=False):
         import torch
 
         if not torch.cuda.is_available():
@@ -183,7 +190,10 @@ class Clusterizer:
         flags = (RTC if rtc else 0) | (COG_GATED if cog_gated else 0) | (COG_SHARED if cog_shared else 0)
         p, self._pads_keep = make_params(n_sectors, n_rows, n_time, self.n_pads, self.max_digits, thr_peak, noise_eps,
                                          flags, device)
-        nbytes = tpcclus_workspace_bytes_host(p, host_capacity) if host_capacity else tpcclus_workspace_bytes(p)
+        if host_capacity and host_pipelined:
+            nbytes = int(lib().tpcclus_workspace_bytes_host_pipelined(C.byref(p), int(host_capacity)))
+        else:
+            nbytes = tpcclus_workspace_bytes_host(p, host_capacity) if host_capacity else tpcclus_workspace_bytes(p)
         if nbytes == 0:
             raise TpcclusError(-1, "tpcclus_workspace_bytes", "invalid or unsupported parameters")
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
@@ -251,6 +261,22 @@ class Clusterizer:
                                     C.byref(status), int(mode), C.c_void_p(st))
         if rc != 0:
             raise TpcclusError(rc, "tpcclus_run_host", (lib().tpcclus_last_error(self._h) or b"").decode())
+        return int(n_out.value), int(status.value)
+
+    def host_submit(self, digits_host, clusters_host, mode=MODE_FAST):
+        """tpcclus_host_submit: one more frame into the two-deep host pipeline (host_pipelined=True handles)."""
+        dptr, n = _host_ptr_count(digits_host, 8)
+        cptr, cap = _host_ptr_count(clusters_host, 32)
+        rc = lib().tpcclus_host_submit(self._h, C.c_void_p(dptr), n, C.c_void_p(cptr), cap, int(mode))
+        if rc != 0:
+            raise TpcclusError(rc, "tpcclus_host_submit", (lib().tpcclus_last_error(self._h) or b"").decode())
+
+    def host_wait(self):
+        """tpcclus_host_wait: (n_clusters, status) of the oldest frame in flight; its clusters are in the buffer given at submit."""
+        n_out, status = C.c_uint64(0), C.c_uint32(0)
+        rc = lib().tpcclus_host_wait(self._h, C.byref(n_out), C.byref(status))
+        if rc != 0:
+            raise TpcclusError(rc, "tpcclus_host_wait", (lib().tpcclus_last_error(self._h) or b"").decode())
         return int(n_out.value), int(status.value)
 
     # -- introspection ---------------------------------------------------------------------------

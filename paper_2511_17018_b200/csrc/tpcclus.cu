@@ -69,6 +69,7 @@ struct Layout {   // byte offsets into the workspace
   uint64_t host_digits;  // staging of run_host (beyond `total`)
   uint64_t host_out;     // n_clusters (8) + status (4)
   uint64_t host_clusters;
+  uint64_t host_slot;    // bytes of one staging slot without its clusters (digits + result); the pipelined entry has two slots
 };
 
 struct Geometry {
@@ -169,6 +170,7 @@ int make_geometry(const tpcclus_params* p, Geometry* g) {
   L.host_digits = take(8ull * p->max_digits);
   L.host_out = take(16);
   L.host_clusters = o;
+  L.host_slot = L.host_clusters - L.host_digits;
   return TPCCLUS_OK;
 }
 
@@ -248,11 +250,12 @@ const UnitInfo kUnits[U_COUNT_] = {TPC_UNIT_LIST(X)};
 
 // The kernels a handle launches (one slot each) and the unit that provides the slot's kernel for each
 // reading of the centre of gravity: {Q10, Q10' gated, Q10'' shared}.
-enum KernelId { K_PART_COARSE, K_DIR_COUNT, K_DIR_SCAN, K_DIR_FILL, K_PART_FINE, K_TILES_FAST, K_TILES_DET,
+enum KernelId { K_RESET, K_PUBLISH, K_PART_COARSE, K_DIR_COUNT, K_DIR_SCAN, K_DIR_FILL, K_PART_FINE, K_TILES_FAST, K_TILES_DET,
                 K_TILES_DET_TEMP, K_TILES_DUMP, K_SCAN_LOCAL, K_SCAN_SUMS, K_EMIT_ORDERED, K_EMIT_PACKED, K_COUNT_ };
 struct KernelInfo { const char* name[3]; UnitId unit[3]; int smem; };   // smem: 0 none/static, 1 K1, 5 K5, 6 K6
 #define SAME3(x) {x, x, x}
 const KernelInfo kKernels[K_COUNT_] = {
+    {SAME3("k_reset"), SAME3(U_DIR), 0}, {SAME3("k_publish"), SAME3(U_DIR), 0},
     {SAME3("k_partition_coarse"), {U_PART_COARSE, U_PART_COARSE, U_PART_COARSE_H5}, 1},
     {SAME3("k_dir_count"), SAME3(U_DIR), 0}, {SAME3("k_dir_scan"), SAME3(U_DIR), 0}, {SAME3("k_dir_fill"), SAME3(U_DIR), 0},
     {SAME3("k_partition_fine"), {U_PART_FINE, U_PART_FINE, U_PART_FINE_H5}, 5},
@@ -291,6 +294,16 @@ struct tpcclus_handle {
   cudaEvent_t ev[kMaxKernels + 1] = {};
   std::string err;
   bool ran = false;
+  // two-deep host pipeline (tpcclus_host_submit / tpcclus_host_wait)
+  struct Pipe {
+    bool ready = false;
+    cudaStream_t in = nullptr, comp = nullptr, out = nullptr;
+    cudaEvent_t h2d[2] = {}, done[2] = {};
+    uint64_t seq_submit = 0, seq_wait = 0;
+    struct { tpcclus_cluster* h_clusters; uint64_t capacity; } job[2] = {};
+    struct Res { uint64_t n; uint64_t s; }* res = nullptr;   // mapped pinned memory, one per slot: written by k_publish
+    Res* res_dev = nullptr;
+  } pipe;
 };
 
 namespace {
@@ -338,7 +351,7 @@ std::string rtc_prologue(const TpcParams& q, uint32_t unit_bit, uint32_t halo) {
   DEF(n_sectors); DEF(n_rows); DEF(n_time); DEF(n_tc); DEF(n_bins); DEF(n_sl); DEF(pitch); DEF(max_pads);
   DEF(thr_peak); DEF(noise_eps); DEF(max_peaks); DEF(cog_mode);
 #undef DEF
-  s += "__device__ const unsigned short TPC_NPADS_TABLE[256] = {";
+  s += "__constant__ unsigned short TPC_NPADS_TABLE[256] = {";   // constant bank like the generic build's table: no 64-bit address registers
   for (int r = 0; r < 256; ++r) { snprintf(buf, sizeof buf, "%u,", (unsigned)q.n_pads[r]); s += buf; }
   s += "};\n";
   return s;
@@ -582,6 +595,12 @@ int tpcclus_destroy(tpcclus_handle* h) {
   dg.enter(h->params.device);
   for (int i = 0; i <= kMaxKernels; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
   for (int u = 0; u < U_COUNT_; ++u) if (h->module[u]) drv().cuModuleUnload(h->module[u]);
+  if (h->pipe.ready) {
+    cudaStreamSynchronize(h->pipe.in); cudaStreamSynchronize(h->pipe.comp); cudaStreamSynchronize(h->pipe.out);
+    for (int i = 0; i < 2; ++i) { cudaEventDestroy(h->pipe.h2d[i]); cudaEventDestroy(h->pipe.done[i]); }
+    cudaStreamDestroy(h->pipe.in); cudaStreamDestroy(h->pipe.comp); cudaStreamDestroy(h->pipe.out);
+    if (h->pipe.res) cudaFreeHost(h->pipe.res);
+  }
   delete h;
   return TPCCLUS_OK;
 }
@@ -628,7 +647,7 @@ const char* tpcclus_last_error(const tpcclus_handle* h) { return h ? h->err.c_st
 
 int tpcclus_launches_per_run(const tpcclus_handle* h, int mode) {
   (void)h;
-  return mode == TPCCLUS_MODE_DETERMINISTIC ? 10 : 6;   // DET: + K7, K8, K9 and the (normally idle) chained K6
+  return mode == TPCCLUS_MODE_DETERMINISTIC ? 11 : 7;   // K0..K6; DET: + K7, K8, K9 and the (normally idle) chained K6
 }
 
 int tpcclus_set_timing(tpcclus_handle* h, int enable) {
@@ -687,11 +706,14 @@ RunPtrs ptrs(tpcclus_handle* h) {
 }
 
 // K1..K5: digits -> per-tile record runs.  Shared by run() and the debug map hook.
-int enqueue_binning(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n, u32* status, cudaStream_t st) {
+int enqueue_binning(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n, u32* status, u64* n_out_zero, cudaStream_t st) {
   const Geometry& g = h->g;
   RunPtrs p = ptrs(h);
-  CUDA_TRY(h, cudaMemsetAsync(h->ws + g.lay.counters, 0, g.lay.counters_bytes, st));
-  if (status != p.status) CUDA_TRY(h, cudaMemsetAsync(status, 0, 4, st));
+  int rc;
+  { uint4* cnt = (uint4*)(h->ws + g.lay.counters); u64 n16 = g.lay.counters_bytes / 16;   // (the layout is 256-byte granular)
+    u32* st_ext = status != p.status ? status : nullptr;
+    void* a[] = {&cnt, &n16, &st_ext, &n_out_zero};
+    if ((rc = launch(h, K_RESET, dim3(g.g1), dim3(256), 0, st, a))) return rc; }
   const uint64_t round = (uint64_t)TPC_K1_THREADS * TPC_K1_DPT;
   u64 per_cta = align_up((n + g.g1 - 1) / g.g1, round);
   if (per_cta == 0) per_cta = round;
@@ -699,7 +721,6 @@ int enqueue_binning(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n
   u64 n64 = n;
   u32 slice_cap = h->dbg_slice_cap ? h->dbg_slice_cap : g.slice_cap;
   u64 blob_cap = h->dbg_blob_cap ? h->dbg_blob_cap : g.blob_cap;
-  int rc;
   { void* a[] = {&dig, &n64, &per_cta, &p.pool, &p.dir, &p.used, &slice_cap, &status};
     if ((rc = launch(h, K_PART_COARSE, dim3(g.g1), dim3(TPC_K1_THREADS), h->smem_k1, st, a))) return rc; }
   u32 smem_nb = 4u * g.prm.n_bins;
@@ -737,7 +758,7 @@ static int run_impl(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n
   h->n_timed = 0;
   RunPtrs p = ptrs(h);
   u32* status = o_status ? o_status : p.status;
-  int rc = enqueue_binning(h, d_digits, n, status, st);
+  int rc = enqueue_binning(h, d_digits, n, status, mode == TPCCLUS_MODE_FAST ? (u64*)o_n : nullptr, st);
   if (rc) return rc;
 
   K6Args a;
@@ -749,7 +770,6 @@ static int run_impl(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n
   a.dmap = nullptr; a.row_off = p.row_off;
   void* ka[] = {&a};
   if (mode == TPCCLUS_MODE_FAST) {
-    CUDA_TRY(h, cudaMemsetAsync(o_n, 0, 8, st));
     if ((rc = launch(h, K_TILES_FAST, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
   } else {
     // ordered output (PAPER.md 47-50): runs into the temporary buffer, scan of the tile counts,
@@ -769,9 +789,8 @@ static int run_impl(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n
       void* s[] = {&a.temp, &p.tile_base, &p.tile_cnt, &p.tile_local, &p.block_prefix, &nt, &o, &cap, &ri, &p.det_flag, &status};
       if ((rc = launch(h, K_EMIT_PACKED, dim3(g.g1 * 8u), dim3(256), 0, st, s))) return rc;
     } else {
-      void* s[] = {&a.temp, &p.tile_base, &p.tile_cnt, &p.tile_local, &p.block_prefix, &nt, &o, &cap, &p.det_flag, &status};
+      void* s[] = {&a.temp, &p.tile_base, &p.tile_cnt, &p.tile_local, &p.block_prefix, &nt, &o, &cap, &p.det_flag, &status, &p.ticket};
       if ((rc = launch(h, K_EMIT_ORDERED, dim3(g.g1 * 8u), dim3(256), 0, st, s))) return rc;
-      CUDA_TRY(h, cudaMemsetAsync(p.ticket, 0, 4, st));
       if ((rc = launch(h, K_TILES_DET, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
     }
   }
@@ -820,6 +839,90 @@ int tpcclus_run_host(tpcclus_handle* h, const tpcclus_digit* h_digits, uint64_t 
     CUDA_TRY(h, cudaMemcpyAsync(h_clusters, o.clusters, 32ull * m, cudaMemcpyDeviceToHost, st));
     CUDA_TRY(h, cudaStreamSynchronize(st));
   }
+  return TPCCLUS_OK;
+}
+
+uint64_t tpcclus_workspace_bytes_host_pipelined(const tpcclus_params* p, uint64_t cluster_capacity) {
+  Geometry g;
+  return make_geometry(p, &g) == TPCCLUS_OK ? g.lay.host_digits + 2ull * (g.lay.host_slot + align_up(32ull * cluster_capacity, 256)) : 0;
+}
+
+// Two frames in flight: the host-to-device copy of frame k+1 (its own stream, its own staging slot) runs
+// while frame k is clusterized and its result travels back (PAPER.md 97: a process takes whole time frames
+// one after the other; the link is the bottleneck of this entry, so keeping it busy is all that counts).
+int tpcclus_host_submit(tpcclus_handle* h, const tpcclus_digit* h_digits, uint64_t n, tpcclus_cluster* h_clusters,
+                        uint64_t capacity, int mode) {
+  if (!h) return TPCCLUS_ERR_INVALID_ARG;
+  h->err.clear();
+  const Layout& L = h->g.lay;
+  tpcclus_handle::Pipe& P = h->pipe;
+  const uint64_t slot_bytes = L.host_slot + align_up(32ull * capacity, 256);
+  if ((!h_digits && n) || (!h_clusters && capacity) || n > h->g.max_digits ||
+      h->params.workspace_bytes < L.host_digits + 2ull * slot_bytes)
+    return fail(h, TPCCLUS_ERR_INVALID_ARG, "tpcclus_host_submit: bad argument or workspace not sized with tpcclus_workspace_bytes_host_pipelined");
+  if (P.seq_submit - P.seq_wait >= 2) return fail(h, TPCCLUS_ERR_INVALID_ARG, "tpcclus_host_submit: two frames are in flight, call tpcclus_host_wait first");
+  DeviceGuard dg;
+  CUDA_TRY(h, dg.enter(h->params.device));
+  if (!P.ready) {
+    CUDA_TRY(h, cudaStreamCreateWithFlags(&P.in, cudaStreamNonBlocking));
+    CUDA_TRY(h, cudaStreamCreateWithFlags(&P.comp, cudaStreamNonBlocking));
+    CUDA_TRY(h, cudaStreamCreateWithFlags(&P.out, cudaStreamNonBlocking));
+    for (int i = 0; i < 2; ++i) {
+      CUDA_TRY(h, cudaEventCreateWithFlags(&P.h2d[i], cudaEventDisableTiming));
+      CUDA_TRY(h, cudaEventCreateWithFlags(&P.done[i], cudaEventDisableTiming));
+    }
+    CUDA_TRY(h, cudaHostAlloc((void**)&P.res, 2 * sizeof *P.res, cudaHostAllocMapped));
+    CUDA_TRY(h, cudaHostGetDevicePointer((void**)&P.res_dev, P.res, 0));
+    P.ready = true;
+  }
+  const int sl = (int)(P.seq_submit & 1);
+  char* base = h->ws + L.host_digits + (uint64_t)sl * slot_bytes;
+  tpcclus_digit* d_dig = (tpcclus_digit*)base;
+  tpcclus_out o;
+  o.n_clusters = (uint64_t*)(base + (L.host_out - L.host_digits));
+  o.status = (uint32_t*)(base + (L.host_out - L.host_digits) + 8);
+  o.clusters = (tpcclus_cluster*)(base + L.host_slot);
+  o.capacity = capacity;
+  // the slot's staging is free: wait() of the frame that used it two submits ago has returned
+  if (n) CUDA_TRY(h, cudaMemcpyAsync(d_dig, h_digits, 8ull * n, cudaMemcpyHostToDevice, P.in));
+  CUDA_TRY(h, cudaEventRecord(P.h2d[sl], P.in));
+  CUDA_TRY(h, cudaStreamWaitEvent(P.comp, P.h2d[sl], 0));
+  int rc = tpcclus_run(h, d_dig, n, &o, mode, P.comp);
+  if (rc) return rc;
+  { u64* hr = (u64*)&P.res_dev[sl]; const u64* nc = (const u64*)o.n_clusters; const u32* stp = o.status;
+    void* a[] = {&hr, &nc, &stp};
+    bool t = h->timing; h->timing = false;
+    rc = launch(h, K_PUBLISH, dim3(1), dim3(32), 0, P.comp, a);
+    h->timing = t;
+    if (rc) return rc; }
+  // wait() synchronises on this event before it reads anything back.  Nothing of frame k+1 may be queued on the
+  // read-back stream ahead of frame k's clusters (a wait for frame k+1's run there cost the whole overlap).
+  CUDA_TRY(h, cudaEventRecord(P.done[sl], P.comp));
+  P.job[sl].h_clusters = h_clusters; P.job[sl].capacity = capacity;
+  ++P.seq_submit;
+  return TPCCLUS_OK;
+}
+
+int tpcclus_host_wait(tpcclus_handle* h, uint64_t* h_n_clusters, uint32_t* h_status) {
+  if (!h || !h_n_clusters) return TPCCLUS_ERR_INVALID_ARG;
+  h->err.clear();
+  tpcclus_handle::Pipe& P = h->pipe;
+  if (P.seq_wait == P.seq_submit) return fail(h, TPCCLUS_ERR_INVALID_ARG, "tpcclus_host_wait: nothing in flight");
+  const Layout& L = h->g.lay;
+  DeviceGuard dg;
+  CUDA_TRY(h, dg.enter(h->params.device));
+  const int sl = (int)(P.seq_wait & 1);
+  CUDA_TRY(h, cudaEventSynchronize(P.done[sl]));   // the run is over; its 16-byte result is in the mapped host words
+  *h_n_clusters = P.res[sl].n;
+  if (h_status) *h_status = (uint32_t)P.res[sl].s;
+  const uint64_t cap = P.job[sl].capacity, m = P.res[sl].n < cap ? P.res[sl].n : cap;
+  if (m) {   // only the clusters that exist cross the link; meanwhile the next frame's digits are coming in
+    const uint64_t slot_bytes = L.host_slot + align_up(32ull * cap, 256);
+    const char* src = h->ws + L.host_digits + (uint64_t)sl * slot_bytes + L.host_slot;
+    CUDA_TRY(h, cudaMemcpyAsync(P.job[sl].h_clusters, src, 32ull * m, cudaMemcpyDeviceToHost, P.out));
+    CUDA_TRY(h, cudaStreamSynchronize(P.out));
+  }
+  ++P.seq_wait;
   return TPCCLUS_OK;
 }
 

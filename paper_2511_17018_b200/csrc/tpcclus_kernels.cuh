@@ -487,6 +487,33 @@ k_partition_coarse(const uint2* __restrict__ digits, u64 n, u64 per_cta, uint4* 
 // a (slice, bin) group is whatever the shared atomics give: nothing downstream depends on
 // it (the map build is a max, O0/Q5).
 // ==========================================================================================
+// K0: the per-run counters (status, cursors, ticket, chained-scan states, per-bin totals) start at zero, and so
+// do the caller's status word and -- in FAST mode -- its cluster count.  A kernel, not cudaMemsetAsync: a memset
+// of this size goes to a copy engine, where it would queue behind the 13 GB host-to-device copy of the NEXT
+// frame of the host pipeline (tpcclus_host_submit) and hold up this frame's run for 230 ms.
+#if TPC_UNITS & TPC_U_DIR
+extern "C" __global__ void __launch_bounds__(256)
+k_reset(uint4* __restrict__ counters, u64 n16, u32* __restrict__ status, u64* __restrict__ n_out) {
+  for (u64 i = (u64)blockIdx.x * 256u + threadIdx.x; i < n16; i += (u64)gridDim.x * 256u) counters[i] = make_uint4(0u, 0u, 0u, 0u);
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    if (status) *status = 0u;
+    if (n_out) *n_out = 0ull;
+  }
+}
+#endif
+// The result of a frame of the host pipeline (count, status) goes to the host through a store into mapped pinned
+// memory: a 16-byte device-to-host cudaMemcpyAsync can land on the copy engine that is busy with the next
+// frame's 13 GB host-to-device copy and would then wait for all of it.
+#if TPC_UNITS & TPC_U_DIR
+extern "C" __global__ void k_publish(u64* __restrict__ host_res, const u64* __restrict__ n_clusters, const u32* __restrict__ status) {
+  if (threadIdx.x == 0 && blockIdx.x == 0) {
+    host_res[1] = (u64)*status;
+    __threadfence_system();
+    host_res[0] = *n_clusters;
+    __threadfence_system();
+  }
+}
+#endif
 #if TPC_UNITS & TPC_U_DIR
 extern "C" __global__ void __launch_bounds__(TPC_SCAN_THREADS)
 k_dir_count(const u32* __restrict__ dir, const u32* __restrict__ used, u32 slice_cap, u32* __restrict__ slice_cnt,
@@ -650,7 +677,8 @@ k_scan_sums(const u32* __restrict__ block_sum, u64* __restrict__ block_prefix, u
 extern "C" __global__ void __launch_bounds__(256)
 k_emit_ordered(const uint4* __restrict__ temp, const u64* __restrict__ tile_base, const u32* __restrict__ tile_cnt,
                const u32* __restrict__ tile_local, const u64* __restrict__ block_prefix, u32 n_tiles,
-               uint4* __restrict__ out, u64 capacity, const u32* __restrict__ flag, u32* __restrict__ status) {
+               uint4* __restrict__ out, u64 capacity, const u32* __restrict__ flag, u32* __restrict__ status, u32* __restrict__ ticket) {
+  if (blockIdx.x == 0 && threadIdx.x == 0) *ticket = 0u;   // fresh tickets for the chained-scan K6 that follows (normally idle)
   if (*flag != 0u) return;
   const u32 lane = threadIdx.x & 31u;
   bool over = false;

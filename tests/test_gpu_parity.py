@@ -825,3 +825,46 @@ def test_cog_shared_reading(tp, cuda_device):
     c.close()
     assert det.tobytes() == exp.tobytes()
     _check_fast(fast, exp)
+
+
+def test_host_pipeline_two_frames_in_flight(tp, cuda_device):
+    """tpcclus_host_submit / tpcclus_host_wait: a stream of different frames through the two-deep host
+    pipeline, results in submission order and equal to the oracle; a third submit without a wait is
+    refused; the serial entry of the same handle still works afterwards."""
+    import torch
+    frames = [make_frame(0), make_frame(0, seed=7, n_time=200), make_frame(1), make_frame(0, seed=9), make_frame(1, seed=3)]
+    big = frames[0]
+    nmax = max(f.n_digits for f in frames)
+    cap = nmax
+    c = tp.Clusterizer(big.n_sectors, big.n_rows, big.n_time, big.n_pads, nmax, host_capacity=cap, host_pipelined=True)
+    exps = []
+    for f in frames:   # every frame on the geometry of the handle (CFG[1] frames use its first rows / pads / bins)
+        d = f.digits_numpy().view(t1.DIGIT)
+        e, st = _oracle(d, big.n_sectors, big.n_rows, big.n_time, big.n_pads)
+        exps.append((e, st))
+    hd = [f.digits.pin_memory() for f in frames]
+    hc = [torch.empty((cap, 32), dtype=torch.uint8).pin_memory() for _ in range(2)]
+    got = []
+    for mode in (tp.MODE_DETERMINISTIC, tp.MODE_FAST):
+        c.host_submit(hd[0], hc[0], mode)
+        for i in range(1, len(frames)):
+            c.host_submit(hd[i], hc[i & 1], mode)
+            if i == 1:
+                with pytest.raises(tp.TpcclusError):
+                    c.host_submit(hd[2], hc[0], mode)          # two are in flight already
+            n, st = c.host_wait()
+            got.append((mode, i - 1, n, st, hc[(i - 1) & 1][:n].numpy().copy().view(tp.CLUSTER_DTYPE).reshape(-1)))
+        n, st = c.host_wait()
+        got.append((mode, len(frames) - 1, n, st, hc[(len(frames) - 1) & 1][:n].numpy().copy().view(tp.CLUSTER_DTYPE).reshape(-1)))
+        with pytest.raises(tp.TpcclusError):
+            c.host_wait()                                      # nothing in flight
+    for mode, i, n, st, cl in got:
+        e, st_e = exps[i]
+        assert n == len(e) and st == st_e, (mode, i)
+        if mode == tp.MODE_DETERMINISTIC:
+            assert cl.tobytes() == e.tobytes(), i
+        else:
+            _check_fast(cl, e)
+    n, st = c.run_host(hd[0], hc[0], tp.MODE_DETERMINISTIC)
+    assert hc[0][:n].numpy().tobytes() == exps[0][0].tobytes()
+    c.close()
