@@ -1781,6 +1781,27 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
         }
         csync();
       }
+      if (total * 4u <= TPC_K6_CONSUMERS) {   // a sparse tile has at most one peak per thread: the clusters are written AFTER
+        const u32 e = tid < npk ? s.peaks[tid] : 0u;   // barrier E, so that nobody waits there for the global atomic
+        const bool keep = tid < npk && (COG == 2 ? owned(e) && survivor(e) : !suppressed(e));
+        const u32 m = __ballot_sync(0xFFFFFFFFu, keep);
+        u64 base = 0ull;
+        if (lane == 0u && m) base = atomicAdd(a.n_clusters, (u64)__popc(m));
+        if (keep) cog_sums(e, o0, o1);
+        csync();   // E
+        if (my_r != 0u) {
+          const u32 tl = k6_row(my_r, sl), pad = my_r & 0xFFu;
+          s.tile[tl * pitch + pad + TPC_PG] = 0;
+          s.pmask[tl * TPC_K6_PMW + ((pad + TPC_PG) >> 5)] = 0u;
+          if (COG == 2) s.rowmask[tl * 8u + (pad >> 5)] = 0u;
+        }
+        if (tid == 0) s.misc[0] = 0u;
+        if (m) {
+          base = __shfl_sync(0xFFFFFFFFu, base, 0);
+          if (keep) emit(base + __popc(m & lt), o0, o1);
+        }
+        continue;
+      }
       for (u32 i0 = (tid >> 5) * 32u; i0 < npk; i0 += TPC_K6_CONSUMERS) {
         const u32 i = i0 + lane;
         const u32 e = i < npk ? s.peaks[i] : 0u;
