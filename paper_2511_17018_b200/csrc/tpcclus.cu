@@ -250,7 +250,7 @@ const UnitInfo kUnits[U_COUNT_] = {TPC_UNIT_LIST(X)};
 
 // The kernels a handle launches (one slot each) and the unit that provides the slot's kernel for each
 // reading of the centre of gravity: {Q10, Q10' gated, Q10'' shared}.
-enum KernelId { K_RESET, K_PUBLISH, K_PART_COARSE, K_DIR_COUNT, K_DIR_SCAN, K_DIR_FILL, K_PART_FINE, K_TILES_FAST, K_TILES_DET,
+enum KernelId { K_RESET, K_PUBLISH, K_PART_COARSE, K_DIR_COUNT, K_DIR_SCAN, K_DIR_FILL, K_PART_FINE, K_TILES_FAST, K_TILES_FAST_E, K_TILES_DET,
                 K_TILES_DET_TEMP, K_TILES_DUMP, K_SCAN_LOCAL, K_SCAN_SUMS, K_EMIT_ORDERED, K_EMIT_PACKED, K_COUNT_ };
 struct KernelInfo { const char* name[3]; UnitId unit[3]; int smem; };   // smem: 0 none/static, 1 K1, 5 K5, 6 K6
 #define SAME3(x) {x, x, x}
@@ -260,6 +260,8 @@ const KernelInfo kKernels[K_COUNT_] = {
     {SAME3("k_dir_count"), SAME3(U_DIR), 0}, {SAME3("k_dir_scan"), SAME3(U_DIR), 0}, {SAME3("k_dir_fill"), SAME3(U_DIR), 0},
     {SAME3("k_partition_fine"), {U_PART_FINE, U_PART_FINE, U_PART_FINE_H5}, 5},
     {{"k_cluster_tiles_fast", "k_cluster_tiles_fast_gated", "k_cluster_tiles_fast_shared"}, {U_TILES_FAST, U_TILES_FAST_G, U_TILES_FAST_S}, 6},
+    // the same with the emitter warp, for sparse frames (reading Q10'' has none: the plain kernel)
+    {{"k_cluster_tiles_fast_e", "k_cluster_tiles_fast_gated_e", "k_cluster_tiles_fast_shared"}, {U_TILES_FAST, U_TILES_FAST_G, U_TILES_FAST_S}, 6},
     {{"k_cluster_tiles_det", "k_cluster_tiles_det_gated", "k_cluster_tiles_det_shared"}, {U_TILES_DET, U_TILES_DET_G, U_TILES_DET_S}, 6},
     {{"k_cluster_tiles_det_temp", "k_cluster_tiles_det_temp_gated", "k_cluster_tiles_det_temp_shared"}, {U_TILES_DET, U_TILES_DET_G, U_TILES_DET_S}, 6},
     {SAME3("k_cluster_tiles_dump_map"), {U_TILES_DUMP, U_TILES_DUMP, U_TILES_DUMP_H5}, 6},
@@ -770,7 +772,10 @@ static int run_impl(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n
   a.dmap = nullptr; a.row_off = p.row_off;
   void* ka[] = {&a};
   if (mode == TPCCLUS_MODE_FAST) {
-    if ((rc = launch(h, K_TILES_FAST, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
+    // the readings Q10 and Q10' run with the emitter warp on sparse frames (K6): it only
+    // serves tiles of at most 256 records, so a frame that averages 512 or more per tile starts without it
+    const bool emitter = h->cog != 2 && n < 512ull * h->g.n_tiles;
+    if ((rc = launch(h, emitter ? K_TILES_FAST_E : K_TILES_FAST, dim3(h->grid_k6), dim3(emitter ? TPC_K6_THREADS_E : TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
   } else {
     // ordered output (PAPER.md 47-50): runs into the temporary buffer, scan of the tile counts,
     // ordered copy.  Should the buffer be too small (more than max_digits/8 clusters) the flag is

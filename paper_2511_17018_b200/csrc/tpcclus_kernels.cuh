@@ -100,6 +100,8 @@ __host__ __device__ inline u32 tpc_k5_smem_bytes() { return (TPC_K5_BUF + 2u * T
 #define TPC_K6_CONSUMERS 256u                   // threads that compute
 #endif
 #define TPC_K6_THREADS (TPC_K6_CONSUMERS + 32u)  // + the producer warp
+#define TPC_K6_THREADS_E (TPC_K6_THREADS + 32u)   // FAST kernels of the readings Q10 and Q10': + the emitter warp (K6, sparse tiles)
+#define TPC_K6_RING 64u                          // clusters in flight between the consumers and the emitter warp
 #ifndef TPC_K6_CAP
 #define TPC_K6_CAP 4096u                         // records staged per round (16 KB)
 #endif
@@ -122,7 +124,7 @@ struct K6Args {
 #define TPC_K6_PMW 9u
 __host__ __device__ inline u32 tpc_k6_smem_bytes(u32 pitch, u32 max_peaks, u32 halo) {   // halo: the TPC_HALO of the handle's units
   const u32 tt = TPC_TS + 2u * halo;
-  return (TPC_K6_CAP + tt * pitch / 2u + 4u + 2u + tt * (8u + TPC_K6_PMW) + tt + 2u + 16u + (max_peaks + 1u) / 2u) * 4u + 128u;
+  return (TPC_K6_CAP + tt * pitch / 2u + TPC_K6_RING * 8u + 4u + 4u + 2u + tt * (8u + TPC_K6_PMW) + tt + 2u + 16u + (max_peaks + 1u) / 2u) * 4u + 128u;
 }
 
 #ifdef TPC_RTC
@@ -1032,6 +1034,8 @@ struct K6Smem {
   u32* pmask;      // [TT][9]  O1 peaks, bit = pad + HALO = the cell's index in its map row
   u32* rowmask;    // [TT][8]  O2 survivors, bit = pad
   u32* rowpre; u32* misc; u16* peaks;
+  uint4* ring;     // [TPC_K6_RING][2] integer sums of a sparse tile's clusters on their way to the emitter warp (FAST)
+  u32* rctl;       // [0] entries reserved  [1] entries consumed  [2] the consumers are done
 };
 // misc: [0] n_peaks  [3] first tile of the stage  [4] tiles in the stage  [5] row | sector << 8 |
 //       n_pads << 16  [6] time of row 0 of the first tile  [7] its slab  [8+2m],[9+2m] offset and
@@ -1040,6 +1044,8 @@ __device__ __forceinline__ K6Smem k6_smem(u32* p) {
   K6Smem s;
   s.rec = p; p += TPC_K6_CAP;
   s.tile32 = p; s.tile = (u16*)p; p += TPC_TT * PRM(pitch) / 2u;
+  s.ring = (uint4*)p; p += TPC_K6_RING * 8u;   // (16-byte aligned: the two areas before it are multiples of 16 bytes)
+  s.rctl = p; p += 4;
   s.bar = (u64*)p; p += 4;
   s.base = (u64*)p; p += 2;
   s.pmask = p; p += TPC_TT * TPC_K6_PMW;   // pmask and rowmask are contiguous: zeroed together
@@ -1116,10 +1122,30 @@ __device__ __forceinline__ u32 k6_stage(const K6Smem& s, const K6Args& a, u64 ib
   return pos;
 }
 
+__device__ __forceinline__ uint4 lds_volatile_u4(const uint4* p) {
+  uint4 v;
+  asm volatile("ld.volatile.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"((u32)__cvta_generic_to_shared(p)) : "memory");
+  return v;
+}
 template <int V> struct TpcInt { static constexpr int v = V; };
+
+// O4: the five exact integer sums of a cluster -> its 32 bytes (IEEE-RN float32 operations only, Q12/Q13).  In:
+// c0 = (Q, Sp, St, Spp), c1 = (Stt, qmax | time << 16, pad | row << 8 | sector << 16 | flags << 24, any).
+__device__ __forceinline__ void k6_finalise(uint4& c0, uint4& c1) {
+  const u32 Q = c0.x, Spp = c0.w, Stt = c1.x;
+  const int Sp = (int)c0.y, St = (int)c0.z;
+  const int Vp = (int)(Q * Spp) - Sp * Sp, Vt = (int)(Q * Stt) - St * St;
+  const float fQ = __uint2float_rn(Q);
+  const float pm = __fadd_rn(__uint2float_rn(c1.z & 0xFFu), __fdiv_rn(__int2float_rn(Sp), fQ));
+  const float tm = __fadd_rn(__uint2float_rn(c1.y >> 16), __fdiv_rn(__int2float_rn(St), fQ));
+  const float sp = __fdiv_rn(__fsqrt_rn(__int2float_rn(Vp)), fQ);
+  const float st = __fdiv_rn(__fsqrt_rn(__int2float_rn(Vt)), fQ);
+  c0 = make_uint4(__float_as_uint(pm), __float_as_uint(tm), __float_as_uint(sp), __float_as_uint(st));
+  c1 = make_uint4(Q, c1.y, c1.z, 0u);
+}
 // COG: the reading of the centre of gravity -- 0 = Q10 (every cell, weight 1), 1 = Q10' (outer ring gated),
 // 2 = Q10'' (charge shared with the surviving peaks on the outer ring; needs TPC_HALO >= 5)
-template <int MODE, int COG>
+template <int MODE, int COG, bool EMIT>
 __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
   const K6Smem s = k6_smem(smem);
   const u32 nb = PRM(n_bins), nsl = PRM(n_sl), pitch = PRM(pitch);
@@ -1137,8 +1163,50 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
     mbar_init(&s.bar[1], TPC_K6_CONSUMERS / 32u);   // empty: one arrive per consumer warp
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  for (u32 i = tid; i < TPC_K6_RING * 2u; i += TPC_K6_CONSUMERS) s.ring[i] = make_uint4(0u, 0u, 0u, 0u);
+  if (tid < 4u) s.rctl[tid] = 0u;
   __syncthreads();
 
+  // The emitter warp (FAST, readings Q10 and Q10'): a sparse tile has its ~4 peaks in ONE warp, and the other
+  // seven waited at barrier E while that warp walked global atomic -> division -> square root -> store (41 % of
+  // the samples of the pp-like frame).  The consumers now leave the integer sums of such a cluster in a ring in
+  // shared memory -- entry i: slot i % RING, valid once word 7 holds its tag i / RING + 1 -- and this warp, which
+  // is outside their barriers, finalises, reserves and writes.  No consumer ever waits for it: a warp that finds
+  // the ring full emits its clusters itself, as the tiles with more than one record per thread always do.
+  // The kernels *_e have the warp; the host launches them when the frame averages less than 512 records per tile.
+  static_assert(!EMIT || (MODE == TPC_MODE_FAST && COG != 2), "the emitter warp serves FAST and the readings Q10, Q10'");
+  if (EMIT && tid >= TPC_K6_CONSUMERS + 32u) {
+    const u32 lane = lane_id();
+    u32 t = 0u;   // entries consumed
+    u32 nap = 100u;
+    for (;;) {
+      const u32 i = t + lane, slot = i % TPC_K6_RING;
+      uint4 c1 = lds_volatile_u4(&s.ring[2u * slot + 1u]);
+      const u32 vm = __ballot_sync(0xFFFFFFFFu, c1.w == i / TPC_K6_RING + 1u);
+      const u32 nv = vm == 0xFFFFFFFFu ? 32u : (u32)__ffs((int)~vm) - 1u;   // the valid entries at the head
+      if (nv == 0u) {
+        if (*(volatile u32*)&s.rctl[2] != 0u && t == *(volatile u32*)&s.rctl[0]) break;   // the consumers are done and nothing is left
+        __nanosleep(nap);
+        if (nap < 1600u) nap *= 2u;
+        continue;
+      }
+      nap = 100u;
+      uint4 c0 = make_uint4(1u, 0u, 0u, 0u);
+      if (lane < nv) c0 = lds_volatile_u4(&s.ring[2u * slot]);
+      __syncwarp();
+      t += nv;
+      u64 base = 0ull;
+      if (lane == 0u) { *(volatile u32*)&s.rctl[1] = t; base = atomicAdd(a.n_clusters, (u64)nv); }   // the slots are free again
+      if (lane < nv) k6_finalise(c0, c1);
+      base = __shfl_sync(0xFFFFFFFFu, base, 0);
+      if (lane < nv) {
+        const u64 o = base + lane;
+        if (o < a.capacity) { a.out[o * 2u] = c0; a.out[o * 2u + 1u] = c1; }
+        else atomicOr(a.status, TPC_STATUS_OVERFLOW);
+      }
+    }
+    return;
+  }
   if (tid >= TPC_K6_CONSUMERS) {
     // ---- producer warp -----------------------------------------------------------------------
     // A ticket = up to TPC_K6_GROUP consecutive slabs of one bin, handed out in increasing order.
@@ -1700,8 +1768,9 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       }
       return true;
     };
-    // O3 + O4 for one surviving peak
-    auto cog_sums = [&](u32 e, uint4& c0, uint4& c1) {
+    // O3 for one surviving peak: the integer sums, (c0, c1) = (Q, Sp, St, Spp), (Stt, words 1 and 2 of the cluster's
+    // second half, 0); O4 = k6_finalise
+    auto cog_int = [&](u32 e, uint4& c0, uint4& c1) {
       const u32 tl = e >> 8, pad = e & 0xFFu;
       const u16* c = s.tile + tl * pitch + pad + TPC_PG;
       // exact integer sums (Q12): per-row partial sums first, so the 25 loads and the adds of
@@ -1746,21 +1815,16 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
           St += (int)rq * dt; Stt += rq * (u32)(dt * dt);
         }
       }
-      const int Vp = (int)(Q * Spp) - Sp * Sp, Vt = (int)(Q * Stt) - St * St;
       const u32 qc = c[0];
       const int t = t_base + (int)tl;
-      const float fQ = __uint2float_rn(Q);
-      const float pm = __fadd_rn(__uint2float_rn(pad), __fdiv_rn(__int2float_rn(Sp), fQ));
-      const float tm = __fadd_rn(__int2float_rn(t), __fdiv_rn(__int2float_rn(St), fQ));
-      const float sp = __fdiv_rn(__fsqrt_rn(__int2float_rn(Vp)), fQ);
-      const float st = __fdiv_rn(__fsqrt_rn(__int2float_rn(Vt)), fQ);
       u32 fl = 0u;
       if (pad < 2u || pad + 2u >= npads) fl |= 1u;
       if (t < 2 || (u32)t + 2u >= PRM(n_time)) fl |= 2u;
       if (qc == 1023u) fl |= 4u;
-      c0 = make_uint4(__float_as_uint(pm), __float_as_uint(tm), __float_as_uint(sp), __float_as_uint(st));
-      c1 = make_uint4(Q, qc | ((u32)t << 16), pad | (row << 8) | (sector << 16) | (fl << 24), 0u);
+      c0 = make_uint4(Q, (u32)Sp, (u32)St, Spp);
+      c1 = make_uint4(Stt, qc | ((u32)t << 16), pad | (row << 8) | (sector << 16) | (fl << 24), 0u);
     };
+    auto cog_sums = [&](u32 e, uint4& c0, uint4& c1) { cog_int(e, c0, c1); k6_finalise(c0, c1); };
     auto emit = [&](u64 slot, const uint4& c0, const uint4& c1) {
       if (MODE == TPC_MODE_DET_TEMP) {
         if (slot < a.temp_cap) { a.temp[slot * 2u] = c0; a.temp[slot * 2u + 1u] = c1; }
@@ -1786,8 +1850,31 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
         const bool keep = tid < npk && (COG == 2 ? owned(e) && survivor(e) : !suppressed(e));
         const u32 m = __ballot_sync(0xFFFFFFFFu, keep);
         u64 base = 0ull;
-        if (lane == 0u && m) base = atomicAdd(a.n_clusters, (u64)__popc(m));
-        if (keep) cog_sums(e, o0, o1);
+        u32 ridx = 0xFFFFFFFFu;   // this warp's first entry in the emitter's ring, if it has room
+        if (EMIT && m) {
+          if (lane == 0u) {
+            const u32 n = (u32)__popc(m);
+            for (;;) {
+              const u32 h = *(volatile u32*)&s.rctl[0];
+              if (h + n - *(volatile u32*)&s.rctl[1] > TPC_K6_RING) break;
+              if (atomicCAS(&s.rctl[0], h, h + n) == h) { ridx = h; break; }
+            }
+          }
+          ridx = __shfl_sync(0xFFFFFFFFu, ridx, 0);
+        }
+        const bool self = m != 0u && ridx == 0xFFFFFFFFu;   // warp-uniform
+        if (lane == 0u && self) base = atomicAdd(a.n_clusters, (u64)__popc(m));
+        if (keep) {
+          cog_int(e, o0, o1);
+          if (self) k6_finalise(o0, o1);
+          else {
+            const u32 i = ridx + __popc(m & lt), slot = i % TPC_K6_RING;
+            o1.w = i / TPC_K6_RING + 1u;
+            s.ring[2u * slot] = o0;
+            __threadfence_block();
+            s.ring[2u * slot + 1u] = o1;
+          }
+        }
         csync();   // E
         if (my_r != 0u) {
           const u32 tl = k6_row(my_r, sl), pad = my_r & 0xFFu;
@@ -1796,7 +1883,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
           if (COG == 2) s.rowmask[tl * 8u + (pad >> 5)] = 0u;
         }
         if (tid == 0) s.misc[0] = 0u;
-        if (m) {
+        if (self) {
           base = __shfl_sync(0xFFFFFFFFu, base, 0);
           if (keep) emit(base + __popc(m & lt), o0, o1);
         }
@@ -1933,40 +2020,46 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       zero_tile();
    }
   }
+  if (EMIT) {   // every entry of the ring is written: tell the emitter warp
+    csync();
+    if (tid == 0) { __threadfence_block(); *(volatile u32*)&s.rctl[2] = 1u; }
+  }
 }
 
-#define TPC_K6_ENTRY(name, MODE, COG, GUARD)                                                            \
-  extern "C" __global__ void __launch_bounds__(TPC_K6_THREADS, TPC_K6_CTAS) name(K6Args a) {             \
+#define TPC_K6_ENTRY(name, MODE, COG, EMIT, GUARD)                                                      \
+  extern "C" __global__ void __launch_bounds__((EMIT) ? TPC_K6_THREADS_E : TPC_K6_THREADS, TPC_K6_CTAS) name(K6Args a) { \
     extern __shared__ __align__(128) u32 smem_u32[];                                                    \
     GUARD                                                                                               \
-    k6_body<MODE, COG>(a, smem_u32);                                                                  \
+    k6_body<MODE, COG, EMIT>(a, smem_u32);                                                            \
   }
 // the chained-scan variants only run when K7-K9 could not deliver the ordered output (flag set)
 #define TPC_K6_IF_FLAG if (*a.det_flag == 0u) return;
 #if TPC_UNITS & TPC_U_TILES_FAST
-TPC_K6_ENTRY(k_cluster_tiles_fast, TPC_MODE_FAST, 0, )
+TPC_K6_ENTRY(k_cluster_tiles_fast, TPC_MODE_FAST, 0, false, )
+TPC_K6_ENTRY(k_cluster_tiles_fast_e, TPC_MODE_FAST, 0, true, )
 #endif
 #if TPC_UNITS & TPC_U_TILES_DET
-TPC_K6_ENTRY(k_cluster_tiles_det, TPC_MODE_DET, 0, TPC_K6_IF_FLAG)
-TPC_K6_ENTRY(k_cluster_tiles_det_temp, TPC_MODE_DET_TEMP, 0, )
+TPC_K6_ENTRY(k_cluster_tiles_det, TPC_MODE_DET, 0, false, TPC_K6_IF_FLAG)
+TPC_K6_ENTRY(k_cluster_tiles_det_temp, TPC_MODE_DET_TEMP, 0, false, )
 #endif
 #if TPC_UNITS & TPC_U_TILES_DUMP
-TPC_K6_ENTRY(k_cluster_tiles_dump_map, TPC_MODE_DUMP_MAP, 0, )
+TPC_K6_ENTRY(k_cluster_tiles_dump_map, TPC_MODE_DUMP_MAP, 0, false, )
 #endif
 // reading Q10' (TPCCLUS_COG_GATED)
 #if TPC_UNITS & TPC_U_TILES_FAST_G
-TPC_K6_ENTRY(k_cluster_tiles_fast_gated, TPC_MODE_FAST, 1, )
+TPC_K6_ENTRY(k_cluster_tiles_fast_gated, TPC_MODE_FAST, 1, false, )
+TPC_K6_ENTRY(k_cluster_tiles_fast_gated_e, TPC_MODE_FAST, 1, true, )
 #endif
 #if TPC_UNITS & TPC_U_TILES_DET_G
-TPC_K6_ENTRY(k_cluster_tiles_det_gated, TPC_MODE_DET, 1, TPC_K6_IF_FLAG)
-TPC_K6_ENTRY(k_cluster_tiles_det_temp_gated, TPC_MODE_DET_TEMP, 1, )
+TPC_K6_ENTRY(k_cluster_tiles_det_gated, TPC_MODE_DET, 1, false, TPC_K6_IF_FLAG)
+TPC_K6_ENTRY(k_cluster_tiles_det_temp_gated, TPC_MODE_DET_TEMP, 1, false, )
 #endif
 // reading Q10'' (TPCCLUS_COG_SHARED): these units -- and the partition units of such a handle -- are compiled with TPC_HALO = 5
 #if TPC_UNITS & TPC_U_TILES_FAST_S
-TPC_K6_ENTRY(k_cluster_tiles_fast_shared, TPC_MODE_FAST, 2, )
+TPC_K6_ENTRY(k_cluster_tiles_fast_shared, TPC_MODE_FAST, 2, false, )
 #endif
 #if TPC_UNITS & TPC_U_TILES_DET_S
-TPC_K6_ENTRY(k_cluster_tiles_det_shared, TPC_MODE_DET, 2, TPC_K6_IF_FLAG)
-TPC_K6_ENTRY(k_cluster_tiles_det_temp_shared, TPC_MODE_DET_TEMP, 2, )
+TPC_K6_ENTRY(k_cluster_tiles_det_shared, TPC_MODE_DET, 2, false, TPC_K6_IF_FLAG)
+TPC_K6_ENTRY(k_cluster_tiles_det_temp_shared, TPC_MODE_DET_TEMP, 2, false, )
 #endif
 #endif   // TPC_UNITS != 0u

@@ -616,6 +616,49 @@ def test_sparse_dense_tile_alternation(tp, cuda_device):
         _check_fast(fast, exp)
 
 
+def test_sparse_tiles_through_the_emitter_ring(tp, cuda_device):
+    """FAST on a sparse frame: the clusters of a tile with <= 256 records leave through a 64-entry ring
+    in shared memory to a warp of their own (k_cluster_tiles_fast_e).  Tiles of single-digit clusters on
+    a 3 x 3 lattice -- up to 240 of them, every digit a surviving peak -- overrun the ring, so warps also
+    take the fall-back (they emit themselves), the tags of the ring wrap many times, and tiles of 0, 1
+    and a few clusters follow in between.  The set must be the oracle's, the count exact under
+    overflow of the output, for the readings Q10 and Q10'."""
+    rng = np.random.default_rng(97)
+    P, n_slabs = 100, 60
+    T = 128 * n_slabs
+    rows = []
+    for r in (0, 1, 2):
+        for sl in range(n_slabs):
+            kind = (sl + r) % 4
+            n = [240, 0, 3, 120][kind] if sl else 1
+            lat = [(t, p) for t in range(1, 127, 3) for p in range(1, P - 1, 3)]   # 42 x 33 sites, pairwise distance >= 3
+            for k in rng.choice(len(lat), size=n, replace=False):
+                t, p = lat[k]
+                rows.append((0, r, p, sl * 128 + t, int(rng.integers(6, 1023))))
+                if kind == 2:   # a real 3 x 3 cluster around it
+                    for dt, dp in ((0, 1), (1, 0), (-1, 0), (0, -1)):
+                        rows.append((0, r, p + dp, sl * 128 + t + dt, 3))
+    d = t1.make_digits(rows)
+    d = d[rng.permutation(len(d))]
+    pads = [P, P, P]
+    assert len(d) < 512 * 3 * n_slabs        # the host picks the emitter kernel below this density
+    for gated in (False, True):
+        cl, st_exp, cnt = t1.clusterize(d.view(t1.DIGIT), 1, 3, T, pads, 6, 4, cog_gated=gated)
+        c = tp.Clusterizer(1, 3, T, pads, len(d), 6, 4, cog_gated=gated)
+        dt_ = _digits_tensor(d, cuda_device)
+        for _ in range(3):
+            fast, n, st = c.run_sync(dt_, tp.MODE_FAST)
+            assert n == cnt == len(fast) and st == st_exp
+            _check_fast(fast, cl)
+        det, n, st = c.run_sync(dt_, tp.MODE_DETERMINISTIC)
+        assert det.tobytes() == cl.tobytes()
+        got, n, st = c.run_sync(dt_, tp.MODE_FAST, capacity=100)
+        assert n == cnt and (st & tp.STATUS_OVERFLOW) and len(got) == 100
+        keys = set(_key(cl).tolist())
+        assert all(k in keys for k in _key(got).tolist()) and len(set(_key(got).tolist())) == 100
+        c.close()
+
+
 def test_two_handles_two_streams_concurrently(tp, cuda_device):
     """Modules and constant blocks are per handle (R6, PAPER.md 81-85): two generic handles of
     different geometry AND thresholds run at the same time on two streams, many times over, and each
