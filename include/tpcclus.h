@@ -112,8 +112,10 @@ enum {
   TPCCLUS_ERR_CUDA = -2,
   TPCCLUS_ERR_NVRTC = -3,
   TPCCLUS_ERR_WORKSPACE_TOO_SMALL = -4,
-  TPCCLUS_ERR_UNSUPPORTED_GEOMETRY = -5 /* more than 5503 coarse bins n_sectors*n_rows*ceil(n_time/16256):
-                                           the first partition pass keeps 40 B of shared memory per bin */
+  TPCCLUS_ERR_UNSUPPORTED_GEOMETRY = -5 /* more than 56064 coarse bins n_sectors*n_rows*ceil(n_time/16256): the
+                                           directory kernels keep a counter per bin in shared memory.  (The first
+                                           partition pass has stages for 5503 bins; beyond that it runs once per
+                                           5503 bins, each time over the whole input: tpcclus_launches_per_run.) */
 };
 
 typedef struct {

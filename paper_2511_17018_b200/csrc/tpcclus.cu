@@ -76,6 +76,7 @@ struct Geometry {
   TpcParams prm;
   uint32_t g1;           // K1 grid = number of SMs
   uint32_t slice_cap;    // chunks per K1 CTA
+  uint32_t k1_passes;    // K1 launches per run: ceil(n_bins / 5503)
   uint32_t n_tiles, n_scan_blocks;
   uint64_t n_chunks_max, n_batches_max, blob_cap, idx_cap;
   uint64_t max_digits;
@@ -109,8 +110,14 @@ int make_geometry(const tpcclus_params* p, Geometry* g) {
   }
   q.n_tc = (p->n_time + TPC_TC - 1) / TPC_TC;
   uint64_t nb = (uint64_t)p->n_sectors * p->n_rows * q.n_tc;
-  if (nb > 65535 || tpc_k1_smem_bytes((uint32_t)nb) > kMaxSmem) return TPCCLUS_ERR_UNSUPPORTED_GEOMETRY;
+  // K2..K4 keep one 4-byte counter per bin in shared memory (k_dir_scan: + 8 KB static): 56064 bins at most.
+  if (nb > (kMaxSmem - 8192u) / 4u) return TPCCLUS_ERR_UNSUPPORTED_GEOMETRY;
   q.n_bins = (uint32_t)nb;
+  // K1 has stages for 5503 bins; a larger geometry is binned in several passes over the input (R1)
+  uint32_t k1_max = (uint32_t)nb;
+  while (tpc_k1_smem_bytes(k1_max) > kMaxSmem) --k1_max;
+  g->k1_passes = (uint32_t)((nb + k1_max - 1) / k1_max);
+  q.k1_bins = (uint32_t)((nb + g->k1_passes - 1) / g->k1_passes);
   uint32_t tmin = p->n_time < TPC_TC ? p->n_time : TPC_TC;
   q.n_sl = (tmin + TPC_TS - 1) / TPC_TS;
   q.max_pads = maxp;
@@ -252,12 +259,12 @@ const UnitInfo kUnits[U_COUNT_] = {TPC_UNIT_LIST(X)};
 // reading of the centre of gravity: {Q10, Q10' gated, Q10'' shared}.
 enum KernelId { K_RESET, K_PUBLISH, K_PART_COARSE, K_DIR_COUNT, K_DIR_SCAN, K_DIR_FILL, K_PART_FINE, K_TILES_FAST, K_TILES_FAST_E, K_TILES_DET,
                 K_TILES_DET_TEMP, K_TILES_DUMP, K_SCAN_LOCAL, K_SCAN_SUMS, K_EMIT_ORDERED, K_EMIT_PACKED, K_COUNT_ };
-struct KernelInfo { const char* name[3]; UnitId unit[3]; int smem; };   // smem: 0 none/static, 1 K1, 5 K5, 6 K6
+struct KernelInfo { const char* name[3]; UnitId unit[3]; int smem; };   // smem: 0 none/static, 1 K1, 2 one word per bin, 5 K5, 6 K6
 #define SAME3(x) {x, x, x}
 const KernelInfo kKernels[K_COUNT_] = {
     {SAME3("k_reset"), SAME3(U_DIR), 0}, {SAME3("k_publish"), SAME3(U_DIR), 0},
     {SAME3("k_partition_coarse"), {U_PART_COARSE, U_PART_COARSE, U_PART_COARSE_H5}, 1},
-    {SAME3("k_dir_count"), SAME3(U_DIR), 0}, {SAME3("k_dir_scan"), SAME3(U_DIR), 0}, {SAME3("k_dir_fill"), SAME3(U_DIR), 0},
+    {SAME3("k_dir_count"), SAME3(U_DIR), 2}, {SAME3("k_dir_scan"), SAME3(U_DIR), 2}, {SAME3("k_dir_fill"), SAME3(U_DIR), 2},
     {SAME3("k_partition_fine"), {U_PART_FINE, U_PART_FINE, U_PART_FINE_H5}, 5},
     {{"k_cluster_tiles_fast", "k_cluster_tiles_fast_gated", "k_cluster_tiles_fast_shared"}, {U_TILES_FAST, U_TILES_FAST_G, U_TILES_FAST_S}, 6},
     // the same with the emitter warp, for sparse frames (reading Q10'' has none: the plain kernel)
@@ -351,7 +358,7 @@ std::string rtc_prologue(const TpcParams& q, uint32_t unit_bit, uint32_t halo) {
   snprintf(buf, sizeof buf, "#define TPC_UNITS %uu\n#define TPC_HALO %uu\n", unit_bit, halo); s += buf;
 #define DEF(f) do { snprintf(buf, sizeof buf, "#define TPC_" #f " %uu\n", q.f); s += buf; } while (0)
   DEF(n_sectors); DEF(n_rows); DEF(n_time); DEF(n_tc); DEF(n_bins); DEF(n_sl); DEF(pitch); DEF(max_pads);
-  DEF(thr_peak); DEF(noise_eps); DEF(max_peaks); DEF(cog_mode);
+  DEF(thr_peak); DEF(noise_eps); DEF(max_peaks); DEF(cog_mode); DEF(k1_bins);
 #undef DEF
   s += "__constant__ unsigned short TPC_NPADS_TABLE[256] = {";   // constant bank like the generic build's table: no 64-bit address registers
   for (int r = 0; r < 256; ++r) { snprintf(buf, sizeof buf, "%u,", (unsigned)q.n_pads[r]); s += buf; }
@@ -464,7 +471,7 @@ int load_unit(tpcclus_handle* h, UnitId u, const void* image) {
     if (kKernels[k].unit[h->cog] != u) continue;
     if ((rc = d.cuModuleGetFunction(&h->fn[k], h->module[u], kKernels[k].name[h->cog])) != 0)
       return fail(nullptr, TPCCLUS_ERR_CUDA, std::string("cuModuleGetFunction(") + kKernels[k].name[h->cog] + "): " + drv_error(rc));
-    const uint32_t smem = kKernels[k].smem == 1 ? h->smem_k1 : kKernels[k].smem == 5 ? h->smem_k5 : kKernels[k].smem == 6 ? h->smem_k6 : 0u;
+    const uint32_t smem = kKernels[k].smem == 1 ? h->smem_k1 : kKernels[k].smem == 5 ? h->smem_k5 : kKernels[k].smem == 6 ? h->smem_k6 : kKernels[k].smem == 2 ? 4u * h->g.prm.n_bins : 0u;
     const int CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES = 8;
     if (smem > 48u * 1024u && (rc = d.cuFuncSetAttribute(h->fn[k], CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES, (int)smem)) != 0)
       return fail(nullptr, TPCCLUS_ERR_CUDA, std::string("cuFuncSetAttribute(") + kKernels[k].name[h->cog] + "): " + drv_error(rc));
@@ -566,7 +573,7 @@ int tpcclus_create(const tpcclus_params* p, tpcclus_handle** out) {
   h->params = *p;
   h->params.n_pads = h->g.prm.n_pads;
   h->ws = (char*)p->workspace;
-  h->smem_k1 = tpc_k1_smem_bytes(g.prm.n_bins);
+  h->smem_k1 = tpc_k1_smem_bytes(g.prm.k1_bins);
   h->smem_k5 = tpc_k5_smem_bytes();
   h->cog = (int)g.prm.cog_mode;
   h->halo = h->cog == 2 ? 5u : 3u;
@@ -648,8 +655,8 @@ const char* tpcclus_error_string(int code) {
 const char* tpcclus_last_error(const tpcclus_handle* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
 
 int tpcclus_launches_per_run(const tpcclus_handle* h, int mode) {
-  (void)h;
-  return mode == TPCCLUS_MODE_DETERMINISTIC ? 11 : 7;   // K0..K6; DET: + K7, K8, K9 and the (normally idle) chained K6
+  const int extra = h ? (int)h->g.k1_passes - 1 : 0;   // K1 once per pass (one, up to 5503 coarse bins)
+  return (mode == TPCCLUS_MODE_DETERMINISTIC ? 11 : 7) + extra;   // K0..K6; DET: + K7, K8, K9 and the (normally idle) chained K6
 }
 
 int tpcclus_set_timing(tpcclus_handle* h, int enable) {
@@ -723,8 +730,11 @@ int enqueue_binning(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n
   u64 n64 = n;
   u32 slice_cap = h->dbg_slice_cap ? h->dbg_slice_cap : g.slice_cap;
   u64 blob_cap = h->dbg_blob_cap ? h->dbg_blob_cap : g.blob_cap;
-  { void* a[] = {&dig, &n64, &per_cta, &p.pool, &p.dir, &p.used, &slice_cap, &status};
-    if ((rc = launch(h, K_PART_COARSE, dim3(g.g1), dim3(TPC_K1_THREADS), h->smem_k1, st, a))) return rc; }
+  for (u32 pass = 0; pass < g.k1_passes; ++pass) {   // one pass, unless the geometry has more bins than K1 has stages for
+    u32 bin_lo = pass * g.prm.k1_bins;
+    void* a[] = {&dig, &n64, &per_cta, &p.pool, &p.dir, &p.used, &slice_cap, &status, &bin_lo};
+    if ((rc = launch(h, K_PART_COARSE, dim3(g.g1), dim3(TPC_K1_THREADS), h->smem_k1, st, a))) return rc;
+  }
   u32 smem_nb = 4u * g.prm.n_bins;
   { void* a[] = {&p.dir, &p.used, &slice_cap, &p.slice_cnt, &p.bin_chunk_start};
     if ((rc = launch(h, K_DIR_COUNT, dim3(g.g1), dim3(TPC_SCAN_THREADS), smem_nb, st, a))) return rc; }

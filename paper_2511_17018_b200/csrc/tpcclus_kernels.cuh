@@ -76,6 +76,7 @@ struct TpcParams {
   u32 thr_peak, noise_eps;
   u32 max_peaks;   // capacity of the per-tile peak list
   u32 cog_mode;    // 0 = Q10, 1 = Q10' gated, 2 = Q10'' shared (host side only: selects the kernel variants)
+  u32 k1_bins;     // coarse bins one K1 launch holds stages for: n_bins, or n_bins / passes (rounded up) beyond the shared-memory budget
   u16 n_pads[256];
 };
 
@@ -194,9 +195,11 @@ struct K1Smem {   // layout computed identically on the host (tpc_k1_smem_bytes)
   u32* spill;     // [2][warps][TPC_K1_WSP][2]  {rec, bin | slot << 16}
   u32* misc;      // [0] next chunk
   u16* fq;        // [warps][TPC_K1_WFQ]
+  u32 bin_lo;     // first bin of this pass (bins are local to the pass in shared memory, global in dir[])
 };
-__device__ __forceinline__ K1Smem k1_smem(u32* base, u32 nb) {   // fixed-size arrays first: constant offsets
+__device__ __forceinline__ K1Smem k1_smem(u32* base, u32 nb, u32 bin_lo) {   // fixed-size arrays first: constant offsets
   K1Smem s;
+  s.bin_lo = bin_lo;
   s.misc = base;
   s.spill = s.misc + 8;
   s.fq = (u16*)(s.spill + 4u * TPC_K1_SPILL);
@@ -218,7 +221,7 @@ __device__ __forceinline__ void k1_flush_pair(const K1Smem& s, bool act, u32 bin
     if (fill == 8u) {
       c = atomicAdd(&s.misc[0], 1u);
       fill = 0u;
-      if (c < slice_cap) dir[slice_base + c] = (bin << 8) | TPC_CHUNK;
+      if (c < slice_cap) dir[slice_base + c] = ((bin + s.bin_lo) << 8) | TPC_CHUNK;
     }
     s.pos[bin] = (c << 4) | (fill + 1u);
     s.cnt[bin] -= 8u;   // one flush per bin and phase: no other thread touches cnt[bin] here
@@ -236,7 +239,7 @@ __device__ __forceinline__ void k1_flush_single(const K1Smem& s, u32 bin, u32 sl
   if (fill == 8u) {
     c = atomicAdd(&s.misc[0], 1u);
     fill = 0u;
-    if (c < slice_cap) dir[slice_base + c] = (bin << 8) | TPC_CHUNK;
+    if (c < slice_cap) dir[slice_base + c] = ((bin + s.bin_lo) << 8) | TPC_CHUNK;
   }
   s.pos[bin] = (c << 4) | (fill + 1u);
   s.cnt[bin] -= 8u;
@@ -326,10 +329,12 @@ __device__ __forceinline__ bool k1_pass(const K1Smem& s, u32& cur, u32& nsp, con
   return __syncthreads_or((int)pend) != 0;
 }
 
+// GENERAL: several coarse time-chunks (halo copies into the neighbouring chunk's bin) and / or several passes over
+// the input (only the bins [bin_lo, bin_lo + k1_bins) of this pass are staged); false: one chunk, one pass
 template <bool MULTI_TC>
 __device__ __forceinline__ void k1_rounds(const K1Smem& s, const uint2* __restrict__ digits, u64 n, u32 n_rounds, u32 slice_base,
                                           u32 slice_cap, uint4* pool, u32* dir, u32& cur, u32& nsp, bool& bad) {
-  const u32 S = PRM(n_sectors), R = PRM(n_rows), T = PRM(n_time), NTC = PRM(n_tc);
+  const u32 S = PRM(n_sectors), R = PRM(n_rows), T = PRM(n_time), NTC = PRM(n_tc), KB = PRM(k1_bins);
   // The input is cut into (2 x warps x CTAs) regions of n_rounds x 64 digits; load h of warp w
   // walks region (2w + h) * CTAs + cta, 512 contiguous bytes per round (lane l: digits 2l, 2l+1).
   // A round of this CTA therefore draws from 64 places spread over the whole frame, so that
@@ -377,15 +382,16 @@ __device__ __forceinline__ void k1_rounds(const K1Smem& s, const uint2* __restri
       u32 tc = 0u, v = t;
       if (MULTI_TC) { tc = t / TPC_TC; v = t - tc * TPC_TC; }
       const u32 b0 = MULTI_TC ? (sec * R + row) * NTC + tc : sec * R + row;
-      bin[k] = ok ? b0 : 0u;
+      const bool mine = ok && (!MULTI_TC || b0 - s.bin_lo < KB);   // (unsigned: also false below bin_lo)
+      bin[k] = mine ? b0 - (MULTI_TC ? s.bin_lo : 0u) : 0u;
       rec[k] = pad | ((v + TPC_HALO) << 8) | (q << 22);
-      pend |= ok ? (1u << k) : 0u;
+      pend |= mine ? (1u << k) : 0u;
       if (MULTI_TC) {   // halo copy into the neighbouring time-chunk's bin
         dbin[k] = 0u; drec[k] = 0u;
-        if (ok && v < TPC_HALO && tc > 0u) {
-          dbin[k] = b0 - 1u; drec[k] = pad | ((v + TPC_TC + TPC_HALO) << 8) | (q << 22); dpend |= 1u << k;
-        } else if (ok && v + TPC_HALO >= TPC_TC && tc + 1u < NTC) {
-          dbin[k] = b0 + 1u; drec[k] = pad | ((v + TPC_HALO - TPC_TC) << 8) | (q << 22); dpend |= 1u << k;
+        if (ok && v < TPC_HALO && tc > 0u && b0 - 1u - s.bin_lo < KB) {
+          dbin[k] = b0 - 1u - s.bin_lo; drec[k] = pad | ((v + TPC_TC + TPC_HALO) << 8) | (q << 22); dpend |= 1u << k;
+        } else if (ok && v + TPC_HALO >= TPC_TC && tc + 1u < NTC && b0 + 1u - s.bin_lo < KB) {
+          dbin[k] = b0 + 1u - s.bin_lo; drec[k] = pad | ((v + TPC_HALO - TPC_TC) << 8) | (q << 22); dpend |= 1u << k;
         }
       }
     }
@@ -431,20 +437,24 @@ __device__ __forceinline__ void k1_rounds(const K1Smem& s, const uint2* __restri
 #if TPC_UNITS & TPC_U_PART_COARSE
 extern "C" __global__ void __launch_bounds__(TPC_K1_THREADS, 1)
 k_partition_coarse(const uint2* __restrict__ digits, u64 n, u64 per_cta, uint4* __restrict__ pool,
-                   u32* __restrict__ dir, u32* __restrict__ used, u32 slice_cap, u32* __restrict__ status) {
+                   u32* __restrict__ dir, u32* __restrict__ used, u32 slice_cap, u32* __restrict__ status, u32 bin_lo) {
+  // A geometry with more coarse bins than shared memory has stages for (5503) is binned in several passes over the
+  // input, pass p staging the bins [p * k1_bins, (p + 1) * k1_bins): `bin_lo` = the first of them.  A pass
+  // continues this CTA's slice of the pool where the pass before stopped (used[]).
   extern __shared__ __align__(128) u32 smem_u32[];
-  const u32 nb = PRM(n_bins);
-  const K1Smem s = k1_smem(smem_u32, nb);
+  const u32 nb = PRM(k1_bins);
+  const K1Smem s = k1_smem(smem_u32, nb, bin_lo);
   for (u32 i = threadIdx.x; i < nb; i += TPC_K1_THREADS) { s.pos[i] = 8u; s.cnt[i] = 0u; }
-  if (threadIdx.x < 8) s.misc[threadIdx.x] = 0u;
+  if (threadIdx.x < 8) s.misc[threadIdx.x] = (threadIdx.x == 0 && bin_lo != 0u) ? used[blockIdx.x] : 0u;
   __syncthreads();
 
   const u32 slice_base = blockIdx.x * slice_cap;
   const u32 n_rounds = (u32)(per_cta / (TPC_K1_THREADS * TPC_K1_DPT));   // per_cta is a multiple of the round
   u32 cur = 0u, nsp = 0u;
   bool bad = false;
-  if (PRM(n_tc) > 1u) k1_rounds<true>(s, digits, n, n_rounds, slice_base, slice_cap, pool, dir, cur, nsp, bad);
-  else k1_rounds<false>(s, digits, n, n_rounds, slice_base, slice_cap, pool, dir, cur, nsp, bad);
+  if (PRM(n_tc) > 1u || PRM(k1_bins) < PRM(n_bins)) k1_rounds<true>(s, digits, n, n_rounds, slice_base, slice_cap, pool, dir, cur, nsp, bad);
+  else { K1Smem s0 = s; s0.bin_lo = 0u;   // (known to be 0 here: keeps the add out of the flush of the common instance)
+         k1_rounds<false>(s0, digits, n, n_rounds, slice_base, slice_cap, pool, dir, cur, nsp, bad); }
   if (bad) atomicOr(status, TPC_STATUS_BAD_DIGITS);
   {   // records still parked in the spill lists
     u32 bin[1] = {0u}, rec[1] = {0u}, slot[1] = {0u}, pend = 0u;
@@ -464,10 +474,10 @@ k_partition_coarse(const uint2* __restrict__ digits, u64 n, u64 per_cta, uint4* 
       const uint4* st = (const uint4*)stw;
       if (c < slice_cap) {
         st_256(pool + ((u64)(slice_base + c) * 16u + fill * 2u), st[0], st[1]);
-        dir[slice_base + c] = (b << 8) | (fill * 8u + m);
+        dir[slice_base + c] = ((b + bin_lo) << 8) | (fill * 8u + m);
       }
     } else if (fill != 8u && fill != 0u) {
-      if (c < slice_cap) dir[slice_base + c] = (b << 8) | (fill * 8u);
+      if (c < slice_cap) dir[slice_base + c] = ((b + bin_lo) << 8) | (fill * 8u);
     }
   }
   __syncthreads();

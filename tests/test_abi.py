@@ -47,6 +47,8 @@ def test_workspace_bytes_and_validation(binding):
     assert binding.tpcclus_workspace_bytes(bad) == 0
     bad, _ = binding.make_params(1, 16, 256, [64] * 15 + [300], 10000)
     assert binding.tpcclus_workspace_bytes(bad) == 0
+    longer, keep3 = binding.make_params(36, 152, 40000, pads, 10**8)   # 16416 coarse bins: three passes of K1 (R1)
+    assert binding.tpcclus_workspace_bytes(longer) > 0
     toomany, _ = binding.make_params(256, 256, 256, [64] * 256, 10000)   # 65536 coarse bins
     assert binding.tpcclus_workspace_bytes(toomany) == 0
     assert binding.lib().tpcclus_error_string(-5).startswith(b"unsupported")

@@ -659,6 +659,43 @@ def test_sparse_tiles_through_the_emitter_ring(tp, cuda_device):
         c.close()
 
 
+def test_more_bins_than_k1_has_stages_for(tp, cuda_device):
+    """R1: K1 holds write-combining stages for 5503 coarse bins; a geometry with more is binned in several passes
+    over the input, pass p staging the bins [p k, (p + 1) k).  (a) 40 x 152 maps (6080 bins, 2 passes); (b) 20 x 140
+    maps over 16300 time bins = two coarse time-chunks (5600 bins, 2 passes), with clusters across the chunk border
+    at t = 16256 whose halo copies go to a bin of the OTHER pass.  Both against the oracle, DET byte for byte and
+    FAST as a set, generic and RTC build."""
+    rng = np.random.default_rng(131)
+    cases = []
+    S, R, T, P = 40, 152, 300, 24
+    n = 400_000
+    rows = np.stack([rng.integers(0, S, n), rng.integers(0, R, n), rng.integers(0, P, n), rng.integers(0, T, n),
+                     rng.integers(1, 200, n)], axis=1)
+    cases.append((S, R, T, [P] * R, t1.make_digits([tuple(int(v) for v in r) for r in rows])))
+    S, R, T, P = 20, 140, 16300, 12
+    n = 300_000
+    t = np.where(rng.random(n) < 0.5, rng.integers(16256 - 8, 16256 + 8, n), rng.integers(0, T, n))
+    rows = np.stack([rng.integers(0, S, n), rng.integers(0, R, n), rng.integers(0, P, n), t, rng.integers(1, 200, n)], axis=1)
+    cases.append((S, R, T, [P] * R, t1.make_digits([tuple(int(v) for v in r) for r in rows])))
+    for S, R, T, pads, d in cases:
+        # one digit per cell (FAST promises the oracle's set for duplicate-free input only, Q5)
+        key = (d["sector"].astype(np.int64) << 40) | (d["row"].astype(np.int64) << 32) | (d["time"].astype(np.int64) << 8) | d["pad"]
+        d = d[np.unique(key, return_index=True)[1]]
+        d = d[rng.permutation(len(d))]
+        exp, st_exp = _oracle(d, S, R, T, pads)
+        assert len(exp) > 1000
+        for rtc in (False, True):
+            c = tp.Clusterizer(S, R, T, pads, len(d), 6, 4, rtc=rtc)
+            assert c.launches_per_run(tp.MODE_FAST) == 8          # K1 twice
+            dt_ = _digits_tensor(d, cuda_device)
+            det, n_det, st = c.run_sync(dt_, tp.MODE_DETERMINISTIC)
+            assert st == st_exp and det.tobytes() == exp.tobytes()
+            fast, n_fast, st = c.run_sync(dt_, tp.MODE_FAST)
+            assert st == st_exp
+            _check_fast(fast, exp)
+            c.close()
+
+
 def test_two_handles_two_streams_concurrently(tp, cuda_device):
     """Modules and constant blocks are per handle (R6, PAPER.md 81-85): two generic handles of
     different geometry AND thresholds run at the same time on two streams, many times over, and each
