@@ -47,11 +47,11 @@ UNIT = "digits/s"
 def _ncu_traffic(k, order, rtc, mode):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch from the newest committed `ncu --set full`
     capture (profiles/*_traffic.json, written by paper_2511_17018_b200/ncu_summary.py).  A capture
-    describes the kernel text it was taken on and the headline workload only: for any other text or
-    workload the field is null rather than stale."""
+    describes the kernel text and the workload it was taken on (its note names config and mode): for any
+    other text or workload the field is null rather than stale."""
     import glob
     import hashlib
-    if not (k == 4 and order == "shuffled" and not rtc and mode == "fast"):
+    if not (order == "shuffled" and not rtc and mode in ("fast", "det")):
         return {}, None
     with open(os.path.join(ROOT, "paper_2511_17018_b200", "csrc", "tpcclus_kernels.cuh"), "rb") as f:
         sha = hashlib.sha256(f.read()).hexdigest()
@@ -61,7 +61,8 @@ def _ncu_traffic(k, order, rtc, mode):
                 t = json.load(f)
         except Exception:
             continue
-        if t.get("kernel_text_sha256") == sha:
+        note = t.get("note", "")
+        if t.get("kernel_text_sha256") == sha and ("CFG[%d]" % k) in note and ("DET" if mode == "det" else "FAST") in note:
             return t.get("traffic_bytes", {}), os.path.relpath(path, ROOT)
     return {}, None
 
@@ -370,6 +371,10 @@ def main():
         "k_emit_ordered": 64 * n_clusters,                       # DET: ordered copy of the runs
         "k_emit_packed": 48 * n_clusters,                        # packed: 32 B in, 16 B out
     }
+    for nm in list(avg):   # the tile kernels of the other readings and the sparse-frame variant (emitter warp) move the same bytes
+        for base in ("k_cluster_tiles_fast", "k_cluster_tiles_det_temp"):
+            if nm.startswith(base) and nm not in alg:
+                alg[nm] = alg[base]
     traffic, traffic_src = _ncu_traffic(k, args.order, args.rtc, args.mode)
     step_sum = sum(avg.values())
     per_kernel_roof = {}
@@ -384,7 +389,7 @@ def main():
     b_alg = 8 * n + 32 * n_clusters
     method = {"b_alg_bytes": b_alg, "achieved_gbs": b_alg / (ms_step * 1e-3) / 1e9,
               "frac_of_peak": b_alg / (ms_step * 1e-3) / 1e9 / peak}
-    if traffic and all(nm in traffic for nm in ("k_partition_coarse", "k_partition_fine", "k_cluster_tiles_fast")):
+    if traffic and all(any(t.startswith(nm) for t in traffic) for nm in ("k_partition_coarse", "k_partition_fine", "k_cluster_tiles_fast")):
         dram = sum(traffic.values())
         method.update({"dram_bytes_per_step_ncu": dram, "dram_gbs": dram / (ms_step * 1e-3) / 1e9,
                        "dram_frac_of_peak": dram / (ms_step * 1e-3) / 1e9 / peak})
