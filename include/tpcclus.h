@@ -268,6 +268,29 @@ TPCCLUS_API int tpcclus_rtc_cache_hit(const tpcclus_handle* h);
 TPCCLUS_API int tpcclus_run_packed(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n,
                                    const tpcclus_out_packed* out, void* cuda_stream);
 
+/* The same packed form for a cluster list that is already on the device, WITHOUT a handle, a workspace or any
+ * allocation: for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid it).  d_clusters: the n clusters tpcclus_run wrote in DETERMINISTIC mode, i.e. ordered by
+ * (sector, row, time_peak, pad_peak) (DEVICE, 16-byte aligned); d_packed: room for n records (DEVICE, 16-byte
+ * aligned); d_row_index: n_sectors * n_rows + 1 entries as in tpcclus_out_packed (DEVICE).  Byte for byte what
+ * tpcclus_run_packed delivers for the same frame (a cluster whose sector or row lies outside the geometry given
+ * here is packed but not indexed).  Enqueues one memset and two kernels on cuda_stream and returns; the device
+ * that owns the buffers must be current.
+ * The only scratch memory -- one 32-bit counter per (sector, row) -- is a file-scope array in device memory,
+ * TPCCLUS_NOALLOC_SCRATCH_BYTES that every GPU that loads the library holds until the process ends; hence the
+ * limits n_sectors * n_rows <= TPCCLUS_NOALLOC_MAX_ROWS and n <= TPCCLUS_NOALLOC_MAX_CLUSTERS: beyond them the
+ * call returns TPCCLUS_ERR_INVALID_ARG and says which limit in `err` (optional, NUL-terminated, at most err_cap
+ * bytes).  The array is shared by every call and keeps the last call's contents: each call clears the counters
+ * it uses first, on its stream.  Calls that overlap on the GPU (two streams) RACE on it: serialise them.  The
+ * first call on a device looks the array's address up (cudaGetSymbolAddress; no allocation): make it once
+ * before a stream capture begins.  Calls no cudaMalloc, cudaFree or allocating library routine. */
+#define TPCCLUS_NOALLOC_MAX_ROWS 65536u             /* (sector, row) pairs: 256 x 256 */
+#define TPCCLUS_NOALLOC_MAX_CLUSTERS 0xFFFFFFFFull   /* 32-bit counters */
+#define TPCCLUS_NOALLOC_SCRATCH_BYTES ((TPCCLUS_NOALLOC_MAX_ROWS + 64u) * 4u)   /* 256.25 KB */
+TPCCLUS_API int tpcclus_pack_noalloc(const tpcclus_cluster* d_clusters, uint64_t n, uint32_t n_sectors, uint32_t n_rows,
+                                     tpcclus_cluster16* d_packed, uint64_t* d_row_index, void* cuda_stream,
+                                     char* err, uint32_t err_cap);
+
 /* Number of constant blocks in the handle's registry (= loaded offline-compiled units; 0 for RTC
  * handles), and the names of the loaded compilation units (static strings; returns the count). */
 TPCCLUS_API int tpcclus_constant_buffers(const tpcclus_handle* h);

@@ -8,5 +8,5 @@ checked), every compute call needs one.
 from .binding import (  # noqa: F401
     CLUSTER16_DTYPE, CLUSTER_DTYPE, COG_GATED, COG_SHARED, DIGIT_DTYPE, FLAG_EDGE_PAD, FLAG_EDGE_TIME, FLAG_SATURATED, MODE_DETERMINISTIC, MODE_FAST,
     RTC, STATUS_BAD_DIGITS, STATUS_INTERNAL, STATUS_NO_PACKED, STATUS_OVERFLOW, Clusterizer, TpcclusError, lib, tpcclus_params, tpcclus_out,
-    tpcclus_set_rtc_cache_dir,
+    tpcclus_set_rtc_cache_dir, tpcclus_pack_noalloc, NOALLOC_MAX_ROWS,
 )

@@ -65,7 +65,8 @@ EXPORTS = ("tpcclus_workspace_bytes", "tpcclus_workspace_bytes_host", "tpcclus_c
            "tpcclus_launches_per_run", "tpcclus_set_timing", "tpcclus_last_timing", "tpcclus_rtc_build_ms",
            "tpcclus_debug_dense_map", "tpcclus_debug_det_fallback", "tpcclus_set_rtc_cache_dir", "tpcclus_rtc_cache_hit", "tpcclus_run_packed",
            "tpcclus_update_params", "tpcclus_constant_buffers", "tpcclus_loaded_units", "tpcclus_debug_shrink",
-           "tpcclus_workspace_bytes_host_pipelined", "tpcclus_host_submit", "tpcclus_host_wait")
+           "tpcclus_workspace_bytes_host_pipelined", "tpcclus_host_submit", "tpcclus_host_wait", "tpcclus_pack_noalloc")
+NOALLOC_MAX_ROWS = 65536   # include/tpcclus.h: TPCCLUS_NOALLOC_MAX_ROWS
 
 
 def lib() -> C.CDLL:
@@ -88,6 +89,9 @@ def lib() -> C.CDLL:
     L.tpcclus_run.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, P(tpcclus_out), C.c_int, C.c_void_p]
     L.tpcclus_run_packed.restype = C.c_int
     L.tpcclus_run_packed.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, P(tpcclus_out_packed), C.c_void_p]
+    L.tpcclus_pack_noalloc.restype = C.c_int
+    L.tpcclus_pack_noalloc.argtypes = [C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_void_p, C.c_void_p, C.c_void_p,
+                                       C.c_char_p, C.c_uint32]
     L.tpcclus_run_host.restype = C.c_int
     L.tpcclus_run_host.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p, C.c_uint64,
                                    P(C.c_uint64), P(C.c_uint32), C.c_int, C.c_void_p]
@@ -170,6 +174,17 @@ def tpcclus_set_rtc_cache_dir(path) -> None:
 
 def tpcclus_destroy(handle) -> None:
     lib().tpcclus_destroy(handle)
+
+
+def tpcclus_pack_noalloc(clusters_ptr: int, n: int, n_sectors: int, n_rows: int, packed_ptr: int, row_index_ptr: int,
+                         stream: int = 0) -> None:
+    """include/tpcclus.h: tpcclus_pack_noalloc -- the packed 16-byte records and the per-row index of an ordered
+    cluster list on the device, without a handle, a workspace or any allocation (DEVICE pointers as integers)."""
+    err = C.create_string_buffer(256)
+    rc = lib().tpcclus_pack_noalloc(C.c_void_p(clusters_ptr), n, n_sectors, n_rows, C.c_void_p(packed_ptr),
+                                    C.c_void_p(row_index_ptr), C.c_void_p(stream), err, 256)
+    if rc != 0:
+        raise TpcclusError(rc, "tpcclus_pack_noalloc", err.value.decode())
 
 
 class Clusterizer:

@@ -21,7 +21,7 @@ LIB = os.path.join(HERE, "libtpcclus.so")
 GEN_DIR = os.path.join(ROOT, "build")
 GEN = os.path.join(GEN_DIR, "tpcclus_embedded.S")
 SOURCES = [os.path.join(CSRC, "tpcclus.cu"), os.path.join(CSRC, "tpcclus_kernels.cuh"), os.path.join(CSRC, "tpcclus_unit.cu"),
-           os.path.join(ROOT, "include", "tpcclus.h")]
+           os.path.join(CSRC, "tpcclus_noalloc.cu"), os.path.join(ROOT, "include", "tpcclus.h")]
 
 # compilation units (PAPER.md 64: one GPU binary per kernel family): name -> TPC_U_* bit of tpcclus_kernels.cuh
 # (the units of reading Q10'' and the partition / debug units that feed them carry a time halo of 5: -DTPC_HALO=5u)
@@ -88,8 +88,12 @@ def build(force: bool = False, verbose: bool = False) -> str:
     _embed()
     obj = os.path.join(GEN_DIR, "tpcclus_embedded.o")
     subprocess.check_call(["gcc", "-c", "-o", obj, GEN])
+    # the handle-free entry point with its scratch in a static device array: an object of its own, device code for sm_100a
+    noalloc = os.path.join(GEN_DIR, "tpcclus_noalloc.o")
+    subprocess.check_call([_nvcc(), *DEVICE_FLAGS, "-Xcompiler", "-fPIC,-fvisibility=hidden", "-c", "-o", noalloc,
+                           os.path.join(CSRC, "tpcclus_noalloc.cu")])
     tmp = LIB + ".tmp%d" % os.getpid()
-    subprocess.check_call([_nvcc(), *HOST_FLAGS, *os.environ.get("TPC_EXTRA", "").split(), "-o", tmp, os.path.join(CSRC, "tpcclus.cu"), obj, "-ldl"])
+    subprocess.check_call([_nvcc(), *HOST_FLAGS, *os.environ.get("TPC_EXTRA", "").split(), "-o", tmp, os.path.join(CSRC, "tpcclus.cu"), noalloc, obj, "-ldl"])
     os.replace(tmp, LIB)
     return LIB
 
