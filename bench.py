@@ -307,7 +307,22 @@ def main():
                   "note": "same resident frame, %d steps each after %d warm-ups; RTC build time excluded" % (args.steps, warmup)}
         r.close()
         del r
-        _log("ratios done: det %.3f ms, rtc %.3f ms" % (ms_det, ms_rtc))
+        # the same FAST step captured once into a CUDA graph and replayed: tpcclus_run only enqueues kernel
+        # launches, so it can be captured; matters for the launch-bound small frames (CFG[0,1])
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            step(c, tp.MODE_FAST)
+        for _ in range(warmup):
+            g.replay()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record()
+        for _ in range(args.steps):
+            g.replay()
+        ev1.record()
+        torch.cuda.synchronize(dev)
+        ratios["ms_graph_replay"] = ev0.elapsed_time(ev1) / args.steps
+        del g
+        _log("ratios done: det %.3f ms, rtc %.3f ms, graph replay %.3f ms" % (ms_det, ms_rtc, ratios["ms_graph_replay"]))
 
     # ---- e2e: host buffers through the C ABI, copies inside the timed region -----------------------
     # (a) tpcclus_run_host: one frame at a time, copy -> run -> copy back, serial;

@@ -188,7 +188,10 @@ TPCCLUS_API int tpcclus_create(const tpcclus_params* params, tpcclus_handle** ou
  * not modified.  out: HOST struct of DEVICE pointers.  The result depends only on
  * (params, digit multiset, mode), never on earlier runs (Q17).  One run at a time per
  * handle (the workspace is per handle).  The caller synchronises the stream before
- * reading *n_clusters / *status / clusters. */
+ * reading *n_clusters / *status / clusters.  Only kernel launches are enqueued -- nothing is
+ * allocated, nothing synchronises, no device result is read on the host -- so the call may be
+ * captured into a CUDA graph (with per-kernel timing off) and replayed with new digits in the
+ * same buffers: n is frozen in the graph, pad a shorter frame with all-zero digits. */
 TPCCLUS_API int tpcclus_run(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n,
                             const tpcclus_out* out, int mode, void* cuda_stream);
 

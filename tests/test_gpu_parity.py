@@ -696,6 +696,44 @@ def test_more_bins_than_k1_has_stages_for(tp, cuda_device):
             c.close()
 
 
+def test_run_under_cuda_graph_capture(tp, cuda_device):
+    """tpcclus_run only enqueues kernel launches on the caller's stream -- no allocation, no synchronisation, no
+    host-side read of device results -- so a caller can capture it into a CUDA graph and replay it (the launch-bound
+    small frames gain a fifth).  Replays with new digits in the same input buffer must give that frame's clusters."""
+    import torch
+    fa, fb = make_frame(0), make_frame(0, seed=4242)
+    n_max = max(fa.n_digits, fb.n_digits)
+    # graph arguments are frozen: the capture takes the larger digit count, the shorter frame is padded with
+    # all-zero digits (charge 0 at sector 0, row 0, pad 0, time 0: in range, ignored, Q4)
+    buf = torch.zeros(n_max, dtype=torch.int64, device=cuda_device)
+    c = tp.Clusterizer(fa.n_sectors, fa.n_rows, fa.n_time, fa.n_pads, n_max)
+    out = torch.empty((n_max, 32), dtype=torch.uint8, device=cuda_device)
+    for mode in (tp.MODE_DETERMINISTIC, tp.MODE_FAST):
+        buf.zero_()
+        buf[:fa.n_digits] = fa.digits.to(cuda_device)
+        c.run(buf, mode, clusters=out)          # warm-up outside the capture (module loading is lazy)
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            _, n_t, st_t = c.run(buf, mode, clusters=out)
+        for fr in (fa, fb, fa):
+            buf.zero_()
+            buf[:fr.n_digits] = fr.digits.to(cuda_device)
+            out.zero_()
+            g.replay()
+            torch.cuda.synchronize()
+            exp, st_exp = _oracle(fr.digits_numpy(), fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads)
+            n = int(n_t.item())
+            got = out[:n].cpu().numpy().view(tp.CLUSTER_DTYPE).reshape(-1)
+            assert n == len(exp) and int(st_t.item()) == st_exp
+            if mode == tp.MODE_DETERMINISTIC:
+                assert got.tobytes() == exp.tobytes()
+            else:
+                _check_fast(got, exp)
+        del g
+    c.close()
+
+
 def test_two_handles_two_streams_concurrently(tp, cuda_device):
     """Modules and constant blocks are per handle (R6, PAPER.md 81-85): two generic handles of
     different geometry AND thresholds run at the same time on two streams, many times over, and each
