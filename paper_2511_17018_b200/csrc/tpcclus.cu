@@ -258,7 +258,7 @@ const UnitInfo kUnits[U_COUNT_] = {TPC_UNIT_LIST(X)};
 // The kernels a handle launches (one slot each) and the unit that provides the slot's kernel for each
 // reading of the centre of gravity: {Q10, Q10' gated, Q10'' shared}.
 enum KernelId { K_RESET, K_PUBLISH, K_PART_COARSE, K_DIR_COUNT, K_DIR_SCAN, K_DIR_FILL, K_PART_FINE, K_TILES_FAST, K_TILES_FAST_E, K_TILES_DET,
-                K_TILES_DET_TEMP, K_TILES_DUMP, K_SCAN_LOCAL, K_SCAN_SUMS, K_EMIT_ORDERED, K_EMIT_PACKED, K_COUNT_ };
+                K_TILES_DET_TEMP, K_TILES_DET_TEMP_E, K_TILES_DUMP, K_SCAN_LOCAL, K_SCAN_SUMS, K_EMIT_ORDERED, K_EMIT_PACKED, K_COUNT_ };
 struct KernelInfo { const char* name[3]; UnitId unit[3]; int smem; };   // smem: 0 none/static, 1 K1, 2 one word per bin, 5 K5, 6 K6
 #define SAME3(x) {x, x, x}
 const KernelInfo kKernels[K_COUNT_] = {
@@ -271,6 +271,7 @@ const KernelInfo kKernels[K_COUNT_] = {
     {{"k_cluster_tiles_fast_e", "k_cluster_tiles_fast_gated_e", "k_cluster_tiles_fast_shared"}, {U_TILES_FAST, U_TILES_FAST_G, U_TILES_FAST_S}, 6},
     {{"k_cluster_tiles_det", "k_cluster_tiles_det_gated", "k_cluster_tiles_det_shared"}, {U_TILES_DET, U_TILES_DET_G, U_TILES_DET_S}, 6},
     {{"k_cluster_tiles_det_temp", "k_cluster_tiles_det_temp_gated", "k_cluster_tiles_det_temp_shared"}, {U_TILES_DET, U_TILES_DET_G, U_TILES_DET_S}, 6},
+    {{"k_cluster_tiles_det_temp_e", "k_cluster_tiles_det_temp_gated_e", "k_cluster_tiles_det_temp_shared"}, {U_TILES_DET, U_TILES_DET_G, U_TILES_DET_S}, 6},
     {SAME3("k_cluster_tiles_dump_map"), {U_TILES_DUMP, U_TILES_DUMP, U_TILES_DUMP_H5}, 6},
     {SAME3("k_scan_local"), SAME3(U_ORDER), 0}, {SAME3("k_scan_sums"), SAME3(U_ORDER), 0},
     {SAME3("k_emit_ordered"), SAME3(U_ORDER), 0}, {SAME3("k_emit_packed"), SAME3(U_ORDER), 0}};
@@ -781,17 +782,17 @@ static int run_impl(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n
   a.tile_base = p.tile_base; a.tile_cnt = p.tile_cnt; a.det_flag = p.det_flag;
   a.dmap = nullptr; a.row_off = p.row_off;
   void* ka[] = {&a};
+  // the readings Q10 and Q10' run with the emitter warp on sparse frames (K6): it only
+  // serves tiles of at most 256 records, so a frame that averages 512 or more per tile starts without it
+  const bool emitter = h->cog != 2 && n < 512ull * h->g.n_tiles;
   if (mode == TPCCLUS_MODE_FAST) {
-    // the readings Q10 and Q10' run with the emitter warp on sparse frames (K6): it only
-    // serves tiles of at most 256 records, so a frame that averages 512 or more per tile starts without it
-    const bool emitter = h->cog != 2 && n < 512ull * h->g.n_tiles;
     if ((rc = launch(h, emitter ? K_TILES_FAST_E : K_TILES_FAST, dim3(h->grid_k6), dim3(emitter ? TPC_K6_THREADS_E : TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
   } else {
     // ordered output (PAPER.md 47-50): runs into the temporary buffer, scan of the tile counts,
     // ordered copy.  Should the buffer be too small (more than max_digits/8 clusters) the flag is
     // set, K9 does nothing and the chained-scan K6 redoes the frame; otherwise that launch exits at once.
     const Geometry& g = h->g;
-    if ((rc = launch(h, K_TILES_DET_TEMP, dim3(h->grid_k6), dim3(TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
+    if ((rc = launch(h, emitter ? K_TILES_DET_TEMP_E : K_TILES_DET_TEMP, dim3(h->grid_k6), dim3(emitter ? TPC_K6_THREADS_E : TPC_K6_THREADS), h->smem_k6, st, ka))) return rc;
     u32 nt = g.n_tiles, nblk = g.n_scan_blocks;
     { void* s[] = {&p.tile_cnt, &p.tile_local, &p.block_sum, &nt};
       if ((rc = launch(h, K_SCAN_LOCAL, dim3(nblk), dim3(TPC_SCAN_THREADS), 0, st, s))) return rc; }

@@ -102,6 +102,7 @@ __host__ __device__ inline u32 tpc_k5_smem_bytes() { return (TPC_K5_BUF + 2u * T
 #endif
 #define TPC_K6_THREADS (TPC_K6_CONSUMERS + 32u)  // + the producer warp
 #define TPC_K6_THREADS_E (TPC_K6_THREADS + 32u)   // FAST kernels of the readings Q10 and Q10': + the emitter warp (K6, sparse tiles)
+#define TPC_K6_BLK 256u                          // clusters of the temporary buffer a CTA reserves at a time (DET, sparse tiles)
 #define TPC_K6_RING 64u                          // clusters in flight between the consumers and the emitter warp
 #ifndef TPC_K6_CAP
 #define TPC_K6_CAP 4096u                         // records staged per round (16 KB)
@@ -1047,7 +1048,7 @@ struct K6Smem {
   uint4* ring;     // [TPC_K6_RING][2] integer sums of a sparse tile's clusters on their way to the emitter warp (FAST)
   u32* rctl;       // [0] entries reserved  [1] entries consumed  [2] the consumers are done
 };
-// misc: [0] n_peaks  [3] first tile of the stage  [4] tiles in the stage  [5] row | sector << 8 |
+// misc: [0] n_peaks  [1],[2] DET: next and end of the CTA's block of the temporary buffer  [3] first tile of the stage  [4] tiles in the stage  [5] row | sector << 8 |
 //       n_pads << 16  [6] time of row 0 of the first tile  [7] its slab  [8+2m],[9+2m] offset and
 //       size (16-byte units) of tile m's records in `rec`
 __device__ __forceinline__ K6Smem k6_smem(u32* p) {
@@ -1175,6 +1176,7 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
   }
   for (u32 i = tid; i < TPC_K6_RING * 2u; i += TPC_K6_CONSUMERS) s.ring[i] = make_uint4(0u, 0u, 0u, 0u);
   if (tid < 4u) s.rctl[tid] = 0u;
+  if (tid == 0) { s.misc[1] = 0u; s.misc[2] = 0u; }   // DET: the CTA's block of the temporary buffer [next, end)
   __syncthreads();
 
   // The emitter warp (FAST, readings Q10 and Q10'): a sparse tile has its ~4 peaks in ONE warp, and the other
@@ -1184,7 +1186,10 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
   // is outside their barriers, finalises, reserves and writes.  No consumer ever waits for it: a warp that finds
   // the ring full emits its clusters itself, as the tiles with more than one record per thread always do.
   // The kernels *_e have the warp; the host launches them when the frame averages less than 512 records per tile.
-  static_assert(!EMIT || (MODE == TPC_MODE_FAST && COG != 2), "the emitter warp serves FAST and the readings Q10, Q10'");
+  // DET_TEMP has it as well: there the consumers know every cluster's place (the tile's run is cut from a block of
+  // the temporary buffer that the CTA holds, its rank comes from the warp that holds the tile's peaks), so the entry
+  // carries the place -- c0 = (Q | Spp << 15, Sp, St, place) -- and the emitter only finalises and stores.
+  static_assert(!EMIT || ((MODE == TPC_MODE_FAST || MODE == TPC_MODE_DET_TEMP) && COG != 2), "the emitter warp serves FAST and DET_TEMP of the readings Q10, Q10'");
   if (EMIT && tid >= TPC_K6_CONSUMERS + 32u) {
     const u32 lane = lane_id();
     u32 t = 0u;   // entries consumed
@@ -1206,6 +1211,16 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
       __syncwarp();
       t += nv;
       u64 base = 0ull;
+      if (MODE == TPC_MODE_DET_TEMP) {
+        if (lane == 0u) *(volatile u32*)&s.rctl[1] = t;   // the slots are free again
+        if (lane < nv) {
+          const u64 o = c0.w;
+          c0 = make_uint4(c0.x & 0x7FFFu, c0.y, c0.z, c0.x >> 15);
+          k6_finalise(c0, c1);
+          if (o < a.temp_cap) { a.temp[o * 2u] = c0; a.temp[o * 2u + 1u] = c1; }
+        }
+        continue;
+      }
       if (lane == 0u) { *(volatile u32*)&s.rctl[1] = t; base = atomicAdd(a.n_clusters, (u64)nv); }   // the slots are free again
       if (lane < nv) k6_finalise(c0, c1);
       base = __shfl_sync(0xFFFFFFFFu, base, 0);
@@ -1927,6 +1942,64 @@ __device__ __forceinline__ void k6_body(const K6Args& a, u32* smem) {
         zero_tile();
       continue;
     }
+    if (MODE == TPC_MODE_DET_TEMP && EMIT && total * 4u <= TPC_K6_CONSUMERS && npk <= 32u) {   // block-uniform
+      // A sparse tile in deterministic mode: its peaks sit in the lanes of warp 0, which settles everything the
+      // ordered output needs among its lanes -- the survivors (ballot), their ranks in (time, pad) order (the
+      // keys compared by shuffle), the tile's run (cut from the CTA's block of the temporary buffer: a global
+      // atomic per TPC_K6_BLK clusters, none per tile) -- and hands the clusters, with their places, to the
+      // emitter warp.  No survivor mask, no rank scan over the 134 rows, barriers F and G gone.
+      if (tid < 32u) {
+        const u32 lane = tid, lt = (1u << lane) - 1u;
+        const u32 e = lane < npk ? s.peaks[lane] : 0xFFFFu;
+        const bool keep = lane < npk && !suppressed(e);
+        const u32 m = __ballot_sync(0xFFFFFFFFu, keep);
+        const u32 count = (u32)__popc(m);
+        u32 rank = 0u;
+        for (u32 mm = m; mm != 0u; mm &= mm - 1u) rank += __shfl_sync(0xFFFFFFFFu, e, __ffs((int)mm) - 1) < e ? 1u : 0u;
+        u32 at = 0u, ridx = 0xFFFFFFFFu;
+        if (lane == 0u) {
+          u32 nx = s.misc[1], en = s.misc[2];
+          if (count != 0u && nx + count > en) {   // a new block (what is left of the old one stays unused)
+            const u64 g = atomicAdd(a.temp_cursor, (u64)TPC_K6_BLK);
+            if (g + TPC_K6_BLK > a.temp_cap) atomicOr(a.det_flag, 1u);
+            nx = (u32)(g < 0xFFFFFF00ull ? g : 0xFFFFFF00ull); en = nx + TPC_K6_BLK;   // (beyond the buffer: the flag is set, nothing is stored)
+          }
+          at = nx;
+          s.misc[1] = nx + count; s.misc[2] = en;
+          a.tile_base[tile] = at; a.tile_cnt[tile] = count;
+          if (count != 0u)
+            for (;;) {   // room in the emitter's ring?
+              const u32 h = *(volatile u32*)&s.rctl[0];
+              if (h + count - *(volatile u32*)&s.rctl[1] > TPC_K6_RING) break;
+              if (atomicCAS(&s.rctl[0], h, h + count) == h) { ridx = h; break; }
+            }
+        }
+        at = __shfl_sync(0xFFFFFFFFu, at, 0);
+        ridx = __shfl_sync(0xFFFFFFFFu, ridx, 0);
+        if (keep) {
+          cog_int(e, o0, o1);
+          if (ridx == 0xFFFFFFFFu) k6_finalise(o0, o1);   // the ring is full: this warp writes them itself, after barrier E
+          else {
+            const u32 i = ridx + __popc(m & lt), slot = i % TPC_K6_RING;
+            o0 = make_uint4(o0.x | (o0.w << 15), o0.y, o0.z, at + rank);
+            o1.w = i / TPC_K6_RING + 1u;
+            s.ring[2u * slot] = o0;
+            __threadfence_block();
+            s.ring[2u * slot + 1u] = o1;
+          }
+        }
+        csync();   // E
+        if (keep && ridx == 0xFFFFFFFFu) emit((u64)(at + rank), o0, o1);
+      } else
+        csync();   // E
+      if (my_r != 0u) {
+        const u32 tl = k6_row(my_r, sl), pad = my_r & 0xFFu;
+        s.tile[tl * pitch + pad + TPC_PG] = 0;
+        s.pmask[tl * TPC_K6_PMW + ((pad + TPC_PG) >> 5)] = 0u;
+      }
+      if (tid == 0) s.misc[0] = 0u;
+      continue;
+    }
     bool survived = false;
     for (u32 i = tid; i < npk; i += TPC_K6_CONSUMERS) {
       const u32 e = s.peaks[i];
@@ -2051,6 +2124,7 @@ TPC_K6_ENTRY(k_cluster_tiles_fast_e, TPC_MODE_FAST, 0, true, )
 #if TPC_UNITS & TPC_U_TILES_DET
 TPC_K6_ENTRY(k_cluster_tiles_det, TPC_MODE_DET, 0, false, TPC_K6_IF_FLAG)
 TPC_K6_ENTRY(k_cluster_tiles_det_temp, TPC_MODE_DET_TEMP, 0, false, )
+TPC_K6_ENTRY(k_cluster_tiles_det_temp_e, TPC_MODE_DET_TEMP, 0, true, )
 #endif
 #if TPC_UNITS & TPC_U_TILES_DUMP
 TPC_K6_ENTRY(k_cluster_tiles_dump_map, TPC_MODE_DUMP_MAP, 0, false, )
@@ -2063,6 +2137,7 @@ TPC_K6_ENTRY(k_cluster_tiles_fast_gated_e, TPC_MODE_FAST, 1, true, )
 #if TPC_UNITS & TPC_U_TILES_DET_G
 TPC_K6_ENTRY(k_cluster_tiles_det_gated, TPC_MODE_DET, 1, false, TPC_K6_IF_FLAG)
 TPC_K6_ENTRY(k_cluster_tiles_det_temp_gated, TPC_MODE_DET_TEMP, 1, false, )
+TPC_K6_ENTRY(k_cluster_tiles_det_temp_gated_e, TPC_MODE_DET_TEMP, 1, true, )
 #endif
 // reading Q10'' (TPCCLUS_COG_SHARED): these units -- and the partition units of such a handle -- are compiled with TPC_HALO = 5
 #if TPC_UNITS & TPC_U_TILES_FAST_S
