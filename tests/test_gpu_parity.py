@@ -353,6 +353,23 @@ def test_det_fallback_when_run_buffer_is_too_small(tp, cuda_device):
     fast, n, st = c.run_sync(_digits_tensor(d, cuda_device), tp.MODE_FAST)
     _check_fast(fast, exp)
     c.close()
+    # the same through the sparse-frame kernel (emitter warp): tiles of 32 isolated digits -- ranked inside one warp, their
+    # runs cut from the CTA's block of the temporary buffer -- in so many tiles that the blocks run past the buffer's end
+    T, P, R = 16000, 64, 40
+    rows = np.zeros((R, T // 16, P // 16), dtype=t1.DIGIT)
+    rows["time"] = (16 * np.arange(T // 16, dtype=np.uint16) + 5)[None, :, None]
+    rows["pad"] = (16 * np.arange(P // 16, dtype=np.uint8) + 3)[None, None, :]
+    rows["row"] = np.arange(R, dtype=np.uint8)[:, None, None]
+    rows["charge"] = 50
+    d = rows.reshape(-1)
+    d = d[np.random.default_rng(37).permutation(len(d))]
+    exp, _ = _oracle(d, 1, R, T, [P] * R)
+    assert len(exp) == len(d) == 160000
+    c = tp.Clusterizer(1, R, T, [P] * R, len(d))
+    det, n, st = c.run_sync(_digits_tensor(d, cuda_device), tp.MODE_DETERMINISTIC)
+    assert c.det_fallback() and st == 0 and n == len(exp)
+    assert det.tobytes() == exp.tobytes()
+    c.close()
     fr = make_frame(0)
     c = tp.Clusterizer(fr.n_sectors, fr.n_rows, fr.n_time, fr.n_pads, fr.n_digits)
     c.run_sync(fr.digits.to(cuda_device), tp.MODE_DETERMINISTIC)
