@@ -649,8 +649,8 @@ def test_sparse_tiles_through_the_emitter_ring(tp, cuda_device):
     rows = []
     for r in (0, 1, 2):
         for sl in range(n_slabs):
-            kind = (sl + r) % 5
-            n = [240, 0, 3, 120, 30][kind] if sl else 1
+            kind = (sl + r) % 7
+            n = [240, 0, 3, 120, 30, 32, 33][kind] if sl else 1   # (32 / 33: either side of the one-warp limit of the deterministic path)
             lat = [(t, p) for t in range(1, 127, 3) for p in range(1, P - 1, 3)]   # 42 x 33 sites, pairwise distance >= 3
             for k in rng.choice(len(lat), size=n, replace=False):
                 t, p = lat[k]
