@@ -741,7 +741,10 @@ int enqueue_binning(tpcclus_handle* h, const tpcclus_digit* d_digits, uint64_t n
     if ((rc = launch(h, K_DIR_COUNT, dim3(g.g1), dim3(TPC_SCAN_THREADS), smem_nb, st, a))) return rc; }
   { void* a[] = {&p.bin_chunk_start, &p.batch_start, &p.batch_bin};
     if ((rc = launch(h, K_DIR_SCAN, dim3(1), dim3(TPC_SCAN_THREADS), smem_nb, st, a))) return rc; }
-  { void* a[] = {&p.dir, &p.used, &slice_cap, &p.slice_cnt, &p.bin_chunk_start, &p.chunk_list};
+  // K4 fills the chunk lists range of bins by range of bins, one pass over the directory per 64 MB of lists (4 bytes per chunk)
+  u32 k4_pass = (u32)((4ull * (n / TPC_CHUNK + (u64)g.prm.n_bins * g.g1) + (64ull << 20) - 1ull) / (64ull << 20));
+  k4_pass = k4_pass < 1u ? 1u : k4_pass > 4u ? 4u : k4_pass;
+  { void* a[] = {&p.dir, &p.used, &slice_cap, &p.slice_cnt, &p.bin_chunk_start, &p.chunk_list, &k4_pass};
     if ((rc = launch(h, K_DIR_FILL, dim3(g.g1), dim3(TPC_SCAN_THREADS), smem_nb, st, a))) return rc; }
   { void* a[] = {&p.pool, &p.dir, &p.chunk_list, &p.bin_chunk_start, &p.batch_start, &p.batch_bin, &p.blob, &p.blob_cursor, &blob_cap, &p.idx, &status};
     if ((rc = launch(h, K_PART_FINE, dim3(h->grid_k5), dim3(TPC_K5_THREADS), h->smem_k5, st, a))) return rc; }
