@@ -8,7 +8,8 @@ wavefronts and bank conflicts, instruction counts, the six largest stall reasons
 (dram__bytes_read.sum + dram__bytes_write.sum per launch and kernel, with the sha256 of the kernel
 text it was measured on: bench.py reports `traffic` from it only while that text is unchanged) and,
 with --launches, profiles/<tag>_launches_summary.txt (mean device time and share per kernel from the
-`--metrics gpu__time_duration.sum` launch list).  Reads reports only; runs no kernel.
+`--metrics gpu__time_duration.sum` launch list), with --top-lines N profiles/<tag>_top_lines.txt (the hottest source
+lines per kernel from the source page).  Reads reports only; runs no kernel.
 """
 from __future__ import annotations
 
@@ -95,6 +96,47 @@ def summarise_launches(path: str, tag: str) -> None:
             f.write("%s, %d, %.4f, %.1f %%\n" % (n, len(x), sum(x) / len(x) / 1e6, 100 * sum(x) / len(x) / tot))
 
 
+def summarise_lines(rep: str, tag: str, top: int) -> None:
+    """profiles/<tag>_top_lines.txt: per kernel of the report, the source lines of the kernel text with the most executed
+    warp instructions (share of instructions, of stall samples and of shared-memory wavefronts, ideal wavefronts beside
+    them).  Needs a capture with --import-source on of a build with -lineinfo; the line numbers are those of the kernel
+    text whose sha256 the traffic json of the same tag records."""
+    raw = subprocess.run(["ncu", "-i", rep, "--page", "source", "--csv", "--print-source", "cuda,sass"], capture_output=True, text=True, check=True).stdout
+
+    def num(x):
+        try:
+            return float(x)
+        except ValueError:
+            return 0.0
+    cur, hdr, idx, data = None, None, None, collections.OrderedDict()
+    for r in csv.reader(raw.splitlines()):
+        if len(r) >= 2 and r[0] == "Function Name":
+            cur = r[1]
+            continue
+        if r and r[0] == "Line No":
+            hdr, idx = r, {h: i for i, h in enumerate(r)}
+            continue
+        if cur is None or hdr is None or len(r) < len(hdr) or r[0] == "":
+            continue
+        d = data.setdefault(cur, {}).setdefault(int(r[0]), [r[1], 0.0, 0.0, 0.0, 0.0])
+        for j, col in ((1, "Instructions Executed"), (2, "# Samples"), (3, "L1 Wavefronts Shared"), (4, "L1 Wavefronts Shared Ideal")):
+            if col in idx:   # (a kernel without shared memory has no wavefront columns)
+                d[j] += num(r[idx[col]])
+    out = ["ncu --page source of %s: the %d source lines with the most executed warp instructions per kernel" % (os.path.basename(rep), top),
+           "(line of csrc/tpcclus_kernels.cuh or of a CUDA header, share of the kernel's instructions / stall samples / shared-memory wavefronts (ideal))", ""]
+    for k, lines in data.items():
+        ti = sum(v[1] for v in lines.values()) or 1.0
+        ts = sum(v[2] for v in lines.values()) or 1.0
+        tw = sum(v[3] for v in lines.values()) or 1.0
+        out.append("== %s: %.3e warp instructions, %.3e shared-memory wavefronts" % (k, ti, tw))
+        for ln, v in sorted(lines.items(), key=lambda kv: -kv[1][1])[:top]:
+            out.append("%5d  inst %5.1f %%  samples %5.1f %%  wavefronts %5.1f %% (ideal %4.1f %%) | %s" %
+                       (ln, 100 * v[1] / ti, 100 * v[2] / ts, 100 * v[3] / tw, 100 * v[4] / tw, v[0].strip()[:110]))
+        out.append("")
+    with open(os.path.join(ROOT, "profiles", "%s_top_lines.txt" % tag), "w") as f:
+        f.write("\n".join(out) + "\n")
+
+
 SASS_PATTERNS = ["UBLKCP", "UBLKPF", "SYNCS", "FENCE.VIEW.ASYNC", "STG.E.ENL2.256", "LDG.E.NA", "VIMNMX", "ATOMS", "ATOMG", "REDG",
                  "VOTE", "SHFL", "BAR.", "LDS", "STS", "HMMA", "UTC"]
 
@@ -131,6 +173,7 @@ def main() -> None:
     ap.add_argument("--launches")
     ap.add_argument("--note", default="CFG[4] shuffled FAST generic")
     ap.add_argument("--sass", action="store_true", help="write profiles/<tag>_sass_summary.txt from build/unit_*.cubin")
+    ap.add_argument("--top-lines", type=int, default=0, help="also write profiles/<tag>_top_lines.txt: the N hottest source lines per kernel")
     a = ap.parse_args()
     if a.sass:
         summarise_sass(a.tag)
@@ -138,6 +181,8 @@ def main() -> None:
         print(json.dumps(summarise_rep(a.rep, a.tag, a.note)["traffic_bytes"]))
     if a.launches:
         summarise_launches(a.launches, a.tag)
+    if a.rep and a.top_lines:
+        summarise_lines(a.rep, a.tag, a.top_lines)
 
 
 if __name__ == "__main__":
